@@ -1,0 +1,295 @@
+"""ctypes harness around the ORACLE (oracle/orc_main.cpp) — TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this package.  Nothing under paper_1503_01722_b200/ imports it, and it imports nothing from the CUDA
+path (the seeded input generators in paper_1503_01722_b200/workloads.py are handed in by callers).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import multiprocessing as mp
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+TABLE_IDS = {"mu_tot": 0, "mu_C": 1, "mu_pp": 2, "R": 3, "L": 4, "S_hard": 5, "S_M": 6, "S_max": 7, "K1": 8,
+             "mu_maj": 9}
+STAT_NAMES = ["e_src", "e_dep", "e_esc", "e_cutdep", "n_hist", "n_flight", "n_fict", "n_compton", "n_pair",
+              "n_pe", "n_estep", "n_moller", "n_brems", "n_sec_e", "n_sec_g", "path_e", "lim_vox", "lim_maxs",
+              "lim_maxe", "lim_range", "lim_event", "max_ledger_rel"]
+
+
+class _Material(C.Structure):
+    _fields_ = [("n_elem", C.c_int32), ("Z", C.POINTER(C.c_int32)), ("A", C.POINTER(C.c_float)),
+                ("w", C.POINTER(C.c_float)), ("I_eV", C.c_float), ("rho_nominal", C.c_float)]
+
+
+class _Params(C.Structure):
+    _fields_ = [("e_cut_MeV", C.c_float), ("g_cut_MeV", C.c_float), ("e_max_MeV", C.c_float),
+                ("n_grid", C.c_int32), ("d_maxs_cm", C.c_float), ("f_maxe", C.c_float), ("flags", C.c_uint32)]
+
+
+class _Beam(C.Structure):
+    _fields_ = [("particle", C.c_int32), ("shape", C.c_int32), ("entry_cm", C.c_float * 3),
+                ("axis", C.c_float * 3), ("ssd_cm", C.c_float), ("field_cm", C.c_float * 2),
+                ("n_nodes", C.c_int32), ("E_nodes_MeV", C.POINTER(C.c_float)),
+                ("pdf_nodes", C.POINTER(C.c_float))]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.orc_eval.restype = C.c_double
+        _lib.orc_eval.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double]
+        _lib.orc_lerp.restype = C.c_double
+        _lib.orc_lerp.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double]
+        _lib.orc_inv_range.restype = C.c_double
+        _lib.orc_inv_range.argtypes = [C.c_void_p, C.c_int, C.c_double]
+        _lib.orc_material_scalar.restype = C.c_double
+        _lib.orc_material_scalar.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        _lib.orc_sigma_pp_atom.restype = C.c_double
+        _lib.orc_sigma_pp_atom.argtypes = [C.c_int, C.c_double]
+        _lib.orc_contract_ln.restype = C.c_float
+        _lib.orc_contract_ln.argtypes = [C.c_float]
+        _lib.orc_destroy.argtypes = [C.c_void_p]
+        _lib.orc_set_flags.argtypes = [C.c_void_p, C.c_uint32]
+    return _lib
+
+
+def _fp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_float))
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _beam_struct(beam):
+    keep = [np.ascontiguousarray(beam["E_nodes_MeV"], np.float32), np.ascontiguousarray(beam["pdf_nodes"], np.float32)]
+    b = _Beam(int(beam["particle"]), int(beam["shape"]), (C.c_float * 3)(*beam["entry_cm"]),
+              (C.c_float * 3)(*beam["axis"]), float(beam["ssd_cm"]), (C.c_float * 2)(*beam["field_cm"]),
+              len(keep[0]), _fp(keep[0]), _fp(keep[1]))
+    return b, keep
+
+
+def philox(ctr, key):
+    c = (C.c_uint32 * 4)(*ctr)
+    k = (C.c_uint32 * 2)(*key)
+    o = (C.c_uint32 * 4)()
+    lib().orc_philox(c, k, o)
+    return [int(x) for x in o]
+
+
+def contract_ln(x):
+    return float(lib().orc_contract_ln(C.c_float(x)))
+
+
+def sigma_pp_reduced(Z, k):
+    """sigma_pair / (alpha r_e^2 Z^2)."""
+    return lib().orc_sigma_pp_atom(int(Z), float(k))
+
+
+class Oracle:
+    """One phantom + one set of tables.  Mirrors the C-ABI calls (create / build_tables / run)."""
+
+    def __init__(self, phantom, materials=None, params=None):
+        L = lib()
+        self._ph = phantom
+        self.dims = np.ascontiguousarray(phantom["dims"], np.int32)
+        self.nvox = int(np.prod(self.dims))
+        self._mat = np.ascontiguousarray(phantom["material"], np.uint8)
+        self._rho = np.ascontiguousarray(phantom["density"], np.float32)
+        vox = np.ascontiguousarray(phantom["voxel_cm"], np.float32)
+        org = np.ascontiguousarray(phantom["origin_cm"], np.float32)
+        h = C.c_void_p()
+        rc = L.orc_create(self._mat.ctypes.data_as(C.c_void_p), _fp(self._rho),
+                          self.dims.ctypes.data_as(C.c_void_p), _fp(vox), _fp(org), C.byref(h))
+        if rc:
+            raise ValueError(f"orc_create failed ({rc})")
+        self._h = h
+        self._materials = self._params = None
+        if materials is not None:
+            self.build_tables(materials, params)
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            lib().orc_destroy(self._h)
+            self._h = None
+
+    def build_tables(self, materials, params):
+        self._materials, self._params = materials, dict(params)
+        keep, arr = [], (_Material * len(materials))()
+        for i, m in enumerate(materials):
+            Z = np.ascontiguousarray(m["Z"], np.int32)
+            A = np.ascontiguousarray(m["A"], np.float32)
+            w = np.ascontiguousarray(m["w"], np.float32)
+            keep += [Z, A, w]
+            arr[i] = _Material(len(Z), Z.ctypes.data_as(C.POINTER(C.c_int32)), _fp(A), _fp(w), m["I_eV"],
+                               m["rho_nominal"])
+        p = _Params(params["e_cut_MeV"], params["g_cut_MeV"], params["e_max_MeV"], params["n_grid"],
+                    params["d_maxs_cm"], params["f_maxe"], params["flags"])
+        rc = lib().orc_build_tables(self._h, arr, len(materials), C.byref(p))
+        if rc:
+            raise ValueError(f"orc_build_tables failed ({rc})")
+
+    def set_flags(self, flags):
+        self._params["flags"] = int(flags)
+        lib().orc_set_flags(self._h, int(flags))
+
+    # -- tables / closed forms ---------------------------------------------------------------
+    def grid(self):
+        o = np.zeros(4)
+        lib().orc_grid(self._h, _dp(o))
+        return {"lnE0": o[0], "dln": o[1], "N": int(o[2]), "k_cut": int(o[3])}
+
+    def energies(self):
+        g = self.grid()
+        return np.exp(g["lnE0"] + g["dln"] * np.arange(g["N"]))
+
+    def table(self, name, m=0):
+        g = self.grid()
+        o = np.zeros(g["N"])
+        rc = lib().orc_table(self._h, int(m), TABLE_IDS[name], _dp(o))
+        if rc:
+            raise ValueError(f"orc_table failed ({rc})")
+        return o
+
+    def eval(self, which, E, arg=0.0, m=0):
+        ids = {"sigma_kn": 0, "mu_C": 1, "mu_pe": 2, "mu_pp": 3, "L_col": 4, "L_rad": 5, "S_M": 6, "S_br": 7,
+               "K1": 8, "delta": 9, "brems_kdsdk": 10, "moller_dsde": 11}
+        return lib().orc_eval(self._h, int(m), ids[which], float(E), float(arg))
+
+    def lerp(self, name, E, m=0):
+        return lib().orc_lerp(self._h, int(m), TABLE_IDS[name], float(E))
+
+    def inv_range(self, Rt, m=0):
+        return lib().orc_inv_range(self._h, int(m), float(Rt))
+
+    def material_scalar(self, name, m=0):
+        return lib().orc_material_scalar(self._h, int(m), {"ne": 0, "ZA": 1, "Cbr": 2, "Lscr": 3}[name])
+
+    # -- transport ------------------------------------------------------------------------------
+    def run_edep(self, beam, n_total, seed, n_batches, h0=0, h1=None, first=False):
+        """Energy deposited per batch grid [B, nvox] (MeV, fp64) for histories [h0, h1) + stats dict.
+        first=True also returns (voxel, channel) of each primary photon's first real interaction."""
+        h1 = n_total if h1 is None else h1
+        b, keep = _beam_struct(beam)
+        edep = np.zeros((n_batches, self.nvox))
+        st = np.zeros(lib().orc_n_stats())
+        fv = np.zeros(h1 - h0, np.int32) if first else None
+        fc = np.zeros(h1 - h0, np.int32) if first else None
+        rc = lib().orc_run(self._h, C.byref(b), C.c_uint64(h0), C.c_uint64(h1), C.c_uint64(n_total),
+                           C.c_uint64(seed), int(n_batches), _dp(edep), _dp(st),
+                           fv.ctypes.data_as(C.c_void_p) if first else None,
+                           fc.ctypes.data_as(C.c_void_p) if first else None)
+        if rc:
+            raise ValueError(f"orc_run failed ({rc})")
+        if first:
+            return edep, dict(zip(STAT_NAMES, st)), fv, fc
+        return edep, dict(zip(STAT_NAMES, st))
+
+    def finalize(self, edep, n_total):
+        B = edep.shape[0]
+        dose, sig = np.zeros(self.nvox), np.zeros(self.nvox)
+        lib().orc_finalize(self._h, _dp(np.ascontiguousarray(edep)), C.c_uint64(n_total), int(B), _dp(dose), _dp(sig))
+        return dose, sig
+
+    def run(self, beam, n_histories, seed, n_batches, workers=1):
+        """dose, sigma (MeV/g per history), stats.  workers>1 shards disjoint history ranges over
+        processes (valid because every stream is keyed by the history index)."""
+        if workers <= 1:
+            edep, st = self.run_edep(beam, n_histories, seed, n_batches)
+        else:
+            edep, st = _run_sharded(self._ph, self._materials, self._params, beam, n_histories, seed, n_batches,
+                                    workers)
+        dose, sig = self.finalize(edep, n_histories)
+        return dose, sig, st
+
+    def run_atten(self, beam, n, seed, tables_f32):
+        """fp32 contract path (R20).  tables_f32: dict(lnE0, inv_dln, mu_maj[N], mu_tot/mu_C/mu_pp[n_mat,N])."""
+        b, keep = _beam_struct(beam)
+        t = {k: np.ascontiguousarray(tables_f32[k], np.float32) for k in ("mu_maj", "mu_tot", "mu_C", "mu_pp")}
+        n_mat, N = t["mu_tot"].shape
+        vox = np.zeros(n, np.int32)
+        ch = np.zeros(n, np.uint8)
+        fl = np.zeros(n, np.uint32)
+        rc = lib().orc_run_atten(self._h, C.byref(b), C.c_uint64(n), C.c_uint64(seed), int(N), int(n_mat),
+                                 C.c_float(tables_f32["lnE0"]), C.c_float(tables_f32["inv_dln"]),
+                                 _fp(t["mu_maj"]), _fp(t["mu_tot"]), _fp(t["mu_C"]), _fp(t["mu_pp"]),
+                                 vox.ctypes.data_as(C.c_void_p), ch.ctypes.data_as(C.c_void_p),
+                                 fl.ctypes.data_as(C.c_void_p))
+        if rc:
+            raise ValueError(f"orc_run_atten failed ({rc})")
+        return vox, ch, fl
+
+    def photon_tables_f32(self):
+        """The oracle's own photon tables rounded to fp32, in the layout run_atten takes."""
+        g = self.grid()
+        nm = len(self._materials)
+        out = {"lnE0": np.float32(g["lnE0"]), "inv_dln": np.float32(1.0 / g["dln"]),
+               "mu_maj": self.table("mu_maj").astype(np.float32)}
+        for k in ("mu_tot", "mu_C", "mu_pp"):
+            out[k] = np.stack([self.table(k, m) for m in range(nm)]).astype(np.float32)
+        return out
+
+    def sample_source(self, beam, n, seed):
+        b, keep = _beam_struct(beam)
+        o = np.zeros((n, 7))
+        lib().orc_sample_source(self._h, C.byref(b), C.c_uint64(n), C.c_uint64(seed), _dp(o))
+        return o
+
+    def sample_brems(self, T0, n, seed, m=0):
+        o = np.zeros(n)
+        lib().orc_sample_brems(self._h, int(m), C.c_double(T0), C.c_uint64(n), C.c_uint64(seed), _dp(o))
+        return o
+
+
+def sample_kn(E, n, seed=1):
+    o = np.zeros((n, 4))
+    lib().orc_sample_kn(C.c_double(E), C.c_uint64(n), C.c_uint64(seed), _dp(o))
+    return o
+
+
+def sample_moller(T0, e_cut, n, seed=1):
+    o = np.zeros((n, 3))
+    lib().orc_sample_moller(C.c_double(T0), C.c_double(e_cut), C.c_uint64(n), C.c_uint64(seed), _dp(o))
+    return o
+
+
+def sample_ms(a, n, seed=1):
+    o = np.zeros(n)
+    lib().orc_sample_ms(C.c_double(a), C.c_uint64(n), C.c_uint64(seed), _dp(o))
+    return o
+
+
+# -- sharding over host cores -------------------------------------------------------------------
+def _shard(args):
+    ph, mats, par, beam, n_total, seed, B, h0, h1 = args
+    o = Oracle(ph, mats, par)
+    return o.run_edep(beam, n_total, seed, B, h0, h1)
+
+
+def _run_sharded(ph, mats, par, beam, n_total, seed, B, workers):
+    # many small contiguous chunks, interleaved, so that every worker ends at about the same time
+    n_chunks = workers * 8
+    edges = np.linspace(0, n_total, n_chunks + 1).astype(np.int64)
+    jobs = [(ph, mats, par, beam, n_total, seed, B, int(edges[i]), int(edges[i + 1])) for i in range(n_chunks)
+            if edges[i + 1] > edges[i]]
+    ctx = mp.get_context("fork")
+    with ctx.Pool(workers) as pool:
+        res = pool.map(_shard, jobs, chunksize=1)
+    edep = sum(r[0] for r in res)
+    st = {k: (max(r[1][k] for r in res) if k == "max_ledger_rel" else sum(r[1][k] for r in res)) for k in STAT_NAMES}
+    return edep, st
+
+
+def host_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
