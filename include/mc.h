@@ -1,0 +1,182 @@
+/* mc.h — C ABI of the B200-native coupled photon–electron Monte Carlo dose engine.
+ *
+ * The calls follow the paper's statement of the problem (arxiv 1503.01722, "oclMC"):
+ *   - a voxelised phantom, "each voxel was assigned to a density value and a material type"
+ *     (§2.1)                                            -> mc_create
+ *   - "physics data needed by oclMC based on a user-defined material composition", cut-offs and
+ *     maximum step sizes are user defined    -> mc_build_tables / mc_set_tables
+ *   - a point source with an energy or spectrum, a field at the surface, an SSD;
+ *     result "in a unit of MeV/g per source particle" with its uncertainty sigma_D
+ *                                                                     -> mc_run
+ * Transport: photons by Woodcock tracking with Compton / pair / photoelectric events,
+ * electrons and positrons by a Class II condensed-history scheme with
+ * d = min[d_vox, d_maxs, d_maxe, d_event], secondaries on per-type stacks
+ * (PAPER.md:60, :72), dose by atomic adds.  Readings of everything the paper leaves
+ * open are listed in DESIGN.md (R1..R26).
+ *
+ * Conventions
+ *   - Every call returns an mc_status and never throws or aborts; mc_last_error() gives a message.
+ *   - Plain pointers and sizes only.  Unless stated otherwise an input pointer is HOST memory that is
+ *     copied during the call (the caller keeps ownership); an output pointer may be HOST or DEVICE
+ *     memory (resolved through unified addressing) and is written before the call returns.
+ *   - The context owns all device memory it allocates.  One context = one phantom on the current
+ *     CUDA device; calls on one context must not overlap.  Work is issued on the context's stream
+ *     (default: the legacy default stream; see mc_set_stream) and the call synchronises that stream
+ *     before returning.
+ *   - Volume layout: x fastest, i = ix + nx*(iy + ny*iz).  Units: MeV, cm, g/cm^3.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns MC_ERR_CUDA.
+ */
+#ifndef MC_B200_H
+#define MC_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mc_ctx mc_ctx; /* opaque, owned by the library */
+
+typedef enum {
+    MC_OK = 0,
+    MC_ERR_INVALID_ARG = 1,
+    MC_ERR_STATE = 2,          /* e.g. mc_run before tables exist                        */
+    MC_ERR_ENERGY_RANGE = 3,   /* beam energy above the table grid (e_max_MeV)           */
+    MC_ERR_QUEUE_OVERFLOW = 4, /* a particle queue overflowed: results invalid, none returned */
+    MC_ERR_OOM = 5,
+    MC_ERR_CUDA = 6
+} mc_status;
+
+/* One material by elemental composition.  Z, A, w: n_elem entries; w = mass fractions
+ * (normalised by the library).  I_eV = mean excitation energy; rho_nominal (g/cm^3) enters only the
+ * density-effect correction (R22). */
+typedef struct {
+    int32_t n_elem;
+    const int32_t *Z;
+    const float *A;
+    const float *w;
+    float I_eV;
+    float rho_nominal;
+} mc_material;
+
+/* flags */
+#define MC_FLAG_NO_HARD_EVENTS 1u     /* no Moller / bremsstrahlung events (d_event = inf)        */
+#define MC_FLAG_NO_MS 2u              /* no multiple-scattering deflection                        */
+#define MC_FLAG_LOCAL_SECONDARIES 4u  /* secondaries deposit their energy where they are born     */
+
+/* Cut-offs and step limits (PAPER.md:39 "user defined maximum step size", :86 cut-off energies).
+ * e_cut_MeV: electron absorption energy = Moller delta-ray threshold; g_cut_MeV: photon absorption
+ * energy = bremsstrahlung production threshold (R1).  e_max_MeV: top of the energy grid.
+ * n_grid: nodes of the uniform ln E grid (8..1024).  d_maxs_cm: geometric step limit; f_maxe:
+ * maximum fractional CSDA energy loss per step (R2). */
+typedef struct {
+    float e_cut_MeV, g_cut_MeV, e_max_MeV;
+    int32_t n_grid;
+    float d_maxs_cm, f_maxe;
+    uint32_t flags;
+} mc_params;
+
+#define MC_PHOTON 0
+#define MC_ELECTRON (-1)
+#define MC_POSITRON 1
+#define MC_SHAPE_PENCIL 0     /* all histories start at entry_cm along axis                              */
+#define MC_SHAPE_POINT_RECT 1 /* point source at ssd_cm behind entry_cm; (x, y) uniform over field_cm in
+                                 the surface plane z = entry_cm[2]; axis must be +z (R13)       */
+
+/* Beam.  Spectrum: n_nodes == 1 -> monoenergetic E_nodes_MeV[0]; otherwise a
+ * piecewise-linear pdf through (E_nodes_MeV[j], pdf_nodes[j]), nodes ascending. */
+typedef struct {
+    int32_t particle;
+    int32_t shape;
+    float entry_cm[3];
+    float axis[3];
+    float ssd_cm;
+    float field_cm[2];
+    int32_t n_nodes;
+    const float *E_nodes_MeV;
+    const float *pdf_nodes;
+} mc_beam;
+
+/* Counters of the last mc_run / mc_run_range on this context. */
+typedef struct {
+    uint64_t n_histories;
+    uint64_t n_electron_steps;   /* condensed-history steps (electrons + positrons)            */
+    uint64_t n_photon_flights;   /* Woodcock flights                                           */
+    uint64_t n_fictitious;       /* flights ending in a fictitious interaction                 */
+    uint64_t n_compton, n_pair, n_photoelectric;
+    uint64_t n_moller, n_brems;
+    uint64_t n_secondary_electrons, n_secondary_photons; /* queued (not counting local deposits) */
+    uint64_t n_dose_atomics;     /* red.global.add.f32 issued                                  */
+    uint64_t n_kernel_launches;  /* transport + finalize kernels launched                      */
+    double e_source_MeV, e_deposited_MeV, e_escaped_MeV; /* energy ledger                      */
+    double transport_ms;         /* CUDA-event time of the transport launches                  */
+    double electron_kernel_ms, photon_kernel_ms; /* split of transport_ms by kernel            */
+} mc_stats;
+
+/* mc_create — copy the phantom to the device.
+ * material_idx, density_gcc: nx*ny*nz entries (host), density > 0.  dims > 0, voxel_cm > 0.
+ * origin_cm: coordinates of the low corner of voxel (0,0,0).  *out receives the context. */
+mc_status mc_create(const uint8_t *material_idx, const float *density_gcc, const int32_t dims[3],
+                    const float voxel_cm[3], const float origin_cm[3], mc_ctx **out);
+void mc_destroy(mc_ctx *ctx);
+
+/* mc_build_tables — closed-form physics tables per material on a uniform ln E grid, the photon
+ * Woodcock majorant from the phantom.  Re-callable.
+ * Errors: a voxel's material index >= n_mats, bad cut-offs / grid -> MC_ERR_INVALID_ARG. */
+mc_status mc_build_tables(mc_ctx *ctx, const mc_material *mats, int32_t n_mats, const mc_params *params);
+
+/* Table access, fp32 as used on the device.  which: 0 mu_tot 1 mu_C 2 mu_pp (cm^2/g) 3 R (g/cm^2)
+ * 4 L (MeV cm^2/g) 5 Sigma_hard 6 Sigma_Moller 7 Sigma_max 8 K1 (cm^2/g); material = -1, which = 9:
+ * photon majorant mu_maj (1/cm).  out: n_grid floats (host). */
+mc_status mc_export_table(const mc_ctx *ctx, int32_t material, int32_t which, float *out);
+/* grid[0] = ln E_0, grid[1] = delta ln E, grid[2] = n_grid, grid[3] = node index of e_cut. */
+mc_status mc_export_grid(const mc_ctx *ctx, double grid[4]);
+/* Replace the PHOTON tables by user-supplied data ("physics data ... stored in a database",
+ * PAPER.md:31): mu_maj[n_grid] (1/cm) and mu_tot / mu_C / mu_pp [n_mats][n_grid] (cm^2/g) on the grid
+ * ln E_j = lnE0 + j/inv_dln.  Requires a previous mc_build_tables with the same n_mats and n_grid. */
+mc_status mc_set_photon_tables(mc_ctx *ctx, float lnE0, float inv_dln, const float *mu_maj,
+                               const float *mu_tot, const float *mu_C, const float *mu_pp);
+
+/* mc_run — simulate histories 0..n_histories-1 (n_histories < 2^32) of the beam with Philox4x32-10
+ * streams keyed by (seed, history index), scoring into n_batches (>= 2, <= n_histories) per-batch
+ * fp32 grids (batch of history h = floor(h*n_batches/n_histories)).
+ * dose_out, sigma_out: nvox floats each (host or device): mean dose and standard error of the batch
+ * means, MeV/g per history (R17, R18).  Results are deterministic per history; grid sums
+ * are reproducible only to fp32 summation order. */
+mc_status mc_run(mc_ctx *ctx, const mc_beam *beam, uint64_t n_histories, uint64_t seed, int32_t n_batches,
+                 float *dose_out, float *sigma_out);
+
+/* mc_run_range — the shard of mc_run one GPU of several computes: histories [h_begin, h_end) of a
+ * job of n_histories.  edep_out: n_batches*nvox floats (host or device), energy deposited per batch
+ * grid in MeV (sum these over shards, then call mc_finalize). */
+mc_status mc_run_range(mc_ctx *ctx, const mc_beam *beam, uint64_t n_histories, uint64_t h_begin,
+                       uint64_t h_end, uint64_t seed, int32_t n_batches, float *edep_out);
+/* mc_finalize — batch statistics kernel: edep [n_batches][nvox] (host or device) -> dose, sigma. */
+mc_status mc_finalize(mc_ctx *ctx, const float *edep, uint64_t n_histories, int32_t n_batches,
+                      float *dose_out, float *sigma_out);
+
+/* mc_run_atten — attenuation-only mode (R20): photon primaries only; per history the
+ * linear voxel index of the first real interaction (-1 = left the phantom or never interacted) and its
+ * channel (0 Compton, 1 pair, 2 photoelectric, 255 none).  fp32 arithmetic contract: bit-exact
+ * against any other implementation of the contract given the same tables.
+ * voxel_out: n int32; channel_out: n uint8 (host or device; channel_out may be NULL). */
+mc_status mc_run_atten(mc_ctx *ctx, const mc_beam *beam, uint64_t n, uint64_t seed, int32_t *voxel_out,
+                       uint8_t *channel_out);
+
+/* Philox4x32-10 on the device: n blocks, ctr[4n], key[2n] -> out[4n] (host pointers). */
+mc_status mc_philox_selftest(const uint32_t *ctr, const uint32_t *key, int32_t n, uint32_t *out);
+
+mc_status mc_get_stats(const mc_ctx *ctx, mc_stats *out);
+/* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); 0 = default stream. */
+mc_status mc_set_stream(mc_ctx *ctx, void *cuda_stream);
+/* Tuning knobs ("the number of workitems M ... manually adjusted"):
+ * name = "wave_size" (histories admitted per scheduling round), "blocks_per_sm", "refill_lanes"
+ * (idle lanes per warp that trigger a refill), "aggregate" (0 plain red, 1 warp-aggregated red). */
+mc_status mc_set_option(mc_ctx *ctx, const char *name, int64_t value);
+const char *mc_last_error(const mc_ctx *ctx);
+const char *mc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MC_B200_H */
