@@ -166,11 +166,19 @@ mc_status mc_run_atten(mc_ctx *ctx, const mc_beam *beam, uint64_t n, uint64_t se
 /* Philox4x32-10 on the device: n blocks, ctr[4n], key[2n] -> out[4n] (host pointers). */
 mc_status mc_philox_selftest(const uint32_t *ctr, const uint32_t *key, int32_t n, uint32_t *out);
 
+/* mc_bench_red — measures the scoring roofline: `blocks` x 256 threads each
+ * issue per_thread red.global.add.f32 into a window of n_cells floats.  mode 0: pseudo-random cell per
+ * thread (no intra-warp collisions on average); mode 1: one cell per warp (full intra-warp collision).
+ * *ms_out (host) = CUDA-event time of the launch. */
+mc_status mc_bench_red(mc_ctx *ctx, uint32_t n_cells, int32_t per_thread, int32_t mode, int32_t blocks,
+                       double *ms_out);
+
 mc_status mc_get_stats(const mc_ctx *ctx, mc_stats *out);
 /* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); 0 = default stream. */
 mc_status mc_set_stream(mc_ctx *ctx, void *cuda_stream);
 /* Tuning knobs ("the number of workitems M ... manually adjusted"):
- * name = "wave_size" (histories admitted per scheduling round), "blocks_per_sm", "refill_lanes"
+ * name = "wave_size" (histories admitted per scheduling round), "queue_factor" (queue capacity in waves),
+ * "blocks_per_sm", "refill_lanes"
  * (idle lanes per warp that trigger a refill), "aggregate" (0 plain red, 1 warp-aggregated red). */
 mc_status mc_set_option(mc_ctx *ctx, const char *name, int64_t value);
 const char *mc_last_error(const mc_ctx *ctx);

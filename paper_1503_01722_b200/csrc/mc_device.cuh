@@ -39,8 +39,12 @@ struct Queue {
 enum Counter { C_HEAD = 0, C_E_A, C_E_B, C_P, C_OVERFLOW, C_COUNT };
 enum StatId {
     S_ESTEP = 0, S_FLIGHT, S_FICT, S_COMPTON, S_PAIR, S_PE, S_MOLLER, S_BREMS, S_SEC_E, S_SEC_G, S_ATOMICS,
-    S_COUNT
+    S_HIST, S_COUNT
 };
+enum LedgerId { LG_SRC = 0, LG_ESC, LG_DEP, LG_COUNT };
+enum { TE_R = 0, TE_L, TE_SMAX, TE_SM, TE_SHARD, TE_K1, TE_COUNT };  // electron tables per material
+enum { TP_TOT = 0, TP_C, TP_PP, TP_COUNT };                         // photon tables per material (after mu_maj)
+enum { CODE_ELECTRON = 0u, CODE_POSITRON = 1u, CODE_PHOTON = 2u };
 struct RunParams {
     Geometry g;
     BeamDev beam;
@@ -49,6 +53,7 @@ struct RunParams {
     const float2* tabE;  // electron tables per material: R, L, S_max, S_M, S_hard, K1
     int N, n_mat, k_cut;
     float lnE0, dln, inv_dln, e_cut, g_cut, d_maxs, f_maxe;
+    float lnE0P, inv_dlnP;  // grid of the photon tables (may be user supplied, mc_set_photon_tables)
     float lscr[MAX_MAT];
     uint32_t flags;
     float* edep;  // [n_batches][nvox]
@@ -61,8 +66,6 @@ struct RunParams {
     unsigned long long* stats;  // StatId
     double* ledger;           // e_src, e_dep, e_esc
     int refill_lanes, aggregate;
-    int32_t* atten_vox;       // attenuation-only outputs (else null)
-    uint8_t* atten_chan;
 };
 
 // ---- Philox4x32-10 -----------------------------------------------------------------------------

@@ -1,0 +1,597 @@
+// C ABI of the engine (include/mc.h): context, table upload, the launch scheduler and the calls.
+// Host logic only; every step of the hot path runs in the kernels of mc_kernels.cuh.
+#include "../../include/mc.h"
+#include "mc_kernels.cuh"
+#include "mc_tables.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace mcb;
+
+struct mc_ctx {
+    // phantom (host copies)
+    Geometry g{};
+    std::vector<uint8_t> h_mat;
+    std::vector<float> h_rho;
+    // tables (host)
+    bool have_tables = false;
+    Tables tabs;
+    mc_params params{};
+    float lnE0P = 0, inv_dlnP = 0;
+    std::vector<float> p_maj, p_tot, p_C, p_pp;  // photon tables in use: [N], [n_mat][N] x 3
+    // device state (allocated at the first compute call)
+    bool dev_ready = false, tables_dirty = true;
+    int sm_count = 0;
+    cudaStream_t stream = nullptr;
+    uint2* d_vox = nullptr;
+    float2 *d_tabP = nullptr, *d_tabE = nullptr;
+    size_t tabP_cap = 0, tabE_cap = 0;
+    uint4* d_q[3] = {nullptr, nullptr, nullptr};  // electron A, electron B, photon
+    uint32_t q_cap = 0;
+    uint32_t* d_counters = nullptr;
+    uint32_t* h_counters = nullptr;  // pinned
+    unsigned long long* d_stats = nullptr;
+    double* d_ledger = nullptr;
+    float* d_edep = nullptr;
+    size_t edep_cap = 0;
+    float *d_dose = nullptr, *d_sigma = nullptr;
+    float* d_beam = nullptr;  // E nodes, pdf nodes, cdf: 3 x kMaxNodes
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    // options (M "manually adjusted")
+    int64_t wave_size = 1 << 22, queue_factor = 6, blocks_per_sm = 0, refill_lanes = 4, aggregate = 0;
+    mc_stats stats{};
+    std::string err;
+};
+
+namespace {
+
+constexpr int kMaxNodes = 4096;
+
+mc_status fail(mc_ctx* c, mc_status s, const std::string& msg) {
+    if (c) c->err = msg;
+    return s;
+}
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? MC_ERR_OOM : MC_ERR_CUDA,           \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                       \
+    } while (0)
+
+std::vector<float2> pairs(const float* t, int N) {  // (value, slope to the next node); fp32 subtraction (R20)
+    std::vector<float2> o(N);
+    for (int i = 0; i < N; ++i) { o[i].x = t[i]; o[i].y = i + 1 < N ? t[i + 1] - t[i] : 0.0f; }
+    return o;
+}
+
+mc_status ensure_device(mc_ctx* ctx) {
+    if (ctx->dev_ready) return MC_OK;
+    int n = 0;
+    if (cudaGetDeviceCount(&n) != cudaSuccess || n <= 0) {
+        cudaGetLastError();
+        return fail(ctx, MC_ERR_CUDA, "no CUDA device: this library has no CPU path");
+    }
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major < 10) return fail(ctx, MC_ERR_CUDA, "built for sm_100a; this device is older");
+    ctx->sm_count = prop.multiProcessorCount;
+    size_t nvox = ctx->g.nvox;
+    std::vector<uint2> pk(nvox);
+    for (size_t i = 0; i < nvox; ++i) { memcpy(&pk[i].x, &ctx->h_rho[i], 4); pk[i].y = ctx->h_mat[i]; }
+    CU(cudaMalloc(&ctx->d_vox, nvox * sizeof(uint2)));
+    CU(cudaMemcpy(ctx->d_vox, pk.data(), nvox * sizeof(uint2), cudaMemcpyHostToDevice));
+    CU(cudaMalloc(&ctx->d_counters, C_COUNT * sizeof(uint32_t)));
+    CU(cudaMallocHost(&ctx->h_counters, C_COUNT * sizeof(uint32_t)));
+    CU(cudaMalloc(&ctx->d_stats, S_COUNT * sizeof(unsigned long long)));
+    CU(cudaMalloc(&ctx->d_ledger, LG_COUNT * sizeof(double)));
+    CU(cudaMalloc(&ctx->d_dose, nvox * sizeof(float)));
+    CU(cudaMalloc(&ctx->d_sigma, nvox * sizeof(float)));
+    CU(cudaMalloc(&ctx->d_beam, 3 * kMaxNodes * sizeof(float)));
+    for (auto& e : ctx->ev) CU(cudaEventCreate(&e));
+    ctx->dev_ready = true;
+    return MC_OK;
+}
+
+mc_status upload_tables(mc_ctx* ctx) {
+    if (!ctx->tables_dirty) return MC_OK;
+    const Tables& t = ctx->tabs;
+    const int N = t.N, nm = t.n_mat;
+    std::vector<float2> P((size_t)(1 + nm * TP_COUNT) * N), E((size_t)nm * TE_COUNT * N);
+    auto put = [&](std::vector<float2>& dst, size_t slot, const float* src) {
+        std::vector<float2> pr = pairs(src, N);
+        std::copy(pr.begin(), pr.end(), dst.begin() + slot * N);
+    };
+    put(P, 0, ctx->p_maj.data());
+    for (int m = 0; m < nm; ++m) {
+        put(P, 1 + m * TP_COUNT + TP_TOT, ctx->p_tot.data() + (size_t)m * N);
+        put(P, 1 + m * TP_COUNT + TP_C, ctx->p_C.data() + (size_t)m * N);
+        put(P, 1 + m * TP_COUNT + TP_PP, ctx->p_pp.data() + (size_t)m * N);
+        const int src[TE_COUNT] = {T_RANGE, T_L, T_S_MAX, T_S_MOLLER, T_S_HARD, T_K1};
+        for (int k = 0; k < TE_COUNT; ++k) put(E, (size_t)m * TE_COUNT + k, t.t[src[k]][m].data());
+    }
+    if (P.size() > ctx->tabP_cap) { cudaFree(ctx->d_tabP); ctx->d_tabP = nullptr; CU(cudaMalloc(&ctx->d_tabP, P.size() * sizeof(float2))); ctx->tabP_cap = P.size(); }
+    if (E.size() > ctx->tabE_cap) { cudaFree(ctx->d_tabE); ctx->d_tabE = nullptr; CU(cudaMalloc(&ctx->d_tabE, E.size() * sizeof(float2))); ctx->tabE_cap = E.size(); }
+    CU(cudaMemcpy(ctx->d_tabP, P.data(), P.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_tabE, E.data(), E.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    ctx->tables_dirty = false;
+    return MC_OK;
+}
+
+size_t smem_e(const mc_ctx* c) { return (size_t)c->tabs.n_mat * TE_COUNT * c->tabs.N * sizeof(float2); }
+size_t smem_p(const mc_ctx* c) { return (size_t)(1 + c->tabs.n_mat * TP_COUNT) * c->tabs.N * sizeof(float2); }
+
+mc_status check_beam(mc_ctx* ctx, const mc_beam* b) {
+    if (!b) return fail(ctx, MC_ERR_INVALID_ARG, "beam is null");
+    if (b->particle < -1 || b->particle > 1) return fail(ctx, MC_ERR_INVALID_ARG, "beam.particle must be -1, 0 or 1");
+    if (b->shape != MC_SHAPE_PENCIL && b->shape != MC_SHAPE_POINT_RECT) return fail(ctx, MC_ERR_INVALID_ARG, "beam.shape");
+    if (b->n_nodes < 1 || b->n_nodes > kMaxNodes || !b->E_nodes_MeV) return fail(ctx, MC_ERR_INVALID_ARG, "beam.n_nodes / E_nodes_MeV");
+    if (b->n_nodes > 1 && !b->pdf_nodes) return fail(ctx, MC_ERR_INVALID_ARG, "beam.pdf_nodes is null");
+    float an = std::sqrt(b->axis[0] * b->axis[0] + b->axis[1] * b->axis[1] + b->axis[2] * b->axis[2]);
+    if (!(std::fabs(an - 1.0f) < 1e-4f)) return fail(ctx, MC_ERR_INVALID_ARG, "beam.axis must be a unit vector");
+    if (b->shape == MC_SHAPE_POINT_RECT) {
+        if (!(b->ssd_cm > 0) || !(b->field_cm[0] >= 0) || !(b->field_cm[1] >= 0)) return fail(ctx, MC_ERR_INVALID_ARG, "beam.ssd_cm / field_cm");
+        if (!(b->axis[2] > 0.9999f)) return fail(ctx, MC_ERR_INVALID_ARG, "POINT_RECT beams must point along +z");
+    }
+    double tot = 0;
+    for (int i = 0; i < b->n_nodes; ++i) {
+        if (!(b->E_nodes_MeV[i] > 0)) return fail(ctx, MC_ERR_INVALID_ARG, "beam energies must be positive");
+        if (b->E_nodes_MeV[i] > ctx->params.e_max_MeV) return fail(ctx, MC_ERR_ENERGY_RANGE, "beam energy above e_max_MeV");
+        if (i && !(b->E_nodes_MeV[i] > b->E_nodes_MeV[i - 1])) return fail(ctx, MC_ERR_INVALID_ARG, "beam energy nodes must ascend");
+        if (b->n_nodes > 1) {
+            if (!(b->pdf_nodes[i] >= 0)) return fail(ctx, MC_ERR_INVALID_ARG, "beam pdf must be non-negative");
+            if (i) tot += 0.5 * ((double)b->pdf_nodes[i] + b->pdf_nodes[i - 1]) * ((double)b->E_nodes_MeV[i] - b->E_nodes_MeV[i - 1]);
+        }
+    }
+    if (b->n_nodes > 1 && !(tot > 0)) return fail(ctx, MC_ERR_INVALID_ARG, "beam pdf integrates to zero");
+    return MC_OK;
+}
+
+mc_status upload_beam(mc_ctx* ctx, const mc_beam* b, BeamDev& out) {
+    const int n = b->n_nodes;
+    std::vector<float> buf(3 * (size_t)kMaxNodes, 0.0f);
+    std::vector<double> cd(n, 0.0);
+    double tot = 0;
+    for (int j = 0; j < n; ++j) {
+        buf[j] = b->E_nodes_MeV[j];
+        buf[kMaxNodes + j] = n > 1 ? b->pdf_nodes[j] : 1.0f;
+        if (j + 1 < n) { tot += 0.5 * ((double)b->pdf_nodes[j] + (double)b->pdf_nodes[j + 1]) * ((double)b->E_nodes_MeV[j + 1] - (double)b->E_nodes_MeV[j]); cd[j + 1] = tot; }
+    }
+    for (int j = 0; j < n; ++j) buf[2 * kMaxNodes + j] = tot > 0 ? (float)(cd[j] / tot) : 0.0f;
+    CU(cudaMemcpyAsync(ctx->d_beam, buf.data(), buf.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));  // buf is pageable and local
+    out.particle = b->particle; out.shape = b->shape; out.n_nodes = n;
+    out.ex = b->entry_cm[0]; out.ey = b->entry_cm[1]; out.ez = b->entry_cm[2];
+    out.ax = b->axis[0]; out.ay = b->axis[1]; out.az = b->axis[2];
+    out.ssd = b->ssd_cm; out.fx = b->field_cm[0]; out.fy = b->field_cm[1];
+    out.E_nodes = ctx->d_beam; out.pdf_nodes = ctx->d_beam + kMaxNodes; out.cdf = ctx->d_beam + 2 * kMaxNodes;
+    return MC_OK;
+}
+
+void fill_params(const mc_ctx* ctx, RunParams& P) {
+    const Tables& t = ctx->tabs;
+    P.g = ctx->g;
+    P.vox = ctx->d_vox; P.tabP = ctx->d_tabP; P.tabE = ctx->d_tabE;
+    P.N = t.N; P.n_mat = t.n_mat; P.k_cut = t.k_cut;
+    P.lnE0 = (float)t.lnE0; P.dln = (float)t.dln; P.inv_dln = (float)(1.0 / t.dln);
+    P.lnE0P = ctx->lnE0P; P.inv_dlnP = ctx->inv_dlnP;
+    P.e_cut = ctx->params.e_cut_MeV; P.g_cut = ctx->params.g_cut_MeV;
+    P.d_maxs = ctx->params.d_maxs_cm; P.f_maxe = ctx->params.f_maxe;
+    for (int m = 0; m < MAX_MAT; ++m) P.lscr[m] = m < t.n_mat ? t.lscr[m] : 0.0f;
+    P.flags = ctx->params.flags;
+    P.counters = ctx->d_counters; P.stats = ctx->d_stats; P.ledger = ctx->d_ledger;
+    P.refill_lanes = (int)ctx->refill_lanes; P.aggregate = (int)ctx->aggregate;
+}
+
+}  // namespace
+
+namespace {
+
+// Launch scheduler (workflow Table 1): same-type launches; the queue holding at least one
+// full wave goes first, otherwise the group with the most particles (source included).
+mc_status transport(mc_ctx* ctx, const mc_beam* beam, uint64_t n_total, uint64_t h0, uint64_t h1, uint64_t seed,
+                    int n_batches, float* d_edep) {
+    mc_status st;
+    if ((st = ensure_device(ctx)) != MC_OK) return st;
+    if ((st = upload_tables(ctx)) != MC_OK) return st;
+    const size_t nvox = ctx->g.nvox;
+    const size_t se = smem_e(ctx), sp = smem_p(ctx);
+    if (se > 200 * 1024 || sp > 200 * 1024) return fail(ctx, MC_ERR_INVALID_ARG, "tables do not fit in shared memory: lower n_grid");
+    CU(cudaFuncSetAttribute(electron_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)se));
+    CU(cudaFuncSetAttribute(photon_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp));
+    int occ_e = 0, occ_p = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_e, electron_kernel, kThreads, se));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, photon_kernel, kThreads, sp));
+    if (occ_e < 1 || occ_p < 1) return fail(ctx, MC_ERR_CUDA, "kernel does not fit on an SM");
+    if (ctx->blocks_per_sm > 0) { occ_e = std::min<int>(occ_e, (int)ctx->blocks_per_sm); occ_p = std::min<int>(occ_p, (int)ctx->blocks_per_sm); }
+
+    // queues
+    const uint64_t n_run = h1 - h0;
+    const uint32_t W = (uint32_t)std::min<uint64_t>((uint64_t)ctx->wave_size, std::max<uint64_t>(n_run, 1024));
+    const uint32_t cap = (uint32_t)std::min<uint64_t>((uint64_t)W * (uint64_t)ctx->queue_factor, 0x7fffffffull / 3);
+    if (cap > ctx->q_cap) {
+        for (auto& q : ctx->d_q) { cudaFree(q); q = nullptr; }
+        ctx->q_cap = 0;
+        for (auto& q : ctx->d_q) CU(cudaMalloc(&q, (size_t)cap * 3 * sizeof(uint4)));
+        ctx->q_cap = cap;
+    }
+    cudaStream_t s = ctx->stream;
+    CU(cudaMemsetAsync(d_edep, 0, (size_t)n_batches * nvox * sizeof(float), s));
+    CU(cudaMemsetAsync(ctx->d_counters, 0, C_COUNT * sizeof(uint32_t), s));
+    CU(cudaMemsetAsync(ctx->d_stats, 0, S_COUNT * sizeof(unsigned long long), s));
+    CU(cudaMemsetAsync(ctx->d_ledger, 0, LG_COUNT * sizeof(double), s));
+
+    RunParams P;
+    memset(&P, 0, sizeof P);
+    fill_params(ctx, P);
+    if ((st = upload_beam(ctx, beam, P.beam)) != MC_OK) return st;
+    P.edep = d_edep; P.n_total = n_total; P.n_batches = n_batches;
+    P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32);
+
+    const bool photon_beam = beam->particle == MC_PHOTON;
+    uint64_t remaining = n_run, h_next = h0;
+    uint32_t cnt_e[2] = {0, 0}, cnt_p = 0;
+    int cur = 0;
+    mc_stats& S = ctx->stats;
+    S = mc_stats{};
+    double ms_e = 0, ms_p = 0;
+    CU(cudaEventRecord(ctx->ev[0], s));
+    while (remaining > 0 || cnt_e[cur] > 0 || cnt_p > 0) {
+        bool run_p;
+        if (cnt_p >= W) run_p = true;
+        else if (cnt_e[cur] >= W) run_p = false;
+        else {
+            uint64_t avail_e = cnt_e[cur] + (photon_beam ? 0 : remaining), avail_p = cnt_p + (photon_beam ? remaining : 0);
+            run_p = avail_p > avail_e;
+        }
+        uint32_t n_in = run_p ? cnt_p : cnt_e[cur], n_new = 0;
+        if (run_p == photon_beam && n_in < W) n_new = (uint32_t)std::min<uint64_t>(remaining, W - n_in);
+        P.n_in = n_in; P.n_new = n_new; P.h_first = h_next;
+        Queue qe_cur{ctx->d_q[cur], ctx->d_counters + C_E_A + cur, ctx->q_cap};
+        Queue qe_oth{ctx->d_q[1 - cur], ctx->d_counters + C_E_A + (1 - cur), ctx->q_cap};
+        Queue qp{ctx->d_q[2], ctx->d_counters + C_P, ctx->q_cap};
+        const uint64_t items = (uint64_t)n_in + n_new;
+        const int occ = run_p ? occ_p : occ_e;
+        int grid = (int)std::min<uint64_t>((uint64_t)ctx->sm_count * occ, (items + kThreads - 1) / kThreads);
+        grid = std::max(grid, 1);
+        CU(cudaEventRecord(ctx->ev[2], s));
+        if (run_p) {
+            P.q_in = qp; P.q_e_out = qe_cur; P.q_p_out = qp;
+            photon_kernel<<<grid, kThreads, sp, s>>>(P);
+        } else {
+            P.q_in = qe_cur; P.q_e_out = qe_oth; P.q_p_out = qp;
+            electron_kernel<<<grid, kThreads, se, s>>>(P);
+        }
+        CU(cudaGetLastError());
+        CU(cudaEventRecord(ctx->ev[3], s));
+        // the consumed queue and the work counter start the next launch empty
+        CU(cudaMemsetAsync(ctx->d_counters + C_HEAD, 0, sizeof(uint32_t), s));
+        CU(cudaMemsetAsync(run_p ? qp.count : qe_cur.count, 0, sizeof(uint32_t), s));
+        CU(cudaMemcpyAsync(ctx->h_counters, ctx->d_counters, C_COUNT * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+        CU(cudaStreamSynchronize(s));
+        float ms = 0;
+        CU(cudaEventElapsedTime(&ms, ctx->ev[2], ctx->ev[3]));
+        (run_p ? ms_p : ms_e) += ms;
+        ++S.n_kernel_launches;
+        if (ctx->h_counters[C_OVERFLOW])
+            return fail(ctx, MC_ERR_QUEUE_OVERFLOW, "particle queue overflow: lower option wave_size or raise queue_factor");
+        remaining -= n_new; h_next += n_new;
+        if (run_p) { cnt_p = 0; cnt_e[cur] = ctx->h_counters[C_E_A + cur]; }
+        else { cnt_e[cur] = 0; cur = 1 - cur; cnt_e[cur] = ctx->h_counters[C_E_A + cur]; cnt_p = ctx->h_counters[C_P]; }
+    }
+    CU(cudaEventRecord(ctx->ev[1], s));
+    // ledger: deposited energy is the total of the batch grids
+    sum_kernel<<<ctx->sm_count * 4, kThreads, 0, s>>>(d_edep, (size_t)n_batches * nvox, ctx->d_ledger + LG_DEP);
+    CU(cudaGetLastError());
+    unsigned long long hs[S_COUNT];
+    double hl[LG_COUNT];
+    CU(cudaMemcpyAsync(hs, ctx->d_stats, sizeof hs, cudaMemcpyDeviceToHost, s));
+    CU(cudaMemcpyAsync(hl, ctx->d_ledger, sizeof hl, cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    float ms = 0;
+    CU(cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]));
+    S.n_histories = hs[S_HIST]; S.n_electron_steps = hs[S_ESTEP]; S.n_photon_flights = hs[S_FLIGHT];
+    S.n_fictitious = hs[S_FICT]; S.n_compton = hs[S_COMPTON]; S.n_pair = hs[S_PAIR]; S.n_photoelectric = hs[S_PE];
+    S.n_moller = hs[S_MOLLER]; S.n_brems = hs[S_BREMS]; S.n_secondary_electrons = hs[S_SEC_E];
+    S.n_secondary_photons = hs[S_SEC_G]; S.n_dose_atomics = hs[S_ATOMICS];
+    S.e_source_MeV = hl[LG_SRC]; S.e_escaped_MeV = hl[LG_ESC]; S.e_deposited_MeV = hl[LG_DEP];
+    S.transport_ms = ms; S.electron_kernel_ms = ms_e; S.photon_kernel_ms = ms_p;
+    return MC_OK;
+}
+
+mc_status check_run_args(mc_ctx* ctx, const mc_beam* beam, uint64_t n_histories, uint64_t h0, uint64_t h1, int32_t n_batches) {
+    if (!ctx) return MC_ERR_INVALID_ARG;
+    if (!ctx->have_tables) return fail(ctx, MC_ERR_STATE, "mc_build_tables has not been called");
+    mc_status st = check_beam(ctx, beam);
+    if (st != MC_OK) return st;
+    if (n_histories == 0 || n_histories >= (1ull << 32)) return fail(ctx, MC_ERR_INVALID_ARG, "n_histories must be in [1, 2^32)");
+    if (n_batches < 2 || (uint64_t)n_batches > n_histories) return fail(ctx, MC_ERR_INVALID_ARG, "n_batches must be in [2, n_histories]");
+    if (h0 > h1 || h1 > n_histories) return fail(ctx, MC_ERR_INVALID_ARG, "history range");
+    if ((uint64_t)n_batches * (uint64_t)ctx->g.nvox >= (1ull << 32)) return fail(ctx, MC_ERR_INVALID_ARG, "n_batches * nvox must be < 2^32");
+    return MC_OK;
+}
+
+mc_status ensure_edep(mc_ctx* ctx, size_t n) {
+    if (n <= ctx->edep_cap) return MC_OK;
+    cudaFree(ctx->d_edep); ctx->d_edep = nullptr; ctx->edep_cap = 0;
+    CU(cudaMalloc(&ctx->d_edep, n * sizeof(float)));
+    ctx->edep_cap = n;
+    return MC_OK;
+}
+
+mc_status finalize_device(mc_ctx* ctx, const float* d_edep, uint64_t n_histories, int n_batches) {
+    const int nvox = ctx->g.nvox;
+    const double vol = (double)ctx->g.hx * (double)ctx->g.hy * (double)ctx->g.hz;
+    int grid = std::min(ctx->sm_count * 8, (nvox + kThreads - 1) / kThreads);
+    finalize_kernel<<<grid, kThreads, n_batches * sizeof(double), ctx->stream>>>(d_edep, ctx->d_vox, nvox, n_batches, n_histories, vol,
+                                                                                  ctx->d_dose, ctx->d_sigma);
+    CU(cudaGetLastError());
+    ++ctx->stats.n_kernel_launches;
+    return MC_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
+// C ABI
+// =================================================================================================
+extern "C" {
+
+mc_status mc_create(const uint8_t* material_idx, const float* density_gcc, const int32_t dims[3], const float voxel_cm[3],
+                    const float origin_cm[3], mc_ctx** out) {
+    if (!out) return MC_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!material_idx || !density_gcc || !dims || !voxel_cm || !origin_cm) return MC_ERR_INVALID_ARG;
+    for (int a = 0; a < 3; ++a)
+        if (dims[a] <= 0 || !(voxel_cm[a] > 0.0f) || !std::isfinite(voxel_cm[a]) || !std::isfinite(origin_cm[a])) return MC_ERR_INVALID_ARG;
+    const uint64_t nvox = (uint64_t)dims[0] * (uint64_t)dims[1] * (uint64_t)dims[2];
+    if (nvox >= (1ull << 31)) return MC_ERR_INVALID_ARG;
+    for (uint64_t i = 0; i < nvox; ++i)
+        if (!(density_gcc[i] > 0.0f) || !std::isfinite(density_gcc[i])) return MC_ERR_INVALID_ARG;
+    mc_ctx* ctx = new (std::nothrow) mc_ctx();
+    if (!ctx) return MC_ERR_OOM;
+    Geometry& g = ctx->g;
+    g.nx = dims[0]; g.ny = dims[1]; g.nz = dims[2]; g.nvox = (int)nvox;
+    g.hx = voxel_cm[0]; g.hy = voxel_cm[1]; g.hz = voxel_cm[2];
+    g.ox = origin_cm[0]; g.oy = origin_cm[1]; g.oz = origin_cm[2];
+    g.ihx = 1.0f / g.hx; g.ihy = 1.0f / g.hy; g.ihz = 1.0f / g.hz;
+    try {
+        ctx->h_mat.assign(material_idx, material_idx + nvox);
+        ctx->h_rho.assign(density_gcc, density_gcc + nvox);
+    } catch (...) { delete ctx; return MC_ERR_OOM; }
+    *out = ctx;
+    return MC_OK;
+}
+
+void mc_destroy(mc_ctx* ctx) {
+    if (!ctx) return;
+    if (ctx->dev_ready) {
+        cudaFree(ctx->d_vox); cudaFree(ctx->d_tabP); cudaFree(ctx->d_tabE);
+        for (auto q : ctx->d_q) cudaFree(q);
+        cudaFree(ctx->d_counters); cudaFreeHost(ctx->h_counters); cudaFree(ctx->d_stats); cudaFree(ctx->d_ledger);
+        cudaFree(ctx->d_edep); cudaFree(ctx->d_dose); cudaFree(ctx->d_sigma); cudaFree(ctx->d_beam);
+        for (auto e : ctx->ev) if (e) cudaEventDestroy(e);
+    }
+    delete ctx;
+}
+
+mc_status mc_build_tables(mc_ctx* ctx, const mc_material* mats, int32_t n_mats, const mc_params* params) {
+    if (!ctx) return MC_ERR_INVALID_ARG;
+    if (!mats || !params || n_mats <= 0 || n_mats > MAX_MAT) return fail(ctx, MC_ERR_INVALID_ARG, "materials / params (n_mats must be 1..8)");
+    if (!(params->d_maxs_cm > 0) || !(params->f_maxe > 0) || !(params->f_maxe <= 1)) return fail(ctx, MC_ERR_INVALID_ARG, "d_maxs_cm must be > 0 and f_maxe in (0, 1]");
+    std::vector<double> rho_max(n_mats, 0.0);
+    for (size_t i = 0; i < ctx->h_mat.size(); ++i) {
+        if (ctx->h_mat[i] >= n_mats) return fail(ctx, MC_ERR_INVALID_ARG, "a voxel's material index is >= n_mats");
+        rho_max[ctx->h_mat[i]] = std::max(rho_max[ctx->h_mat[i]], (double)ctx->h_rho[i]);
+    }
+    std::vector<MaterialSpec> specs(n_mats);
+    for (int m = 0; m < n_mats; ++m) {
+        const mc_material& s = mats[m];
+        if (s.n_elem <= 0 || !s.Z || !s.A || !s.w) return fail(ctx, MC_ERR_INVALID_ARG, "material without elements");
+        for (int e = 0; e < s.n_elem; ++e) specs[m].el.push_back(Element{s.Z[e], (double)s.A[e], (double)s.w[e]});
+        specs[m].I_eV = s.I_eV; specs[m].rho_nominal = s.rho_nominal;
+    }
+    TableParams tp{(double)params->e_cut_MeV, (double)params->g_cut_MeV, (double)params->e_max_MeV, params->n_grid};
+    Tables t;
+    std::string msg = build_tables(specs, tp, rho_max, t);
+    if (!msg.empty()) return fail(ctx, MC_ERR_INVALID_ARG, msg);
+    ctx->tabs = std::move(t);
+    ctx->params = *params;
+    const int N = ctx->tabs.N;
+    ctx->lnE0P = (float)ctx->tabs.lnE0; ctx->inv_dlnP = (float)(1.0 / ctx->tabs.dln);
+    ctx->p_maj = ctx->tabs.mu_maj;
+    ctx->p_tot.resize((size_t)n_mats * N); ctx->p_C.resize((size_t)n_mats * N); ctx->p_pp.resize((size_t)n_mats * N);
+    for (int m = 0; m < n_mats; ++m) {
+        std::copy(ctx->tabs.t[T_MU_TOT][m].begin(), ctx->tabs.t[T_MU_TOT][m].end(), ctx->p_tot.begin() + (size_t)m * N);
+        std::copy(ctx->tabs.t[T_MU_C][m].begin(), ctx->tabs.t[T_MU_C][m].end(), ctx->p_C.begin() + (size_t)m * N);
+        std::copy(ctx->tabs.t[T_MU_PP][m].begin(), ctx->tabs.t[T_MU_PP][m].end(), ctx->p_pp.begin() + (size_t)m * N);
+    }
+    ctx->have_tables = true; ctx->tables_dirty = true;
+    return MC_OK;
+}
+
+mc_status mc_export_table(const mc_ctx* cctx, int32_t material, int32_t which, float* out) {
+    mc_ctx* ctx = const_cast<mc_ctx*>(cctx);
+    if (!ctx || !out) return MC_ERR_INVALID_ARG;
+    if (!ctx->have_tables) return fail(ctx, MC_ERR_STATE, "mc_build_tables has not been called");
+    const int N = ctx->tabs.N;
+    if (which == 9) { std::copy(ctx->p_maj.begin(), ctx->p_maj.end(), out); return MC_OK; }
+    if (which < 0 || which > 8 || material < 0 || material >= ctx->tabs.n_mat) return fail(ctx, MC_ERR_INVALID_ARG, "table id / material");
+    const float* src;
+    if (which == 0) src = ctx->p_tot.data() + (size_t)material * N;
+    else if (which == 1) src = ctx->p_C.data() + (size_t)material * N;
+    else if (which == 2) src = ctx->p_pp.data() + (size_t)material * N;
+    else src = ctx->tabs.t[which][material].data();  // TableId order matches mc.h for 3..8
+    std::copy(src, src + N, out);
+    return MC_OK;
+}
+
+mc_status mc_export_grid(const mc_ctx* cctx, double grid[4]) {
+    mc_ctx* ctx = const_cast<mc_ctx*>(cctx);
+    if (!ctx || !grid) return MC_ERR_INVALID_ARG;
+    if (!ctx->have_tables) return fail(ctx, MC_ERR_STATE, "mc_build_tables has not been called");
+    grid[0] = ctx->tabs.lnE0; grid[1] = ctx->tabs.dln; grid[2] = ctx->tabs.N; grid[3] = ctx->tabs.k_cut;
+    return MC_OK;
+}
+
+mc_status mc_set_photon_tables(mc_ctx* ctx, float lnE0, float inv_dln, const float* mu_maj, const float* mu_tot, const float* mu_C,
+                               const float* mu_pp) {
+    if (!ctx) return MC_ERR_INVALID_ARG;
+    if (!ctx->have_tables) return fail(ctx, MC_ERR_STATE, "mc_build_tables has not been called");
+    if (!mu_maj || !mu_tot || !mu_C || !mu_pp || !(inv_dln > 0)) return fail(ctx, MC_ERR_INVALID_ARG, "photon tables");
+    const size_t N = ctx->tabs.N, nm = ctx->tabs.n_mat;
+    ctx->lnE0P = lnE0; ctx->inv_dlnP = inv_dln;
+    ctx->p_maj.assign(mu_maj, mu_maj + N);
+    ctx->p_tot.assign(mu_tot, mu_tot + nm * N); ctx->p_C.assign(mu_C, mu_C + nm * N); ctx->p_pp.assign(mu_pp, mu_pp + nm * N);
+    ctx->tables_dirty = true;
+    return MC_OK;
+}
+
+mc_status mc_run_range(mc_ctx* ctx, const mc_beam* beam, uint64_t n_histories, uint64_t h_begin, uint64_t h_end, uint64_t seed,
+                       int32_t n_batches, float* edep_out) {
+    mc_status st = check_run_args(ctx, beam, n_histories, h_begin, h_end, n_batches);
+    if (st != MC_OK) return st;
+    if (!edep_out) return fail(ctx, MC_ERR_INVALID_ARG, "edep_out is null");
+    if ((st = ensure_device(ctx)) != MC_OK) return st;
+    const size_t n = (size_t)n_batches * ctx->g.nvox;
+    if ((st = ensure_edep(ctx, n)) != MC_OK) return st;
+    if ((st = transport(ctx, beam, n_histories, h_begin, h_end, seed, n_batches, ctx->d_edep)) != MC_OK) return st;
+    CU(cudaMemcpyAsync(edep_out, ctx->d_edep, n * sizeof(float), cudaMemcpyDefault, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return MC_OK;
+}
+
+mc_status mc_finalize(mc_ctx* ctx, const float* edep, uint64_t n_histories, int32_t n_batches, float* dose_out, float* sigma_out) {
+    if (!ctx) return MC_ERR_INVALID_ARG;
+    if (!edep || !dose_out || !sigma_out || n_batches < 2 || n_histories < (uint64_t)n_batches) return fail(ctx, MC_ERR_INVALID_ARG, "mc_finalize arguments");
+    mc_status st;
+    if ((st = ensure_device(ctx)) != MC_OK) return st;
+    const size_t nvox = ctx->g.nvox, n = (size_t)n_batches * nvox;
+    if ((st = ensure_edep(ctx, n)) != MC_OK) return st;
+    if (edep != ctx->d_edep) CU(cudaMemcpyAsync(ctx->d_edep, edep, n * sizeof(float), cudaMemcpyDefault, ctx->stream));
+    if ((st = finalize_device(ctx, ctx->d_edep, n_histories, n_batches)) != MC_OK) return st;
+    CU(cudaMemcpyAsync(dose_out, ctx->d_dose, nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
+    CU(cudaMemcpyAsync(sigma_out, ctx->d_sigma, nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return MC_OK;
+}
+
+mc_status mc_run(mc_ctx* ctx, const mc_beam* beam, uint64_t n_histories, uint64_t seed, int32_t n_batches, float* dose_out,
+                 float* sigma_out) {
+    mc_status st = check_run_args(ctx, beam, n_histories, 0, n_histories, n_batches);
+    if (st != MC_OK) return st;
+    if (!dose_out || !sigma_out) return fail(ctx, MC_ERR_INVALID_ARG, "dose_out / sigma_out is null");
+    if ((st = ensure_device(ctx)) != MC_OK) return st;
+    const size_t nvox = ctx->g.nvox;
+    if ((st = ensure_edep(ctx, (size_t)n_batches * nvox)) != MC_OK) return st;
+    if ((st = transport(ctx, beam, n_histories, 0, n_histories, seed, n_batches, ctx->d_edep)) != MC_OK) return st;
+    if ((st = finalize_device(ctx, ctx->d_edep, n_histories, n_batches)) != MC_OK) return st;
+    CU(cudaMemcpyAsync(dose_out, ctx->d_dose, nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
+    CU(cudaMemcpyAsync(sigma_out, ctx->d_sigma, nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return MC_OK;
+}
+
+mc_status mc_run_atten(mc_ctx* ctx, const mc_beam* beam, uint64_t n, uint64_t seed, int32_t* voxel_out, uint8_t* channel_out) {
+    if (!ctx) return MC_ERR_INVALID_ARG;
+    if (!ctx->have_tables) return fail(ctx, MC_ERR_STATE, "mc_build_tables has not been called");
+    mc_status st = check_beam(ctx, beam);
+    if (st != MC_OK) return st;
+    if (beam->particle != MC_PHOTON) return fail(ctx, MC_ERR_INVALID_ARG, "mc_run_atten takes photon beams only");
+    if (n >= (1ull << 32)) return fail(ctx, MC_ERR_INVALID_ARG, "n must be < 2^32");
+    if (n == 0) return MC_OK;
+    if (!voxel_out) return fail(ctx, MC_ERR_INVALID_ARG, "voxel_out is null");
+    if ((st = ensure_device(ctx)) != MC_OK) return st;
+    if ((st = upload_tables(ctx)) != MC_OK) return st;
+    RunParams P;
+    memset(&P, 0, sizeof P);
+    fill_params(ctx, P);
+    if ((st = upload_beam(ctx, beam, P.beam)) != MC_OK) return st;
+    P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32);
+    int32_t* d_v = nullptr; uint8_t* d_c = nullptr;
+    CU(cudaMalloc(&d_v, n * sizeof(int32_t)));
+    if (cudaMalloc(&d_c, n) != cudaSuccess) { cudaFree(d_v); return fail(ctx, MC_ERR_OOM, "cudaMalloc"); }
+    const int grid = (int)std::min<uint64_t>((uint64_t)ctx->sm_count * 8, (n + kThreads - 1) / kThreads);
+    atten_kernel<<<grid, kThreads, 0, ctx->stream>>>(P, n, d_v, d_c);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(voxel_out, d_v, n * sizeof(int32_t), cudaMemcpyDefault, ctx->stream);
+    if (e == cudaSuccess && channel_out) e = cudaMemcpyAsync(channel_out, d_c, n, cudaMemcpyDefault, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(d_v); cudaFree(d_c);
+    if (e != cudaSuccess) return fail(ctx, MC_ERR_CUDA, std::string("mc_run_atten: ") + cudaGetErrorString(e));
+    return MC_OK;
+}
+
+mc_status mc_philox_selftest(const uint32_t* ctr, const uint32_t* key, int32_t n, uint32_t* out) {
+    if (!ctr || !key || !out || n <= 0) return MC_ERR_INVALID_ARG;
+    uint32_t *d_c = nullptr, *d_k = nullptr, *d_o = nullptr;
+    cudaError_t e = cudaMalloc(&d_c, (size_t)n * 16);
+    if (e == cudaSuccess) e = cudaMalloc(&d_k, (size_t)n * 8);
+    if (e == cudaSuccess) e = cudaMalloc(&d_o, (size_t)n * 16);
+    if (e == cudaSuccess) e = cudaMemcpy(d_c, ctr, (size_t)n * 16, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(d_k, key, (size_t)n * 8, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        philox_test_kernel<<<(n + 127) / 128, 128>>>(d_c, d_k, n, d_o);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(out, d_o, (size_t)n * 16, cudaMemcpyDeviceToHost);
+    cudaFree(d_c); cudaFree(d_k); cudaFree(d_o);
+    if (e != cudaSuccess) { cudaGetLastError(); return MC_ERR_CUDA; }
+    return MC_OK;
+}
+
+mc_status mc_bench_red(mc_ctx* ctx, uint32_t n_cells, int32_t per_thread, int32_t mode, int32_t blocks, double* ms_out) {
+    if (!ctx || !ms_out || n_cells == 0 || per_thread <= 0 || blocks <= 0 || mode < 0 || mode > 1) return MC_ERR_INVALID_ARG;
+    mc_status st;
+    if ((st = ensure_device(ctx)) != MC_OK) return st;
+    float* d = nullptr;
+    CU(cudaMalloc(&d, (size_t)n_cells * sizeof(float)));
+    cudaMemsetAsync(d, 0, (size_t)n_cells * sizeof(float), ctx->stream);
+    red_bench_kernel<<<blocks, kThreads, 0, ctx->stream>>>(d, n_cells, 1, mode);  // warm-up
+    cudaEventRecord(ctx->ev[2], ctx->stream);
+    red_bench_kernel<<<blocks, kThreads, 0, ctx->stream>>>(d, n_cells, per_thread, mode);
+    cudaEventRecord(ctx->ev[3], ctx->stream);
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    float ms = 0;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, ctx->ev[2], ctx->ev[3]);
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(ctx, MC_ERR_CUDA, std::string("mc_bench_red: ") + cudaGetErrorString(e));
+    *ms_out = ms;
+    return MC_OK;
+}
+
+mc_status mc_get_stats(const mc_ctx* ctx, mc_stats* out) {
+    if (!ctx || !out) return MC_ERR_INVALID_ARG;
+    *out = ctx->stats;
+    return MC_OK;
+}
+
+mc_status mc_set_stream(mc_ctx* ctx, void* cuda_stream) {
+    if (!ctx) return MC_ERR_INVALID_ARG;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    return MC_OK;
+}
+
+mc_status mc_set_option(mc_ctx* ctx, const char* name, int64_t value) {
+    if (!ctx || !name) return MC_ERR_INVALID_ARG;
+    const std::string n(name);
+    if (n == "wave_size") { if (value < 1024 || value > (1ll << 28)) return fail(ctx, MC_ERR_INVALID_ARG, "wave_size in [1024, 2^28]"); ctx->wave_size = value; }
+    else if (n == "queue_factor") { if (value < 2 || value > 64) return fail(ctx, MC_ERR_INVALID_ARG, "queue_factor in [2, 64]"); ctx->queue_factor = value; }
+    else if (n == "blocks_per_sm") { if (value < 0 || value > 32) return fail(ctx, MC_ERR_INVALID_ARG, "blocks_per_sm in [0, 32]"); ctx->blocks_per_sm = value; }
+    else if (n == "refill_lanes") { if (value < 1 || value > 32) return fail(ctx, MC_ERR_INVALID_ARG, "refill_lanes in [1, 32]"); ctx->refill_lanes = value; }
+    else if (n == "aggregate") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "aggregate in {0, 1}"); ctx->aggregate = value; }
+    else return fail(ctx, MC_ERR_INVALID_ARG, "unknown option: " + n);
+    return MC_OK;
+}
+
+const char* mc_last_error(const mc_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+const char* mc_version(void) { return "paper_1503_01722_b200 0.1 (sm_100a)"; }
+
+}  // extern "C"
