@@ -130,6 +130,10 @@ def mc_version():
     return lib().mc_version().decode()
 
 
+def mc_last_error(ctx):
+    return lib().mc_last_error(ctx).decode()
+
+
 def mc_create(material_idx, density_gcc, dims, voxel_cm, origin_cm):
     mat = np.ascontiguousarray(material_idx, np.uint8).reshape(-1)
     rho = np.ascontiguousarray(density_gcc, np.float32).reshape(-1)
@@ -173,6 +177,16 @@ def mc_export_table(ctx, name, material=0):
     out = np.zeros(N, np.float32)
     which = TABLE_IDS[name]
     _check(ctx, lib().mc_export_table(ctx, -1 if which == 9 else int(material), which, out.ctypes.data))
+    return out
+
+
+def mc_export_photon_tables(ctx, n_mat):
+    """The fp32 photon tables in use, in the dict layout mc_set_photon_tables takes (marshalling only)."""
+    g = mc_export_grid(ctx)
+    out = {"lnE0": np.float32(g["lnE0"]), "inv_dln": np.float32(1.0 / g["dln"]),
+           "mu_maj": mc_export_table(ctx, "mu_maj")}
+    for k in ("mu_tot", "mu_C", "mu_pp"):
+        out[k] = np.stack([mc_export_table(ctx, k, m) for m in range(n_mat)])
     return out
 
 
