@@ -1,0 +1,345 @@
+#!/usr/bin/env python
+"""bench.py — one JSON line per run (driver contract).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl reference]
+
+A "step" is one pass of the whole hot path (source -> photon / electron transport -> scoring ->
+batch statistics) over one job of synthetic histories.  Default workload =
+BASELINE.json configs[1]: 15 MeV electron beam, 10x10 cm^2 at SSD 100, 61x61x60 water phantom at
+0.5 cm, 1e7 histories, 10 batches, cut-offs 0.2 / 0.01 MeV (the configuration the metric is quoted on).
+
+  value          histories/s with phantom, tables and queues resident in HBM, outputs left on the device
+  e2e            the same through the C ABI from HOST buffers: a fresh context per step (mc_create copies
+                 the phantom to the device, mc_build_tables builds + uploads the tables) and mc_run writing
+                 dose and sigma to host memory
+  roofline       dominant kernel (electron_kernel): algorithmic thread-instructions per launch (DESIGN.md
+                 "Measurement") / its CUDA-event time, against the SM issue peak
+  roofline_scoring  dose atomics issued per second against the measured red.global.add.f32 peak
+  cpu_baseline   the oracle as it stands on the host cores, bounded sample of the same workload
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1503_01722_b200 import workloads as W  # noqa: E402  (input generators only)
+
+# Algorithmic thread-instructions per unit of work.
+INSTR_PER = {"e_step": 240.0, "hard_event": 150.0, "photon_flight": 60.0, "photon_interaction": 150.0}
+SM_COUNT, SCHEDULERS_PER_SM, LANES = 148, 4, 32
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="engine", choices=["engine", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config, 1-based (default 2 = configs[1])")
+    ap.add_argument("--beam", default=None, choices=[None, "e", "g"], help="configs 4, 5: electron or photon beam")
+    ap.add_argument("--histories", type=int, default=0, help="override n_histories (the line then says so)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--option", action="append", default=[], help="engine option name=value (mc_set_option)")
+    return ap.parse_args()
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p)), "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) >= 6 and r[2 + i] == "Active" for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def workload(args):
+    cfg = W.config(args.config, args.beam)
+    if args.histories:
+        cfg["n_histories"] = args.histories
+    return cfg
+
+
+def config_dict(cfg, args, extra=None):
+    d = {"workload": f"BASELINE config {args.config}: {cfg['name']}", "n_histories_per_step": cfg["n_histories"],
+         "n_batches": cfg["n_batches"], "dims": [int(x) for x in cfg["phantom"]["dims"]],
+         "voxel_cm": float(cfg["phantom"]["voxel_cm"][0]), "e_cut_MeV": cfg["params"]["e_cut_MeV"],
+         "g_cut_MeV": cfg["params"]["g_cut_MeV"], "seed": cfg["seed"],
+         "histories_overridden": bool(args.histories)}
+    d.update(extra or {})
+    return d
+
+
+# ---- the oracle on the host cores (cpu_baseline leg and --impl reference) --------------------------
+def oracle_sample_rate(cfg, n_sample, workers):
+    import oracle  # test infrastructure: allowed here only (cpu_baseline / reference arm)
+    orc = oracle.Oracle(cfg["phantom"], cfg["materials"], cfg["params"])
+    _, st, dt = orc.run_sample(cfg["beam"], cfg["n_histories"], n_sample, cfg["seed"], cfg["n_batches"], workers)
+    return n_sample / dt, st, dt
+
+
+def oracle_sample_size(cfg, workers, seconds):
+    """Histories for about `seconds` of wall time on `workers` cores, from a 0.5 s single-core probe."""
+    import oracle
+    orc = oracle.Oracle(cfg["phantom"], cfg["materials"], cfg["params"])
+    n_probe, rate = 500, 0.0
+    while True:
+        _, _, dt = orc.run_sample(cfg["beam"], cfg["n_histories"], n_probe, cfg["seed"], cfg["n_batches"], 1)
+        rate = n_probe / dt
+        if dt > 0.3 or n_probe >= cfg["n_histories"]:
+            break
+        n_probe = min(n_probe * 4, cfg["n_histories"])
+    return int(max(1000, min(cfg["n_histories"], rate * workers * seconds)))
+
+
+def cpu_baseline(cfg, seconds=15.0):
+    import oracle
+    cores = oracle.host_cores()
+    n = oracle_sample_size(cfg, cores, seconds)
+    rate, st, dt = oracle_sample_rate(cfg, n, cores)
+    return {"value": rate, "unit": "histories/s", "cores": cores, "kind": "oracle",
+            "sample": f"histories [0, {n}) of the {cfg['n_histories']}-history job, same seed, {cores} processes, {dt:.1f} s",
+            "e_steps_per_s": st["n_estep"] / dt, "single_core_equiv": rate / cores}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    cfg = workload(args)
+    cores = oracle.host_cores()
+    # each step = a bounded sample sized so that warmup + steps end within a few minutes
+    per_step_s = max(2.0, min(20.0, 150.0 / max(1, args.steps + args.warmup)))
+    n = oracle_sample_size(cfg, cores, per_step_s)
+    for _ in range(args.warmup):
+        oracle_sample_rate(cfg, n, cores)
+    t, steps_e = 0.0, 0.0
+    for _ in range(args.steps):
+        _, st, dt = oracle_sample_rate(cfg, n, cores)
+        t += dt
+        steps_e += st["n_estep"]
+    value = n * args.steps / t
+    sample = f"histories [0, {n}) of the {cfg['n_histories']}-history job per step, {cores} processes"
+    print(json.dumps({
+        "impl": "reference", "metric": "histories/s", "value": value, "unit": "histories/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": config_dict(cfg, args, {"sample": sample}),
+        "e_steps_per_s": steps_e / t,
+        "cpu_baseline": {"value": value, "unit": "histories/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "histories/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ---- the CUDA engine ---------------------------------------------------------------------------------
+def run_engine(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1503_01722_b200 as mc
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the engine has no CPU path)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg = workload(args)
+    n, B, seed = cfg["n_histories"], cfg["n_batches"], cfg["seed"]
+    n_job = n * world  # weak scaling: every rank simulates n histories of one job of n * world
+    if n_job >= 2**32:
+        raise SystemExit("job too large: n_histories * gpus must be < 2^32")
+    eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])
+    for kv in args.option:
+        k, v = kv.split("=")
+        mc.mc_set_option(eng.ctx, k, int(v))
+    stream = torch.cuda.Stream()
+    mc.mc_set_stream(eng.ctx, stream.cuda_stream)
+    nvox = eng.nvox
+    dose = torch.empty(nvox, dtype=torch.float32, device="cuda")
+    sigma = torch.empty_like(dose)
+    edep = torch.empty(B * nvox, dtype=torch.float32, device="cuda") if world > 1 else None
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+
+    def step():
+        if world == 1:
+            mc.mc_run(eng.ctx, cfg["beam"], n, seed, B, dose, sigma)
+        else:  # shard = contiguous history range; one exchange: sum of the per-batch grids
+            mc.mc_run_range(eng.ctx, cfg["beam"], n_job, rank * n, (rank + 1) * n, seed, B, edep)
+            dist.all_reduce(edep)
+            mc.mc_finalize(eng.ctx, edep, n_job, B, dose, sigma)
+        return mc.mc_get_stats(eng.ctx)
+
+    def sync_all():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    with torch.cuda.stream(stream):
+        for _ in range(args.warmup):
+            flush.fill_(1)
+            step()
+        sync_all()
+        sampler = ClockSampler(local)
+        if rank == 0:
+            sampler.start()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        acc = {}
+        for i in range(args.steps):
+            flush.fill_(1)          # L2 flush between timed iterations (not timed)
+            ev[i][0].record(stream)
+            st = step()
+            ev[i][1].record(stream)
+            for k, v in st.items():
+                acc[k] = acc.get(k, 0) + v
+        sync_all()
+        clocks = sampler.stop() if rank == 0 else None
+    ms = torch.tensor([sum(a.elapsed_time(b) for a, b in ev)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    total_ms = float(ms.item())
+    K = args.steps
+
+    # ---- e2e: fresh context from HOST buffers every step, dose + sigma back to the host --------------------
+    e2e = None
+    if not args.no_e2e:
+        h_dose, h_sigma = np.zeros(nvox, np.float32), np.zeros(nvox, np.float32)
+        ph = cfg["phantom"]
+        tab_bytes = 0
+
+        def e2e_step():
+            nonlocal tab_bytes
+            e = mc.Engine(ph, cfg["materials"], cfg["params"])
+            mc.mc_set_stream(e.ctx, stream.cuda_stream)
+            if world == 1:
+                mc.mc_run(e.ctx, cfg["beam"], n, seed, B, h_dose, h_sigma)
+            else:
+                mc.mc_run_range(e.ctx, cfg["beam"], n_job, rank * n, (rank + 1) * n, seed, B, edep)
+                dist.all_reduce(edep)
+                mc.mc_finalize(e.ctx, edep, n_job, B, h_dose, h_sigma)
+            g = mc.mc_export_grid(e.ctx)
+            tab_bytes = (1 + 3 * len(cfg["materials"]) + 6 * len(cfg["materials"])) * g["N"] * 8
+            e.close()
+
+        with torch.cuda.stream(stream):
+            e2e_step()
+            sync_all()
+            t0 = time.perf_counter()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(K):
+                e2e_step()
+            e1.record(stream)
+            sync_all()
+            wall = time.perf_counter() - t0
+        # the host work (table build, allocation) is part of the call: take the wall clock, max over ranks
+        tw = torch.tensor([max(wall, e0.elapsed_time(e1) * 1e-3)], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(tw, op=dist.ReduceOp.MAX)
+        h2d = nvox * 8 + tab_bytes + 3 * 4096 * 4  # packed (density, material) volume + tables + beam nodes
+        e2e = {"value": n_job * K / float(tw.item()), "unit": "histories/s", "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(2 * nvox * 4 + 5 * 4 + 12 * 8 + 3 * 8),
+               "what": "mc_create + mc_build_tables + mc_run(host dose, sigma) + mc_destroy per step"}
+
+    # ---- rooflines (rank 0's kernels) ----------------------------------------------------------------------
+    pk, pk_kind = peaks()
+    issue_peak = SM_COUNT * SCHEDULERS_PER_SM * LANES * pk["sm_max_mhz"] * 1e6  # thread-instructions / s
+    e_ms, p_ms = acc["electron_kernel_ms"], acc["photon_kernel_ms"]
+    alg_e = acc["n_electron_steps"] * INSTR_PER["e_step"] + (acc["n_moller"] + acc["n_brems"]) * INSTR_PER["hard_event"]
+    alg_p = acc["n_photon_flights"] * INSTR_PER["photon_flight"] + \
+        (acc["n_compton"] + acc["n_pair"] + acc["n_photoelectric"]) * INSTR_PER["photon_interaction"]
+    dom = "electron_kernel" if e_ms >= p_ms else "photon_kernel"
+    alg, kms = (alg_e, e_ms) if dom == "electron_kernel" else (alg_p, p_ms)
+    achieved = alg / (kms * 1e-3) if kms > 0 else 0.0
+    roofline = {"bound": "alu", "kernel": dom, "achieved": achieved / 1e12, "peak": issue_peak / 1e12,
+                "unit": "Tinstr/s (thread-instructions)", "frac": achieved / issue_peak, "traffic": None,
+                "peak_source": f"148 SM x 4 schedulers x 32 lanes x sm_max_mhz ({pk_kind} MEASURED_PEAKS.json clock)",
+                "kernel_ms_per_step": kms / K, "kernel_share_of_step": kms / total_ms if world == 1 else None}
+    # scoring roofline: measured red.global.add.f32 peak into a window the size of one batch grid
+    red_ms = min(mc.mc_bench_red(eng.ctx, nvox, 64, 0, SM_COUNT * 8) for _ in range(3))
+    red_peak = SM_COUNT * 8 * 256 * 64 / (red_ms * 1e-3)
+    red_rate = acc["n_dose_atomics"] / ((e_ms + p_ms) * 1e-3)
+    roofline_scoring = {"bound": "l2_atomic", "achieved": red_rate / 1e9, "peak": red_peak / 1e9, "unit": "Gred/s",
+                        "frac": red_rate / red_peak,
+                        "peak_source": "mc_bench_red: random cells of one batch grid, 148x8 CTAs x 256 thr x 64 reds, best of 3"}
+
+    if rank == 0:
+        out = {"metric": "histories/s", "value": n_job * K / (total_ms * 1e-3), "unit": "histories/s",
+               "n_gpus": world, "steps": K, "warmup": args.warmup, "ms_per_step": total_ms / K,
+               "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+               "data": "synthetic",
+               "config": config_dict(cfg, args, {"l2": "256 MiB fill between timed steps (L2 flush)",
+                                                 "parallelism": f"history ranges x{world}, all-reduce of batch grids" if world > 1 else "single GPU"}),
+               "e_steps_per_s": acc["n_electron_steps"] * world / (total_ms * 1e-3),
+               "photon_flights_per_s": acc["n_photon_flights"] * world / (total_ms * 1e-3),
+               "per_history": {"e_steps": acc["n_electron_steps"] / (n * K), "photon_flights": acc["n_photon_flights"] / (n * K),
+                               "fictitious_fraction": acc["n_fictitious"] / max(1, acc["n_photon_flights"]),
+                               "hard_events": (acc["n_moller"] + acc["n_brems"]) / (n * K),
+                               "dose_atomics": acc["n_dose_atomics"] / (n * K),
+                               "secondaries": (acc["n_secondary_electrons"] + acc["n_secondary_photons"]) / (n * K)},
+               "ledger_rel": abs(acc["e_deposited_MeV"] + acc["e_escaped_MeV"] - acc["e_source_MeV"]) / acc["e_source_MeV"],
+               "clocks": clocks, "e2e": e2e, "gpu_launches": int(acc["n_kernel_launches"]),
+               "roofline": roofline, "roofline_scoring": roofline_scoring}
+        # statistics of the result: mean sigma/D inside the 10 % isodose and time to 1 %
+        d, s = dose.cpu().numpy().astype(np.float64), sigma.cpu().numpy().astype(np.float64)
+        m = d >= 0.1 * d.max()
+        rel = float(np.mean(s[m] / d[m]))
+        out["mean_rel_sigma_10pct_isodose"] = rel
+        out["time_to_1pct_s"] = (total_ms / K * 1e-3) * (rel / 0.01) ** 2
+        if world == 1 and not args.no_cpu_baseline:
+            out["cpu_baseline"] = cpu_baseline(cfg)
+        print(json.dumps(out))
+    eng.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_engine(a)

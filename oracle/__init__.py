@@ -205,10 +205,20 @@ class Oracle:
         if workers <= 1:
             edep, st = self.run_edep(beam, n_histories, seed, n_batches)
         else:
-            edep, st = _run_sharded(self._ph, self._materials, self._params, beam, n_histories, seed, n_batches,
-                                    workers)
+            edep, st = _run_sharded(self, beam, n_histories, seed, n_batches, workers)
         dose, sig = self.finalize(edep, n_histories)
         return dose, sig, st
+
+    def run_sample(self, beam, n_total, n_sample, seed, n_batches, workers=1):
+        """Histories [0, n_sample) of a job of n_total, sharded over `workers` processes: edep[B, nvox],
+        stats, wall seconds (the timed CPU baseline of bench.py)."""
+        import time
+        t0 = time.perf_counter()
+        if workers <= 1:
+            edep, st = self.run_edep(beam, n_total, seed, n_batches, 0, n_sample)
+        else:
+            edep, st = _run_sharded(self, beam, n_total, seed, n_batches, workers, h_end=n_sample)
+        return edep, st, time.perf_counter() - t0
 
     def run_atten(self, beam, n, seed, tables_f32):
         """fp32 contract path (R20).  tables_f32: dict(lnE0, inv_dln, mu_maj[N], mu_tot/mu_C/mu_pp[n_mat,N])."""
@@ -268,21 +278,27 @@ def sample_ms(a, n, seed=1):
 
 
 # -- sharding over host cores -------------------------------------------------------------------
+_FORK_ORC = None  # the parent's Oracle, inherited by forked workers (tables are built once, not per chunk)
+
+
 def _shard(args):
-    ph, mats, par, beam, n_total, seed, B, h0, h1 = args
-    o = Oracle(ph, mats, par)
-    return o.run_edep(beam, n_total, seed, B, h0, h1)
+    beam, n_total, seed, B, h0, h1 = args
+    return _FORK_ORC.run_edep(beam, n_total, seed, B, h0, h1)
 
 
-def _run_sharded(ph, mats, par, beam, n_total, seed, B, workers):
-    # many small contiguous chunks, interleaved, so that every worker ends at about the same time
+def _run_sharded(orc, beam, n_total, seed, B, workers, h_end=None):
+    # many small contiguous chunks so that every worker ends at about the same time
+    global _FORK_ORC
     n_chunks = workers * 8
-    edges = np.linspace(0, n_total, n_chunks + 1).astype(np.int64)
-    jobs = [(ph, mats, par, beam, n_total, seed, B, int(edges[i]), int(edges[i + 1])) for i in range(n_chunks)
+    edges = np.linspace(0, n_total if h_end is None else h_end, n_chunks + 1).astype(np.int64)
+    jobs = [(beam, n_total, seed, B, int(edges[i]), int(edges[i + 1])) for i in range(n_chunks)
             if edges[i + 1] > edges[i]]
-    ctx = mp.get_context("fork")
-    with ctx.Pool(workers) as pool:
-        res = pool.map(_shard, jobs, chunksize=1)
+    _FORK_ORC = orc
+    try:
+        with mp.get_context("fork").Pool(workers) as pool:
+            res = pool.map(_shard, jobs, chunksize=1)
+    finally:
+        _FORK_ORC = None
     edep = sum(r[0] for r in res)
     st = {k: (max(r[1][k] for r in res) if k == "max_ledger_rel" else sum(r[1][k] for r in res)) for k in STAT_NAMES}
     return edep, st

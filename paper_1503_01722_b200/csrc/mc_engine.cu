@@ -290,6 +290,7 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, uint64_t n_total, uint64_t
     // ledger: deposited energy is the total of the batch grids
     sum_kernel<<<ctx->sm_count * 4, kThreads, 0, s>>>(d_edep, (size_t)n_batches * nvox, ctx->d_ledger + LG_DEP);
     CU(cudaGetLastError());
+    ++S.n_kernel_launches;
     unsigned long long hs[S_COUNT];
     double hl[LG_COUNT];
     CU(cudaMemcpyAsync(hs, ctx->d_stats, sizeof hs, cudaMemcpyDeviceToHost, s));
