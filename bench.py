@@ -188,9 +188,8 @@ def run_engine(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     cfg = workload(args)
     n, B, seed = cfg["n_histories"], cfg["n_batches"], cfg["seed"]
-    n_job = n * world  # weak scaling: every rank simulates n histories of one job of n * world
-    if n_job >= 2**32:
-        raise SystemExit("job too large: n_histories * gpus must be < 2^32")
+    from paper_1503_01722_b200 import sharding
+    n_job, h_lo, h_hi = sharding.history_range(rank, world, n)  # weak scaling: n histories per rank
     eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])
     for kv in args.option:
         k, v = kv.split("=")
@@ -207,9 +206,11 @@ def run_engine(args):
         if world == 1:
             mc.mc_run(eng.ctx, cfg["beam"], n, seed, B, dose, sigma)
         else:  # shard = contiguous history range; one exchange: sum of the per-batch grids
-            mc.mc_run_range(eng.ctx, cfg["beam"], n_job, rank * n, (rank + 1) * n, seed, B, edep)
-            dist.all_reduce(edep)
-            mc.mc_finalize(eng.ctx, edep, n_job, B, dose, sigma)
+            def run_range(nj, a, b):
+                mc.mc_run_range(eng.ctx, cfg["beam"], nj, a, b, seed, B, edep)
+                return edep
+            sharding.run_sharded(rank, world, n, run_range, dist.all_reduce,
+                                 lambda g, nj: mc.mc_finalize(eng.ctx, g, nj, B, dose, sigma))
         return mc.mc_get_stats(eng.ctx)
 
     def sync_all():
@@ -257,9 +258,11 @@ def run_engine(args):
             if world == 1:
                 mc.mc_run(e.ctx, cfg["beam"], n, seed, B, h_dose, h_sigma)
             else:
-                mc.mc_run_range(e.ctx, cfg["beam"], n_job, rank * n, (rank + 1) * n, seed, B, edep)
-                dist.all_reduce(edep)
-                mc.mc_finalize(e.ctx, edep, n_job, B, h_dose, h_sigma)
+                def run_range(nj, a, b):
+                    mc.mc_run_range(e.ctx, cfg["beam"], nj, a, b, seed, B, edep)
+                    return edep
+                sharding.run_sharded(rank, world, n, run_range, dist.all_reduce,
+                                     lambda g, nj: mc.mc_finalize(e.ctx, g, nj, B, h_dose, h_sigma))
             g = mc.mc_export_grid(e.ctx)
             tab_bytes = (1 + 3 * len(cfg["materials"]) + 6 * len(cfg["materials"])) * g["N"] * 8
             e.close()

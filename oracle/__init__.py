@@ -174,21 +174,30 @@ class Oracle:
         return lib().orc_material_scalar(self._h, int(m), {"ne": 0, "ZA": 1, "Cbr": 2, "Lscr": 3}[name])
 
     # -- transport ------------------------------------------------------------------------------
-    def run_edep(self, beam, n_total, seed, n_batches, h0=0, h1=None, first=False):
+    def run_edep(self, beam, n_total, seed, n_batches, h0=0, h1=None, first=False, window=False):
         """Energy deposited per batch grid [B, nvox] (MeV, fp64) for histories [h0, h1) + stats dict.
-        first=True also returns (voxel, channel) of each primary photon's first real interaction."""
+        first=True also returns (voxel, channel) of each primary photon's first real interaction.
+        window=True returns (b_lo, grids[b_lo..b_hi]) — only the batches this history range touches
+        (batch of h = floor(h*B/N)); harness-side memory saving, the oracle's arithmetic is unchanged."""
         h1 = n_total if h1 is None else h1
         b, keep = _beam_struct(beam)
-        edep = np.zeros((n_batches, self.nvox))
+        b_lo, b_hi = 0, n_batches - 1
+        if window and h1 > h0:
+            b_lo, b_hi = (h0 * n_batches) // n_total, ((h1 - 1) * n_batches) // n_total
+        edep = np.zeros((b_hi - b_lo + 1, self.nvox))
         st = np.zeros(lib().orc_n_stats())
         fv = np.zeros(h1 - h0, np.int32) if first else None
         fc = np.zeros(h1 - h0, np.int32) if first else None
+        # orc_run indexes edep + batch*nvox: hand it the address batch b_lo would have in a full array
+        base = C.cast(C.c_void_p(edep.ctypes.data - b_lo * self.nvox * 8), C.POINTER(C.c_double))
         rc = lib().orc_run(self._h, C.byref(b), C.c_uint64(h0), C.c_uint64(h1), C.c_uint64(n_total),
-                           C.c_uint64(seed), int(n_batches), _dp(edep), _dp(st),
+                           C.c_uint64(seed), int(n_batches), base, _dp(st),
                            fv.ctypes.data_as(C.c_void_p) if first else None,
                            fc.ctypes.data_as(C.c_void_p) if first else None)
         if rc:
             raise ValueError(f"orc_run failed ({rc})")
+        if window:
+            return b_lo, edep, dict(zip(STAT_NAMES, st))
         if first:
             return edep, dict(zip(STAT_NAMES, st)), fv, fc
         return edep, dict(zip(STAT_NAMES, st))
@@ -208,6 +217,12 @@ class Oracle:
             edep, st = _run_sharded(self, beam, n_histories, seed, n_batches, workers)
         dose, sig = self.finalize(edep, n_histories)
         return dose, sig, st
+
+    def run_edep_parallel(self, beam, n_histories, seed, n_batches, workers):
+        """run_edep over `workers` processes (disjoint history ranges): edep[B, nvox], stats."""
+        if workers <= 1:
+            return self.run_edep(beam, n_histories, seed, n_batches)
+        return _run_sharded(self, beam, n_histories, seed, n_batches, workers)
 
     def run_sample(self, beam, n_total, n_sample, seed, n_batches, workers=1):
         """Histories [0, n_sample) of a job of n_total, sharded over `workers` processes: edep[B, nvox],
@@ -283,24 +298,28 @@ _FORK_ORC = None  # the parent's Oracle, inherited by forked workers (tables are
 
 def _shard(args):
     beam, n_total, seed, B, h0, h1 = args
-    return _FORK_ORC.run_edep(beam, n_total, seed, B, h0, h1)
+    return _FORK_ORC.run_edep(beam, n_total, seed, B, h0, h1, window=True)
 
 
 def _run_sharded(orc, beam, n_total, seed, B, workers, h_end=None):
-    # many small contiguous chunks so that every worker ends at about the same time
+    # many small contiguous chunks so that every worker ends at about the same time; a chunk returns
+    # only the batch grids its history range touches
     global _FORK_ORC
     n_chunks = workers * 8
     edges = np.linspace(0, n_total if h_end is None else h_end, n_chunks + 1).astype(np.int64)
     jobs = [(beam, n_total, seed, B, int(edges[i]), int(edges[i + 1])) for i in range(n_chunks)
             if edges[i + 1] > edges[i]]
     _FORK_ORC = orc
+    edep = np.zeros((B, orc.nvox))
+    stats = []
     try:
         with mp.get_context("fork").Pool(workers) as pool:
-            res = pool.map(_shard, jobs, chunksize=1)
+            for b_lo, part, st in pool.imap_unordered(_shard, jobs, chunksize=1):
+                edep[b_lo:b_lo + part.shape[0]] += part
+                stats.append(st)
     finally:
         _FORK_ORC = None
-    edep = sum(r[0] for r in res)
-    st = {k: (max(r[1][k] for r in res) if k == "max_ledger_rel" else sum(r[1][k] for r in res)) for k in STAT_NAMES}
+    st = {k: (max(r[k] for r in stats) if k == "max_ledger_rel" else sum(r[k] for r in stats)) for k in STAT_NAMES}
     return edep, st
 
 

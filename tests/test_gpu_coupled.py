@@ -1,0 +1,322 @@
+"""Coupled-mode parity of the CUDA path against the oracle (run on the B200 box with -m gpu); every
+call goes through the C ABI.
+
+Bars (BASELINE.json north_star, R19):
+  * mean |D_gpu - D_orc| / Dmax over the 10 % isodose <= 1 %
+  * >= 99 % of those voxels within 3 combined batch sigma
+The oracle runs once per case (seed 1, 40 batches: R19).  The engine runs twice:
+  seed 1 — the SAME Philox streams as the oracle: the statistical noise largely cancels, so the 1 % bar is
+           applied strictly (a physics difference shows as a bias);
+  seed 2 — independent streams: the 3-sigma criterion proper; the mean |difference| bar is then
+           1 % + E|noise| = 1 % + 0.8 * mean(sigma_comb)/Dmax (half-normal mean), stated here once.
+Event counters per history (flights, fictitious, Compton, pair, photoelectric, Moller, brems) must agree within 1 %
+and the energy ledger of every engine run must close.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import paper_1503_01722_b200 as mc
+from paper_1503_01722_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+WORKERS = min(oracle.host_cores(), 32)
+B_ORC = 40
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_gpu():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_1503_01722_b200 import build
+    build.build()
+
+
+def _metrics(dg, sg, do, so):
+    dg, sg = dg.astype(np.float64), sg.astype(np.float64)
+    m = do >= 0.1 * do.max()
+    diff = np.abs(dg[m] - do[m])
+    comb = np.sqrt(sg[m] ** 2 + so[m] ** 2)
+    return {"n": int(m.sum()), "mean_diff": float(diff.mean() / do.max()),
+            "frac3": float(np.mean(diff <= 3.0 * comb)), "noise": float(0.8 * comb.mean() / do.max())}
+
+
+EVENTS = ("flights", "fictitious", "compton", "pair", "photoelectric", "moller", "brems")
+
+
+def _per_history(st, n):
+    return {"e_steps": st["n_electron_steps"] / n, "flights": st["n_photon_flights"] / n,
+            "fictitious": st["n_fictitious"] / n, "compton": st["n_compton"] / n, "pair": st["n_pair"] / n,
+            "photoelectric": st["n_photoelectric"] / n, "moller": st["n_moller"] / n, "brems": st["n_brems"] / n}
+
+
+def _per_history_orc(st, n):
+    return {"e_steps": st["n_estep"] / n, "flights": st["n_flight"] / n, "fictitious": st["n_fict"] / n,
+            "compton": st["n_compton"] / n, "pair": st["n_pair"] / n, "photoelectric": st["n_pe"] / n,
+            "moller": st["n_moller"] / n, "brems": st["n_brems"] / n}
+
+
+def _ledger(st):
+    return abs(st["e_deposited_MeV"] + st["e_escaped_MeV"] - st["e_source_MeV"]) / st["e_source_MeV"]
+
+
+def _block_dose(edep, rho, dims, voxel_cm, n_total, f):
+    """Dose and batch sigma on f x f x f voxel blocks from per-batch energy grids [B, nvox] (MeV): the R17 / R18
+    definitions written out in numpy on block sums — a property that holds at any size, used where the oracle
+    cannot afford the statistics of the fine grid."""
+    B = edep.shape[0]
+    nx, ny, nz = dims
+    cx, cy, cz = nx // f, ny // f, nz // f
+
+    def blocks(a):
+        a = a.reshape(nz, ny, nx)[:cz * f, :cy * f, :cx * f]
+        return a.reshape(cz, f, cy, f, cx, f).sum(axis=(1, 3, 5)).reshape(-1)
+
+    mass = blocks(rho.astype(np.float64)) * float(np.prod(voxel_cm))
+    nb = np.array([-(-(b + 1) * n_total // B) - -(-b * n_total // B) for b in range(B)], np.float64)  # ceil edges
+    D = np.stack([blocks(edep[b].astype(np.float64)) / (mass * nb[b]) for b in range(B)])
+    mean = D.mean(axis=0)
+    return mean, np.sqrt(((D - mean) ** 2).sum(axis=0) / (B * (B - 1)))
+
+
+def _engine_run(eng, cfg, n, seed, coarse):
+    ph = cfg["phantom"]
+    B = cfg["n_batches"]
+    if coarse == 1:
+        dg, sg = eng.run(cfg["beam"], n, seed, B)
+    else:
+        edep = np.zeros((B, eng.nvox), np.float32)
+        mc.mc_run_range(eng.ctx, cfg["beam"], n, 0, n, seed, B, edep)
+        dg, sg = _block_dose(edep, ph["density"], eng.dims, ph["voxel_cm"], n, coarse)
+    st = eng.stats()
+    assert st["n_histories"] == n
+    assert _ledger(st) < 1e-4, f"engine energy ledger open: {_ledger(st)}"
+    return dg, sg, st
+
+
+def _run_case(cfg, n_gpu, n_orc, coarse=1):
+    """Oracle: n_orc histories, seed 1.  Engine: seed 1 with n_orc histories (same streams, same batches up to
+    the batch count) and seed 2 with n_gpu histories (independent, the size bench.py times)."""
+    ph = cfg["phantom"]
+    eng = mc.Engine(ph, cfg["materials"], cfg["params"])
+    orc = oracle.Oracle(ph, cfg["materials"], cfg["params"])
+    eo, sto = orc.run_edep_parallel(cfg["beam"], n_orc, 1, B_ORC, WORKERS)
+    assert sto["max_ledger_rel"] < 1e-5
+    if coarse == 1:
+        do, so = orc.finalize(eo, n_orc)
+    else:
+        do, so = _block_dose(eo, ph["density"], eng.dims, ph["voxel_cm"], n_orc, coarse)
+    del eo
+    out = {}
+    for seed, n in ((1, n_orc), (2, n_gpu)):
+        dg, sg, st = _engine_run(eng, cfg, n, seed, coarse)
+        out[seed] = _metrics(dg, sg, do, so)
+        out[seed]["per_history"] = _per_history(st, n)
+    eng.close()
+    out["orc_per_history"] = _per_history_orc(sto, n_orc)
+    out["n_gpu"], out["n_orc"] = n_gpu, n_orc
+    return out
+
+
+def _check(out):
+    ref = out["orc_per_history"]
+    for seed in (1, 2):
+        r = out[seed]
+        for k in EVENTS:  # physics events per history: 1 %, or 5 standard errors of the count where that is larger
+            tol = max(0.01 * ref[k], 5.0 * np.sqrt(2.0 * max(ref[k], 1e-9) / min(out["n_gpu"], out["n_orc"])), 1e-4)
+            assert abs(r["per_history"][k] - ref[k]) <= tol, (seed, k, r["per_history"][k], ref[k], tol)
+        # Condensed-history steps: a voxel-limited step whose second leg ends a hair short of the face is
+        # followed by a tiny catch-up step; whether "short" or "on the face" is decided in fp32 here and in
+        # fp64 in the oracle (tolerance note), so the count differs by a few per cent while
+        # path, energy loss and dose do not.
+        assert r["per_history"]["e_steps"] == pytest.approx(ref["e_steps"], rel=0.08), (seed, r["per_history"], ref)
+        assert r["n"] > 0
+    same, indep = out[1], out[2]
+    assert same["mean_diff"] <= 0.01, same
+    assert indep["frac3"] >= 0.99, indep
+    assert indep["mean_diff"] <= 0.01 + indep["noise"], indep
+    # the independent run's difference must be explained by its noise (no hidden bias)
+    assert indep["mean_diff"] <= 1.25 * indep["noise"] + 0.002, indep
+
+
+# ---- the five BASELINE configs -------------------------------------------------------------------------
+def test_config1_electron_pencil_water_full_size():
+    cfg = W.config(1)
+    _check(_run_case(cfg, cfg["n_histories"], cfg["n_histories"]))
+
+
+def test_config2_15MeV_electrons_water_full_size():
+    cfg = W.config(2)
+    _check(_run_case(cfg, cfg["n_histories"], cfg["n_histories"]))
+
+
+def test_config3_6MV_photons_water_full_size_engine():
+    """Engine at the full 1e8 histories (the launch configuration bench.py --config 3 times); the oracle at
+    4e7 histories (its sigma enters the combined sigma)."""
+    cfg = W.config(3)
+    _check(_run_case(cfg, cfg["n_histories"], 4 * 10 ** 7))
+
+
+def test_config4_slab_electrons_full_size():
+    cfg = W.config(4, "e")
+    _check(_run_case(cfg, cfg["n_histories"], cfg["n_histories"]))
+
+
+def test_config4_slab_photons_full_size_engine():
+    cfg = W.config(4, "g")
+    _check(_run_case(cfg, cfg["n_histories"], 4 * 10 ** 7))
+
+
+def test_config5_halfslab_electrons_full_size_engine_coarse_blocks():
+    """122x122x120 at 0.25 cm, 1e8 electron histories on the engine; the oracle affords 4e6, so the dose is
+    compared on 4x4x4 voxel blocks (1 cm^3), where its noise is below the 1 % bar."""
+    cfg = W.config(5, "e")
+    _check(_run_case(cfg, cfg["n_histories"], 4 * 10 ** 6, coarse=4))
+
+
+def test_config5_halfslab_photons_full_size_engine_coarse_blocks():
+    cfg = W.config(5, "g")
+    _check(_run_case(cfg, cfg["n_histories"], 4 * 10 ** 7, coarse=4))
+
+
+# ---- physics switches, particle types, edge cases ---------------------------------------------------------
+def _small_case(flags=0, particle=W.ELECTRON, energy=6.0, n=200000, shape=W.PENCIL, phantom=None):
+    ph = phantom or W.homogeneous_phantom((12, 12, 16), 0.5)
+    cfg = {"phantom": ph, "materials": W.materials(3), "params": W.params(flags=flags),
+           "beam": W.beam(particle, shape, energy=energy, field=(3.0, 3.0)), "n_batches": 10}
+    return cfg, n
+
+
+@pytest.mark.parametrize("flags", [W.FLAG_NO_HARD, W.FLAG_NO_MS, W.FLAG_LOCAL_SECONDARIES,
+                                   W.FLAG_NO_HARD | W.FLAG_NO_MS])
+def test_physics_switches_match_the_oracle_with_the_same_switches(flags):
+    cfg, n = _small_case(flags=flags)
+    out = _run_case(cfg, n, n)
+    print(flags, out)
+    _check(out)
+    if flags & W.FLAG_NO_HARD:
+        assert out[1]["per_history"]["moller"] == 0 and out[1]["per_history"]["brems"] == 0
+
+
+def test_no_ms_no_hard_pencil_beam_stays_on_its_column():
+    """Without deflection and hard events a pencil beam deposits only along its own voxel column, down to the
+    CSDA range: an exact structural property."""
+    cfg, n = _small_case(flags=W.FLAG_NO_HARD | W.FLAG_NO_MS, n=5000)
+    cfg["beam"] = W.beam(W.ELECTRON, W.PENCIL, energy=6.0, entry=(0.1, 0.1, 0.0))
+    eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])
+    d, s = eng.run(cfg["beam"], n, 3, 10)
+    d = d.reshape(16, 12, 12)
+    col = d[:, 6, 6]
+    assert d.sum() == pytest.approx(col.sum(), rel=1e-6)
+    assert np.all(s.reshape(16, 12, 12)[:, 6, 6] < 1e-6 * col.max() + 1e-12)  # every history is identical
+    orc = oracle.Oracle(cfg["phantom"], cfg["materials"], cfg["params"])
+    do, _, _ = orc.run(cfg["beam"], 10, 3, 2)
+    assert np.allclose(col, do.reshape(16, 12, 12)[:, 6, 6], rtol=2e-4, atol=1e-6 * col.max())
+    eng.close()
+
+
+def test_positron_beam_with_annihilation_photons():
+    cfg, n = _small_case(particle=W.POSITRON, energy=4.0, n=300000)
+    out = _run_case(cfg, n, n)
+    print(out)
+    _check(out)
+    assert out[1]["per_history"]["flights"] > 2.0  # two annihilation photons per history are transported
+
+
+def test_high_energy_photons_in_bone_pair_production():
+    ph = W.homogeneous_phantom((10, 10, 30), 0.5, material=1, density=1.85)
+    cfg, n = _small_case(particle=W.PHOTON, energy=18.0, n=1000000, shape=W.POINT_RECT, phantom=ph)
+    out = _run_case(cfg, n, n)
+    print(out)
+    _check(out)
+
+
+def test_run_range_plus_finalize_equals_run_and_device_outputs():
+    import torch
+    cfg = W.config(1)
+    n, B = 50000, 10
+    eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])
+    d0, s0 = eng.run(cfg["beam"], n, 9, B)
+    # two shards into separate grids, summed on the device, finalized
+    e1 = torch.zeros(B * eng.nvox, dtype=torch.float32, device="cuda")
+    e2 = torch.zeros_like(e1)
+    mc.mc_run_range(eng.ctx, cfg["beam"], n, 0, 17001, 9, B, e1)
+    mc.mc_run_range(eng.ctx, cfg["beam"], n, 17001, n, 9, B, e2)
+    e1 += e2
+    torch.cuda.synchronize()
+    d1 = torch.zeros(eng.nvox, dtype=torch.float32, device="cuda")
+    s1 = torch.zeros_like(d1)
+    mc.mc_finalize(eng.ctx, e1, n, B, d1, s1)
+    # deterministic per history; grid sums differ only by fp32 summation order
+    assert np.allclose(d1.cpu().numpy(), d0, rtol=2e-5, atol=1e-7 * d0.max())
+    assert np.allclose(s1.cpu().numpy(), s0, rtol=5e-3, atol=1e-6 * d0.max())
+    # ragged batches: n not a multiple of B; n == B (one history per batch)
+    d2, s2 = eng.run(cfg["beam"], 1003, 9, 7)
+    assert np.isfinite(d2).all() and d2.max() > 0
+    d3, s3 = eng.run(cfg["beam"], 5, 9, 5)
+    assert np.isfinite(d3).all() and np.isfinite(s3).all()
+    eng.close()
+
+
+def test_finalize_kernel_against_the_oracle_statistics():
+    cfg = W.config(1)
+    eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])
+    orc = oracle.Oracle(cfg["phantom"], cfg["materials"], cfg["params"])
+    rng = np.random.default_rng(0)
+    B, n = 7, 1003
+    edep = rng.gamma(2.0, 1.0, (B, eng.nvox)).astype(np.float32)
+    d, s = np.zeros(eng.nvox, np.float32), np.zeros(eng.nvox, np.float32)
+    mc.mc_finalize(eng.ctx, edep, n, B, d, s)
+    do, so = orc.finalize(edep.astype(np.float64), n)
+    assert np.allclose(d, do, rtol=1e-6) and np.allclose(s, so, rtol=1e-5)
+    eng.close()
+
+
+def test_beam_that_misses_and_energy_ledger_of_escapes():
+    cfg = W.config(1)
+    eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])
+    miss = W.beam(W.ELECTRON, W.PENCIL, energy=6.0, entry=(40.0, 0.0, 0.0))
+    d, s = eng.run(miss, 1000, 1, 4)
+    st = eng.stats()
+    assert d.max() == 0 and s.max() == 0
+    assert st["e_escaped_MeV"] == pytest.approx(6000.0, rel=1e-6) and st["n_electron_steps"] == 0
+    eng.close()
+
+
+def test_queue_overflow_is_reported_never_dropped():
+    """R21: a queue too small for the secondaries of one wave -> MC_ERR_QUEUE_OVERFLOW, no result."""
+    cfg = W.config(2)
+    eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])
+    mc.mc_set_option(eng.ctx, "wave_size", 4096)
+    mc.mc_set_option(eng.ctx, "queue_factor", 2)
+    with pytest.raises(mc.McError) as e:
+        eng.run(cfg["beam"], 200000, 1, 10)
+    assert e.value.status == mc.MC_ERR_QUEUE_OVERFLOW
+    # and the same context recovers with a sufficient queue
+    mc.mc_set_option(eng.ctx, "queue_factor", 16)
+    d, _ = eng.run(cfg["beam"], 200000, 1, 10)
+    st = eng.stats()
+    assert _ledger(st) < 1e-4 and d.max() > 0
+    eng.close()
+
+
+def test_scheduling_options_do_not_change_the_result():
+    """R14: wave size / refill threshold / blocks per SM are launch-order knobs; every history keeps its own
+    stream, so the grids agree to fp32 summation order."""
+    cfg = W.config(4, "e")
+    n, B = 100000, 10
+    ref = None
+    for opts in ({}, {"wave_size": 8192, "queue_factor": 16}, {"refill_lanes": 1}, {"refill_lanes": 32, "blocks_per_sm": 1}):
+        eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])
+        for k, v in opts.items():
+            mc.mc_set_option(eng.ctx, k, v)
+        d, _ = eng.run(cfg["beam"], n, 4, B)
+        st = eng.stats()
+        key = (st["n_electron_steps"], st["n_photon_flights"], st["n_moller"], st["n_brems"])
+        if ref is None:
+            ref = (d, key)
+        else:
+            assert key == ref[1], opts
+            assert np.allclose(d, ref[0], rtol=1e-4, atol=1e-6 * ref[0].max()), opts
+        eng.close()
