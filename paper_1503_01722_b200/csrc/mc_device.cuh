@@ -14,6 +14,19 @@ constexpr int MAX_MAT = 8;
 constexpr float kMeF = 0.51099895f;
 constexpr float kTwoPiF = 6.28318530717958647692f;
 
+// ---- single-instruction MUFU wrappers (approx, flush-to-zero): the transport kernels' fast math ------------
+__device__ __forceinline__ float f_rcp(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float f_lg2(float x) { float r; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float f_ex2(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float f_sqrt(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float f_rsqrt(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float f_sin(float x) { float r; asm("sin.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float f_cos(float x) { float r; asm("cos.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+constexpr float kLn2F = 0.69314718055994530942f;
+constexpr float kLog2eF = 1.44269504088896340736f;
+__device__ __forceinline__ float f_ln(float x) { return f_lg2(x) * kLn2F; }
+__device__ __forceinline__ float f_exp(float x) { return f_ex2(x * kLog2eF); }
+
 // ---- parameters handed to every kernel by value ------------------------------------------------
 struct Geometry {
     int nx, ny, nz, nvox;
@@ -66,6 +79,9 @@ struct RunParams {
     unsigned long long* stats;  // StatId
     double* ledger;           // e_src, e_dep, e_esc
     int refill_lanes, aggregate;
+    int hard_lanes;           // lanes of a warp that must hold a pending hard event before the warp runs that block
+    // table coordinate <-> energy in base 2: ex = lg2(T) * ex_a - ex_b;  T = ex2(ex * t_a + t_b)
+    float ex_a, ex_b, t_a, t_b;
 };
 
 // ---- Philox4x32-10 -----------------------------------------------------------------------------
@@ -89,6 +105,9 @@ __device__ __forceinline__ uint4 next_block(Rng& r, uint32_t seed_lo, uint32_t s
 }
 // u = ((w >> 9) + 0.5) * 2^-23 in (0, 1): exact in fp32
 __device__ __forceinline__ float u01(uint32_t w) { return __fmul_rn(__fadd_rn((float)(w >> 9), 0.5f), 1.1920928955078125e-07f); }
+
+// same value as u01 (both exact in fp32), one FFMA
+__device__ __forceinline__ float u01f(uint32_t w) { return fmaf((float)(w >> 9), 1.1920928955078125e-07f, 5.9604644775390625e-08f); }
 
 // ---- fp32 arithmetic contract (R20) -----------------------------------------------------------
 __device__ __forceinline__ float c_ln(float x) {
@@ -162,6 +181,24 @@ __device__ __forceinline__ void rotate(float& u, float& v, float& w, float omu, 
     }
     float n = rsqrtf(fmaf(nu, nu, fmaf(nv, nv, nw * nw)));
     u = nu * n; v = nv * n; w = nw * n;
+}
+
+// Same rotation with single-instruction MUFU ops, no divergent branch, first-order renormalisation.
+// sphi, cphi: sine and cosine of the azimuth.
+__device__ __forceinline__ void rotate_fast(float& u, float& v, float& w, float omu, float sphi, float cphi) {
+    float mu = 1.0f - omu;
+    float st = f_sqrt(fmaxf(omu * (2.0f - omu), 0.0f));
+    float s2 = fmaf(-w, w, 1.0f);
+    bool pole = s2 < 1e-6f;
+    float is = f_rsqrt(fmaxf(s2, 1e-12f));
+    float a = st * cphi * is, b = st * sphi * is;
+    float nu = fmaf(u, mu, fmaf(u * w, a, -v * b));
+    float nv = fmaf(v, mu, fmaf(v * w, a, u * b));
+    float nw = fmaf(w, mu, -s2 * a);
+    nu = pole ? st * cphi : nu; nv = pole ? st * sphi : nv; nw = pole ? (w >= 0.0f ? mu : -mu) : nw;
+    float n2 = fmaf(nu, nu, fmaf(nv, nv, nw * nw));
+    float sc = fmaf(-0.5f, n2, 1.5f);  // 1/sqrt(n2) to first order around 1 (|n2 - 1| ~ 1e-6)
+    u = nu * sc; v = nv * sc; w = nw * sc;
 }
 
 // ---- source (R13), arithmetic contract ----------------------------------------------------------

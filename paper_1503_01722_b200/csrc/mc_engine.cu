@@ -43,7 +43,7 @@ struct mc_ctx {
     float* d_beam = nullptr;  // E nodes, pdf nodes, cdf: 3 x kMaxNodes
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     // options (M "manually adjusted")
-    int64_t wave_size = 1 << 22, queue_factor = 6, blocks_per_sm = 0, refill_lanes = 4, aggregate = 0;
+    int64_t wave_size = 1 << 22, queue_factor = 6, blocks_per_sm = 0, refill_lanes = 8, aggregate = 0, hard_lanes = 8;
     mc_stats stats{};
     std::string err;
 };
@@ -125,7 +125,9 @@ mc_status upload_tables(mc_ctx* ctx) {
     return MC_OK;
 }
 
-size_t smem_e(const mc_ctx* c) { return (size_t)c->tabs.n_mat * TE_COUNT * c->tabs.N * sizeof(float2); }
+size_t smem_e(const mc_ctx* c) {  // tables + per-thread counters + per-thread energy ledger
+    return (size_t)c->tabs.n_mat * TE_COUNT * c->tabs.N * sizeof(float2) + (size_t)SE_COUNT * kThreadsE * sizeof(uint32_t) + 2 * (size_t)kThreadsE * sizeof(double);
+}
 size_t smem_p(const mc_ctx* c) { return (size_t)(1 + c->tabs.n_mat * TP_COUNT) * c->tabs.N * sizeof(float2); }
 
 mc_status check_beam(mc_ctx* ctx, const mc_beam* b) {
@@ -187,7 +189,10 @@ void fill_params(const mc_ctx* ctx, RunParams& P) {
     for (int m = 0; m < MAX_MAT; ++m) P.lscr[m] = m < t.n_mat ? t.lscr[m] : 0.0f;
     P.flags = ctx->params.flags;
     P.counters = ctx->d_counters; P.stats = ctx->d_stats; P.ledger = ctx->d_ledger;
-    P.refill_lanes = (int)ctx->refill_lanes; P.aggregate = (int)ctx->aggregate;
+    P.refill_lanes = (int)ctx->refill_lanes; P.aggregate = (int)ctx->aggregate; P.hard_lanes = (int)ctx->hard_lanes;
+    const double ln2 = 0.69314718055994530942, log2e = 1.44269504088896340736;
+    P.ex_a = (float)(ln2 / t.dln); P.ex_b = (float)(t.lnE0 / t.dln);
+    P.t_a = (float)(t.dln * log2e); P.t_b = (float)(t.lnE0 * log2e);
 }
 
 }  // namespace
@@ -207,7 +212,7 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, uint64_t n_total, uint64_t
     CU(cudaFuncSetAttribute(electron_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)se));
     CU(cudaFuncSetAttribute(photon_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp));
     int occ_e = 0, occ_p = 0;
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_e, electron_kernel, kThreads, se));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_e, electron_kernel, kThreadsE, se));
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, photon_kernel, kThreads, sp));
     if (occ_e < 1 || occ_p < 1) return fail(ctx, MC_ERR_CUDA, "kernel does not fit on an SM");
     if (ctx->blocks_per_sm > 0) { occ_e = std::min<int>(occ_e, (int)ctx->blocks_per_sm); occ_p = std::min<int>(occ_p, (int)ctx->blocks_per_sm); }
@@ -258,8 +263,8 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, uint64_t n_total, uint64_t
         Queue qe_oth{ctx->d_q[1 - cur], ctx->d_counters + C_E_A + (1 - cur), ctx->q_cap};
         Queue qp{ctx->d_q[2], ctx->d_counters + C_P, ctx->q_cap};
         const uint64_t items = (uint64_t)n_in + n_new;
-        const int occ = run_p ? occ_p : occ_e;
-        int grid = (int)std::min<uint64_t>((uint64_t)ctx->sm_count * occ, (items + kThreads - 1) / kThreads);
+        const int occ = run_p ? occ_p : occ_e, thr = run_p ? kThreads : kThreadsE;
+        int grid = (int)std::min<uint64_t>((uint64_t)ctx->sm_count * occ, (items + thr - 1) / thr);
         grid = std::max(grid, 1);
         CU(cudaEventRecord(ctx->ev[2], s));
         if (run_p) {
@@ -267,7 +272,7 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, uint64_t n_total, uint64_t
             photon_kernel<<<grid, kThreads, sp, s>>>(P);
         } else {
             P.q_in = qe_cur; P.q_e_out = qe_oth; P.q_p_out = qp;
-            electron_kernel<<<grid, kThreads, se, s>>>(P);
+            electron_kernel<<<grid, kThreadsE, se, s>>>(P);
         }
         CU(cudaGetLastError());
         CU(cudaEventRecord(ctx->ev[3], s));
@@ -587,6 +592,7 @@ mc_status mc_set_option(mc_ctx* ctx, const char* name, int64_t value) {
     else if (n == "queue_factor") { if (value < 2 || value > 64) return fail(ctx, MC_ERR_INVALID_ARG, "queue_factor in [2, 64]"); ctx->queue_factor = value; }
     else if (n == "blocks_per_sm") { if (value < 0 || value > 32) return fail(ctx, MC_ERR_INVALID_ARG, "blocks_per_sm in [0, 32]"); ctx->blocks_per_sm = value; }
     else if (n == "refill_lanes") { if (value < 1 || value > 32) return fail(ctx, MC_ERR_INVALID_ARG, "refill_lanes in [1, 32]"); ctx->refill_lanes = value; }
+    else if (n == "hard_lanes") { if (value < 1 || value > 32) return fail(ctx, MC_ERR_INVALID_ARG, "hard_lanes in [1, 32]"); ctx->hard_lanes = value; }
     else if (n == "aggregate") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "aggregate in {0, 1}"); ctx->aggregate = value; }
     else return fail(ctx, MC_ERR_INVALID_ARG, "unknown option: " + n);
     return MC_OK;

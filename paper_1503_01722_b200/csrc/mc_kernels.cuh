@@ -46,14 +46,21 @@ __device__ __forceinline__ float face_dist(const Geometry& g, float x, float y, 
 }
 
 // Table coordinate (node + fraction) of the energy whose residual range is Rt: exact inverse of the
-// piecewise-linear (in ln T) range interpolant (R5); search starts at a first-order guess.
-__device__ __forceinline__ float inv_range_coord(const float2* R, float Rt, int guess, int k_cut, int N) {
+// piecewise-linear (in ln T) range interpolant (R5).  The bracket search starts at `guess` (callers pass
+// the constant-L estimate ex + ln(1 - rho d L/T)/dln, which is within a fraction of a node) and needs one shared
+// load per probe: node lo brackets Rt iff 0 <= (Rt - R[lo]) / (R[lo+1] - R[lo]) < 1.
+__device__ __forceinline__ float inv_range_coord(const float2* R, float Rt, float guess, int k_cut, int N) {
     if (Rt <= 0.0f) return (float)k_cut;
-    int lo = min(max(guess, k_cut), N - 2);
-    while (lo > k_cut && R[lo].x > Rt) --lo;
-    while (lo < N - 2 && R[lo + 1].x <= Rt) ++lo;
-    float2 a = R[lo];
-    float f = __fdividef(Rt - a.x, a.y);
+    int lo = min(max((int)guess, k_cut), N - 2);
+    float f;
+    int way = 0;  // the walk never turns round: a value in the rounding gap between two segments ends it
+    for (;;) {
+        float2 a = R[lo];
+        f = (Rt - a.x) * f_rcp(a.y);
+        if (f < 0.0f && lo > k_cut && way <= 0) { --lo; way = -1; }
+        else if (f >= 1.0f && lo < N - 2 && way >= 0) { ++lo; way = 1; }
+        else break;
+    }
     return (float)lo + fminf(fmaxf(f, 0.0f), 1.0f);
 }
 
@@ -95,226 +102,297 @@ __device__ __forceinline__ void emit(const RunParams& P, const Queue& q, Score& 
 
 // =================================================================================================
 // electron / positron kernel
+//
+// One lane = one track.  A warp executes, per iteration, ONE of three blocks for the lanes that want it:
+//   STEP   one condensed-history step (S4-S6, S8)            — lanes in state L_STEP
+//   HARD   hard-event thinning + Moller / bremsstrahlung (S7) — lanes in state L_HARD (pending)
+//   REFILL queue pop / source generation (S0, S1)            — lanes in state L_IDLE
+// Divergent work is deferred until enough lanes of the warp want it (hard_lanes / refill_lanes) or nothing
+// else can run, so the rare blocks run with many lanes instead of one or two (profiles/README.md).
 // =================================================================================================
-__global__ void __launch_bounds__(kThreads) electron_kernel(const __grid_constant__ RunParams P) {
+constexpr int kThreadsE = 128;
+enum LaneState { L_IDLE = 0, L_STEP = 1, L_HARD = 2, L_DONE = 3 };
+enum { SE_STEP = 0, SE_MOLLER, SE_BREMS, SE_SEC_E, SE_SEC_G, SE_HIST, SE_RED, SE_COUNT };
+
+// distances along (u,v,w) to the three faces of voxel (ix,iy,iz) the direction points at
+__device__ __forceinline__ void face_all(const Geometry& g, float x, float y, float z, float u, float v, float w, int ix, int iy,
+                                         int iz, float& tx, float& ty, float& tz) {
+    float px = fmaf((float)(ix + (u > 0.0f ? 1 : 0)), g.hx, g.ox);
+    float py = fmaf((float)(iy + (v > 0.0f ? 1 : 0)), g.hy, g.oy);
+    float pz = fmaf((float)(iz + (w > 0.0f ? 1 : 0)), g.hz, g.oz);
+    float a = fmaxf((px - x) * f_rcp(u), 0.0f), b = fmaxf((py - y) * f_rcp(v), 0.0f), c = fmaxf((pz - z) * f_rcp(w), 0.0f);
+    tx = fabsf(u) > 1e-20f ? a : kInf;
+    ty = fabsf(v) > 1e-20f ? b : kInf;
+    tz = fabsf(w) > 1e-20f ? c : kInf;
+}
+
+struct ELane {
+    float x, y, z, u, v, w, T, ex, rho, tx, ty, tz, acc, smax;
+    int ix, iy, iz, vox, mat;
+    uint32_t tag;
+    Rng rng;
+};
+
+__global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_constant__ RunParams P) {
     extern __shared__ float2 s_tab[];
-    {
-        const int ntab = P.n_mat * TE_COUNT * P.N;
-        for (int i = threadIdx.x; i < ntab; i += blockDim.x) s_tab[i] = P.tabE[i];
-    }
+    const int ntab = P.n_mat * TE_COUNT * P.N;
+    uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_tab + ntab);           // [SE_COUNT][kThreadsE]
+    double* s_led = reinterpret_cast<double*>(s_cnt + SE_COUNT * kThreadsE);  // [2][kThreadsE]: e_src, e_esc
+    for (int i = threadIdx.x; i < ntab; i += kThreadsE) s_tab[i] = P.tabE[i];
+    const int tid = threadIdx.x;
+#pragma unroll
+    for (int k = 0; k < SE_COUNT; ++k) s_cnt[k * kThreadsE + tid] = 0u;
+    s_led[tid] = 0.0; s_led[kThreadsE + tid] = 0.0;
     __syncthreads();
-    const int lane = threadIdx.x & 31;
+    const int lane = tid & 31;
     const int N = P.N, k_cut = P.k_cut;
     const Geometry& g = P.g;
-    const bool no_hard = P.flags & 1u, no_ms = P.flags & 2u;
+    const bool no_hard = P.flags & 1u, no_ms = P.flags & 2u, local_sec = P.flags & 4u;
+    const float2* const tR = s_tab + TE_R * N;  // + mat * TE_COUNT * N
+    const int mstride = TE_COUNT * N;
+    const int KH = P.hard_lanes, KR = P.refill_lanes;
 
-    bool active = false, exhausted = false;
-    float x = 0, y = 0, z = 0, u = 0, v = 0, w = 1, T = 0, ex = 0, rho = 1;
-    int ix = 0, iy = 0, iz = 0, vox = 0;
-    const float2* tm = s_tab;  // tables of the current voxel's material
-    int mat = 0;
-    Rng rng = {0, 0, 0, 0};
-    uint32_t tag = 0, cell0 = 0;  // cell0 = batch * nvox
-    Score sc = {0.0f, 0u, 0u};
-    uint32_t n_step = 0, n_moller = 0, n_brems = 0, n_sec_e = 0, n_sec_g = 0, n_hist = 0;
-    double e_src = 0.0, e_esc = 0.0;
+    int state = L_IDLE;
+    ELane L;
+    L.x = L.y = L.z = 0.f; L.u = L.v = 0.f; L.w = 1.f; L.T = 0.f; L.ex = 0.f; L.rho = 1.f; L.tx = L.ty = L.tz = 0.f;
+    L.acc = 0.f; L.smax = 0.f; L.ix = L.iy = L.iz = L.vox = L.mat = 0; L.tag = 0u; L.rng = {0, 0, 0, 0};
+
+    auto bump = [&](int k) { s_cnt[k * kThreadsE + tid] += 1u; };
+    auto flush = [&]() {  // one red.global.add.f32 per (track, voxel) visit (S6)
+        if (L.acc > 0.0f) { atomicAdd(P.edep + (size_t)(L.tag >> 2) * (uint32_t)g.nvox + (uint32_t)L.vox, L.acc); bump(SE_RED); }
+        L.acc = 0.0f;
+    };
+    auto emit_rec = [&](const Queue& q, const QRec& r, int stat) {
+        if (local_sec) { L.acc += r.E + (((r.tag & 3u) == CODE_POSITRON) ? 2.0f * kMeF : 0.0f); return; }
+        bump(stat);
+        push_record(q, P.counters + C_OVERFLOW, r);
+    };
+    // end of track (S8): absorb the remaining kinetic energy; a positron annihilates at rest (R9)
+    auto terminate = [&]() {
+        L.acc += L.T;
+        if ((L.tag & 3u) == CODE_POSITRON) {
+            uint4 a4 = next_block(L.rng, P.seed_lo, P.seed_hi);
+            float mu = 2.0f * u01f(a4.z) - 1.0f, sn = f_sqrt(fmaxf(1.0f - mu * mu, 0.0f)), ph = kTwoPiF * u01f(a4.w);
+            QRec r; r.x = L.x; r.y = L.y; r.z = L.z; r.u = sn * f_cos(ph); r.v = sn * f_sin(ph); r.w = mu; r.E = kMeF;
+            r.hist = L.rng.hist; r.trk_lo = a4.x; r.trk_hi = a4.y; r.vox = L.vox; r.tag = (L.tag & ~3u) | CODE_PHOTON;
+            emit_rec(P.q_p_out, r, SE_SEC_G);
+            uint4 b4 = next_block(L.rng, P.seed_lo, P.seed_hi);
+            r.u = -r.u; r.v = -r.v; r.w = -r.w; r.trk_lo = b4.x; r.trk_hi = b4.y;
+            emit_rec(P.q_p_out, r, SE_SEC_G);
+        }
+        flush();
+        state = L_IDLE;
+    };
 
     for (;;) {
-        // ---- lane refill: queue first, then new primaries ----
-        unsigned want = __ballot_sync(kFull, !active && !exhausted);
-        unsigned act = __ballot_sync(kFull, active);
-        if (want == 0u && act == 0u) break;
-        if (want != 0u && (act == 0u || __popc(want) >= P.refill_lanes)) {
-            uint32_t item = claim(P.counters + C_HEAD, want, lane);
-            if (!active && !exhausted) {
+        const unsigned m_step = __ballot_sync(kFull, state == L_STEP), m_hard = __ballot_sync(kFull, state == L_HARD),
+                       m_idle = __ballot_sync(kFull, state == L_IDLE);
+        const int ns = __popc(m_step), nh = __popc(m_hard), ni = __popc(m_idle);
+        if ((ns | nh | ni) == 0) break;
+        const bool do_hard = nh > 0 && (nh >= KH || nh > ns || (ns == 0 && ni == 0));
+        const bool do_refill = !do_hard && ni > 0 && (ni >= KR || ns == 0);
+
+        if (do_refill) {
+            // ---- REFILL: queue first, then new primaries (S0, S1) --------------------------------
+            uint32_t item = claim(P.counters + C_HEAD, m_idle, lane);
+            if (state == L_IDLE) {
+                bool ok = false;
                 if (item < P.n_in) {
                     QRec r = load_record(P.q_in, item);
-                    x = r.x; y = r.y; z = r.z; u = r.u; v = r.v; w = r.w; T = r.E;
-                    rng.hist = r.hist; rng.trk_lo = r.trk_lo; rng.trk_hi = r.trk_hi; rng.block = 0;
-                    vox = r.vox; tag = r.tag;
-                    ix = vox % g.nx; int t2 = vox / g.nx; iy = t2 % g.ny; iz = t2 / g.ny;
-                    active = true;
+                    L.x = r.x; L.y = r.y; L.z = r.z; L.u = r.u; L.v = r.v; L.w = r.w; L.T = r.E;
+                    L.rng.hist = r.hist; L.rng.trk_lo = r.trk_lo; L.rng.trk_hi = r.trk_hi; L.rng.block = 0;
+                    L.vox = r.vox; L.tag = r.tag;
+                    L.ix = L.vox % g.nx; int t2 = L.vox / g.nx; L.iy = t2 % g.ny; L.iz = t2 / g.ny;
+                    ok = true;
                 } else if (item < P.n_in + P.n_new) {
                     unsigned long long h = P.h_first + (item - P.n_in);
-                    rng.hist = (uint32_t)h; rng.trk_lo = 0; rng.trk_hi = 0; rng.block = 0;
-                    uint4 w4 = next_block(rng, P.seed_lo, P.seed_hi);
+                    L.rng.hist = (uint32_t)h; L.rng.trk_lo = 0; L.rng.trk_hi = 0; L.rng.block = 0;
+                    uint4 w4 = next_block(L.rng, P.seed_lo, P.seed_hi);
                     Primary p = sample_primary(P, w4);
                     uint32_t code = P.beam.particle > 0 ? CODE_POSITRON : CODE_ELECTRON;
-                    tag = (batch_of(h, P.n_batches, P.n_total) << 2) | code;
+                    L.tag = (batch_of(h, P.n_batches, P.n_total) << 2) | code;
                     float e0 = p.E + (code == CODE_POSITRON ? 2.0f * kMeF : 0.0f);
-                    e_src += (double)e0; ++n_hist;
-                    x = p.x; y = p.y; z = p.z; u = p.u; v = p.v; w = p.w; T = p.E;
-                    ix = p.ix; iy = p.iy; iz = p.iz; vox = ix + g.nx * (iy + g.ny * iz);
-                    if (p.inside) active = true; else e_esc += (double)e0;
-                } else exhausted = true;
-                if (active) {
-                    uint2 vd = P.vox[vox];
-                    rho = __uint_as_float(vd.x); mat = (int)vd.y; tm = s_tab + mat * TE_COUNT * N;
-                    cell0 = (tag >> 2) * (uint32_t)g.nvox;
-                    ex = (__logf(T) - P.lnE0) * P.inv_dln;
+                    s_led[tid] += (double)e0; bump(SE_HIST);
+                    L.x = p.x; L.y = p.y; L.z = p.z; L.u = p.u; L.v = p.v; L.w = p.w; L.T = p.E;
+                    L.ix = p.ix; L.iy = p.iy; L.iz = p.iz; L.vox = L.ix + g.nx * (L.iy + g.ny * L.iz);
+                    if (p.inside) ok = true; else s_led[kThreadsE + tid] += (double)e0;
+                } else state = L_DONE;
+                if (ok) {
+                    uint2 vd = P.vox[L.vox];
+                    L.rho = __uint_as_float(vd.x); L.mat = (int)vd.y;
+                    state = L_STEP;
+                    if (L.T <= P.e_cut) terminate();  // born at or below the cut-off (pair electrons)
+                    else {
+                        L.ex = fmaf(f_lg2(L.T), P.ex_a, -P.ex_b);
+                        face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, L.ix, L.iy, L.iz, L.tx, L.ty, L.tz);
+                    }
                 }
             }
-            act = __ballot_sync(kFull, active);
-            if (act == 0u) continue;
-        }
-        if (!active) continue;
-
-        // ---- end of track: absorb below the cut-off; a positron annihilates at rest (R9) -----------
-        if (T <= P.e_cut) {
-            score_add(sc, P.edep, cell0 + vox, T);
-            if ((tag & 3u) == CODE_POSITRON) {
-                uint4 a4 = next_block(rng, P.seed_lo, P.seed_hi);
-                float mu = 2.0f * u01(a4.z) - 1.0f, sn = sqrtf(fmaxf(1.0f - mu * mu, 0.0f)), sp, cp;
-                __sincosf(kTwoPiF * u01(a4.w), &sp, &cp);
-                QRec r; r.x = x; r.y = y; r.z = z; r.u = sn * cp; r.v = sn * sp; r.w = mu; r.E = kMeF;
-                r.hist = rng.hist; r.trk_lo = a4.x; r.trk_hi = a4.y; r.vox = vox; r.tag = (tag & ~3u) | CODE_PHOTON;
-                emit(P, P.q_p_out, sc, cell0 + vox, r, n_sec_g);
-                uint4 b4 = next_block(rng, P.seed_lo, P.seed_hi);
-                r.u = -r.u; r.v = -r.v; r.w = -r.w; r.trk_lo = b4.x; r.trk_hi = b4.y;
-                emit(P, P.q_p_out, sc, cell0 + vox, r, n_sec_g);
-            }
-            active = false;
             continue;
         }
 
-        // ---- step set-up (S4): d = min[d_vox, d_maxs, d_maxe, d_range, d_event] -------------------------
-        ++n_step;
-        int i0 = min(max((int)ex, 0), N - 2);
-        float f0 = ex - (float)i0;
-        float R0 = lerp(tm + TE_R * N, i0, f0), L0 = lerp(tm + TE_L * N, i0, f0), Smax = lerp(tm + TE_SMAX * N, i0, f0);
-        uint4 w4 = next_block(rng, P.seed_lo, P.seed_hi);
-        int ax;
-        float d = face_dist(g, x, y, z, u, v, w, ix, iy, iz, ax);
+        if (do_hard) {
+            // ---- HARD: thinning against the running-max majorant (R6), then Moller (R10) / bremsstrahlung (R11) ---
+            if (state == L_HARD) {
+                state = L_STEP;
+                const float2* tm = tR + L.mat * mstride;
+                uint4 h4 = next_block(L.rng, P.seed_lo, P.seed_hi);
+                float r = u01f(h4.x) * L.smax;
+                int i1 = min(max((int)L.ex, 0), N - 2);
+                float f1 = L.ex - (float)i1;
+                float SH = lerp(tm + (TE_SHARD - TE_R) * N, i1, f1);
+                if (r < SH) {
+                    float SM = lerp(tm + (TE_SM - TE_R) * N, i1, f1);
+                    float phi = kTwoPiF * u01f(h4.w), sphi = f_sin(phi), cphi = f_cos(phi);
+                    float T0 = L.T;
+                    QRec q; q.x = L.x; q.y = L.y; q.z = L.z; q.u = L.u; q.v = L.v; q.w = L.w; q.hist = L.rng.hist;
+                    q.trk_lo = h4.y; q.trk_hi = h4.z; q.vox = L.vox;
+                    if (r < SM) {  // Moller
+                        bump(SE_MOLLER);
+                        float tau = T0 * (1.0f / kMeF), gm = tau + 1.0f, ig2 = f_rcp(gm * gm);
+                        float qq = (2.0f * gm - 1.0f) * ig2, q1 = tau * tau * ig2;
+                        float ec = P.e_cut * f_rcp(T0), iec = T0 * f_rcp(P.e_cut);
+                        auto gf = [&](float e) { float o = f_rcp(1.0f - e); return 1.0f - qq * e * o + e * e * (q1 + o * o); };
+                        float gmax = fmaxf(gf(ec), gf(0.5f)), eps;
+                        for (;;) {
+                            uint4 m4 = next_block(L.rng, P.seed_lo, P.seed_hi);
+                            eps = f_rcp(iec - u01f(m4.x) * (iec - 2.0f));
+                            if (u01f(m4.y) * gmax <= gf(eps)) break;
+                            eps = f_rcp(iec - u01f(m4.z) * (iec - 2.0f));
+                            if (u01f(m4.w) * gmax <= gf(eps)) break;
+                        }
+                        float W = eps * T0, Tp = T0 - W, t2m = T0 + 2.0f * kMeF;
+                        float c1 = f_sqrt(Tp * t2m * f_rcp(T0 * (Tp + 2.0f * kMeF)));
+                        float c2 = f_sqrt(W * t2m * f_rcp(T0 * (W + 2.0f * kMeF)));
+                        q.E = W; q.tag = (L.tag & ~3u) | CODE_ELECTRON;
+                        rotate_fast(q.u, q.v, q.w, 1.0f - c2, -sphi, -cphi);  // azimuth phi + pi
+                        rotate_fast(L.u, L.v, L.w, 1.0f - c1, sphi, cphi);
+                        L.T = Tp;
+                        emit_rec(P.q_e_out, q, SE_SEC_E);
+                        face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, L.ix, L.iy, L.iz, L.tx, L.ty, L.tz);
+                    } else {  // bremsstrahlung
+                        bump(SE_BREMS);
+                        float Et = T0 + kMeF, lscr = P.lscr[L.mat], iEt = f_rcp(Et);
+                        auto Ff = [&](float k) {
+                            float Ep = Et - k, rr = Ep * iEt;
+                            return (1.0f + rr * rr - (2.0f / 3.0f) * rr) * (fminf(f_ln(2.0f * Et * Ep * f_rcp(kMeF * k)), lscr) - 0.5f);
+                        };
+                        float Fmax = (4.0f / 3.0f) * (fminf(f_ln(2.0f * Et * (Et - P.g_cut) * f_rcp(kMeF * P.g_cut)), lscr) - 0.5f);
+                        float l2r = f_lg2(T0 * f_rcp(P.g_cut)), kk;
+                        for (;;) {
+                            uint4 m4 = next_block(L.rng, P.seed_lo, P.seed_hi);
+                            kk = fminf(P.g_cut * f_ex2(l2r * u01f(m4.x)), T0);
+                            if (u01f(m4.y) * Fmax <= Ff(kk)) break;
+                            kk = fminf(P.g_cut * f_ex2(l2r * u01f(m4.z)), T0);
+                            if (u01f(m4.w) * Fmax <= Ff(kk)) break;
+                        }
+                        q.E = kk; q.tag = (L.tag & ~3u) | CODE_PHOTON;
+                        float sh = f_sin(0.5f * kMeF * iEt);
+                        rotate_fast(q.u, q.v, q.w, 2.0f * sh * sh, sphi, cphi);
+                        L.T = T0 - kk;
+                        emit_rec(P.q_p_out, q, SE_SEC_G);
+                    }
+                    if (L.T <= P.e_cut) terminate();
+                    else L.ex = fmaf(f_lg2(L.T), P.ex_a, -P.ex_b);
+                }
+            }
+            continue;
+        }
+
+        if (state != L_STEP) continue;
+        // ---- STEP set-up (S4): d = min[d_vox, d_maxs, d_maxe, d_range, d_event] ------------------------------
+        bump(SE_STEP);
+        const float2* tm = tR + L.mat * mstride;
+        int i0 = min(max((int)L.ex, 0), N - 2);
+        float f0 = L.ex - (float)i0;
+        float R0 = lerp(tm, i0, f0), L0 = lerp(tm + (TE_L - TE_R) * N, i0, f0), Smax = lerp(tm + (TE_SMAX - TE_R) * N, i0, f0);
+        uint4 w4 = next_block(L.rng, P.seed_lo, P.seed_hi);
+        const float rho = L.rho, irho = f_rcp(rho);
+        float d = fminf(L.tx, fminf(L.ty, L.tz));
         int lim = 0;
-        float rl = rho * L0;
-        float d_maxe = __fdividef(P.f_maxe * T, rl);
-        float d_range = __fdividef(fmaxf(R0, 0.0f), rho);
+        float d_maxe = P.f_maxe * L.T * irho * f_rcp(L0);
+        float d_range = fmaxf(R0, 0.0f) * irho;
         if (P.d_maxs < d) { d = P.d_maxs; lim = 1; }
         if (d_maxe < d) { d = d_maxe; lim = 2; }
         if (d_range < d) { d = d_range; lim = 3; }
         if (!no_hard) {
-            float d_event = __fdividef(-__logf(u01(w4.x)), rho * Smax);
+            float d_event = -kLn2F * f_lg2(u01f(w4.x)) * irho * f_rcp(Smax);
             if (d_event < d) { d = d_event; lim = 4; }
         }
-        // ---- random hinge (S5; R7, R8) ----------------------------------------------------------------
-        float xi = u01(w4.y), legA = xi * d;
-        x = fmaf(legA, u, x); y = fmaf(legA, v, y); z = fmaf(legA, w, z);
-        // first-order guess of the table-coordinate shift per unit range: d ex / d R = 1 / (T/L * dln) per g/cm^2
-        float dex_dR = __fdividef(L0 * P.inv_dln, T);
-        float rd = rho * d;
+        // ---- random hinge (S5; R7, R8) ---------------------------------------------------------------------
+        const float legA = u01f(w4.y) * d;
+        L.x = fmaf(legA, L.u, L.x); L.y = fmaf(legA, L.v, L.y); L.z = fmaf(legA, L.w, L.z);
+        const float xl = rho * L0 * f_rcp(L.T);  // fractional energy loss per unit path at constant L (search guess only)
+        const float rd = rho * d;
+        bool turned = false;
         if (!no_ms) {
-            float Rm = fmaf(-0.5f, rd, R0);
-            float em = inv_range_coord(tm + TE_R * N, Rm, (int)(ex - 0.5f * rd * dex_dR), k_cut, N);
+            float em = inv_range_coord(tm, fmaf(-0.5f, rd, R0), fmaf(f_lg2(fmaf(-0.5f * d, xl, 1.0f)), P.ex_a, L.ex), k_cut, N);
             int im = min(max((int)em, 0), N - 2);
-            float k1 = lerp(tm + TE_K1 * N, im, em - (float)im);
-            float t = k1 * rd;
-            float am = t < 1e-3f ? t * (1.0f - 0.5f * t) : 1.0f - __expf(-t);
+            float t = lerp(tm + (TE_K1 - TE_R) * N, im, em - (float)im) * rd;
+            float am = t < 1e-3f ? t * (1.0f - 0.5f * t) : 1.0f - f_exp(-t);
             if (am > 0.0f) {
-                float omu = -am * __logf(1.0f - u01(w4.z) * (1.0f - __expf(__fdividef(-2.0f, am))));
-                rotate(u, v, w, fminf(omu, 2.0f), kTwoPiF * u01(w4.w));
+                float omu = -am * kLn2F * f_lg2(1.0f - u01f(w4.z) * (1.0f - f_exp(-2.0f * f_rcp(am))));
+                float phi = kTwoPiF * u01f(w4.w);
+                rotate_fast(L.u, L.v, L.w, fminf(omu, 2.0f), f_sin(phi), f_cos(phi));
+                turned = true;
             }
         }
-        float rest = d - legA;
-        float tf = face_dist(g, x, y, z, u, v, w, ix, iy, iz, ax);
-        bool cross = tf <= rest;
-        float legB = cross ? tf : rest;
-        x = fmaf(legB, u, x); y = fmaf(legB, v, y); z = fmaf(legB, w, z);
-        float d_act = legA + legB;
-        // ---- CSDA loss through the range table (S6; R5) + scoring ---------------------------------------
+        if (turned) face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, L.ix, L.iy, L.iz, L.tx, L.ty, L.tz);
+        else { L.tx -= legA; L.ty -= legA; L.tz -= legA; }
+        const float rest = d - legA;
+        int ax = 0;
+        float tf = L.tx;
+        if (L.ty < tf) { tf = L.ty; ax = 1; }
+        if (L.tz < tf) { tf = L.tz; ax = 2; }
+        const bool cross = tf <= rest;
+        const float legB = cross ? tf : rest;
+        L.x = fmaf(legB, L.u, L.x); L.y = fmaf(legB, L.v, L.y); L.z = fmaf(legB, L.w, L.z);
+        L.tx = fmaxf(L.tx - legB, 0.0f); L.ty = fmaxf(L.ty - legB, 0.0f); L.tz = fmaxf(L.tz - legB, 0.0f);
+        const float d_act = legA + legB;
+        // ---- CSDA loss through the range table (S6; R5) + scoring ------------------------------------------
         float T1, ex1;
         if (lim == 3 && !cross) { T1 = P.e_cut; ex1 = (float)k_cut; }
         else {
-            float ra = rho * d_act;
-            ex1 = inv_range_coord(tm + TE_R * N, fmaf(-rho, d_act, R0), (int)(ex - ra * dex_dR), k_cut, N);
-            T1 = fminf(__expf(fmaf(ex1, P.dln, P.lnE0)), T);
+            ex1 = inv_range_coord(tm, fmaf(-rho, d_act, R0), fmaf(f_lg2(fmaxf(fmaf(-d_act, xl, 1.0f), 1e-3f)), P.ex_a, L.ex), k_cut, N);
+            T1 = fminf(f_ex2(fmaf(ex1, P.t_a, P.t_b)), L.T);
         }
-        score_add(sc, P.edep, cell0 + vox, T - T1);
-        T = T1; ex = ex1;
+        L.acc += L.T - T1;
+        L.T = T1; L.ex = ex1;
         if (cross) {
-            // move to the neighbour voxel, coordinate snapped to the face (R8)
-            int dir;
-            if (ax == 0) { dir = u > 0.0f ? 1 : -1; ix += dir; x = fmaf((float)(ix + (dir > 0 ? 0 : 1)), g.hx, g.ox); vox += dir; }
-            else if (ax == 1) { dir = v > 0.0f ? 1 : -1; iy += dir; y = fmaf((float)(iy + (dir > 0 ? 0 : 1)), g.hy, g.oy); vox += dir * g.nx; }
-            else { dir = w > 0.0f ? 1 : -1; iz += dir; z = fmaf((float)(iz + (dir > 0 ? 0 : 1)), g.hz, g.oz); vox += dir * g.nx * g.ny; }
-            if ((unsigned)ix >= (unsigned)g.nx || (unsigned)iy >= (unsigned)g.ny || (unsigned)iz >= (unsigned)g.nz) {
-                e_esc += (double)(T + ((tag & 3u) == CODE_POSITRON ? 2.0f * kMeF : 0.0f));
-                active = false;
-                continue;
+            // leave the voxel: flush its deposit, move to the neighbour, coordinate snapped to the face (R8).
+            // Written with one predicate per axis so that it compiles to selects, not to a 3-way branch.
+            flush();
+            const bool a0 = ax == 0, a1 = ax == 1, a2 = ax == 2;
+            const float dc = a0 ? L.u : (a1 ? L.v : L.w);
+            const int dir = dc > 0.0f ? 1 : -1, up = dc > 0.0f ? 1 : 0;
+            const float tnew = (a0 ? g.hx : (a1 ? g.hy : g.hz)) * f_rcp(fabsf(dc));
+            // the face that was hit is the one the direction points at
+            const float fx = fmaf((float)(L.ix + up), g.hx, g.ox), fy = fmaf((float)(L.iy + up), g.hy, g.oy),
+                        fz = fmaf((float)(L.iz + up), g.hz, g.oz);
+            L.x = a0 ? fx : L.x; L.y = a1 ? fy : L.y; L.z = a2 ? fz : L.z;
+            L.tx = a0 ? tnew : L.tx; L.ty = a1 ? tnew : L.ty; L.tz = a2 ? tnew : L.tz;
+            L.ix += a0 ? dir : 0; L.iy += a1 ? dir : 0; L.iz += a2 ? dir : 0;
+            L.vox += dir * (a0 ? 1 : (a1 ? g.nx : g.nx * g.ny));
+            if ((unsigned)L.ix >= (unsigned)g.nx || (unsigned)L.iy >= (unsigned)g.ny || (unsigned)L.iz >= (unsigned)g.nz) {
+                s_led[kThreadsE + tid] += (double)(L.T + ((L.tag & 3u) == CODE_POSITRON ? 2.0f * kMeF : 0.0f));
+                state = L_IDLE;
+            } else {
+                uint2 vd = P.vox[L.vox];
+                L.rho = __uint_as_float(vd.x); L.mat = (int)vd.y;
+                if (L.T <= P.e_cut) terminate();
             }
-            uint2 vd = P.vox[vox];
-            rho = __uint_as_float(vd.x);
-            if ((int)vd.y != mat) { mat = (int)vd.y; tm = s_tab + mat * TE_COUNT * N; }
-            continue;
-        }
-        if (lim != 4 || T <= P.e_cut) continue;
-
-        // ---- hard-event candidate (S7): thinning against the running-max majorant (R6) -------------------
-        uint4 h4 = next_block(rng, P.seed_lo, P.seed_hi);
-        float r = u01(h4.x) * Smax;
-        int i1 = min(max((int)ex, 0), N - 2);
-        float f1 = ex - (float)i1;
-        float SH = lerp(tm + TE_SHARD * N, i1, f1);
-        if (r >= SH) continue;  // fictitious
-        float SM = lerp(tm + TE_SM * N, i1, f1);
-        float phi = kTwoPiF * u01(h4.w);
-        float T0 = T;
-        QRec q; q.x = x; q.y = y; q.z = z; q.u = u; q.v = v; q.w = w; q.hist = rng.hist; q.trk_lo = h4.y; q.trk_hi = h4.z; q.vox = vox;
-        if (r < SM) {  // Moller (R10)
-            ++n_moller;
-            float tau = T0 * (1.0f / kMeF), gm = tau + 1.0f, ig2 = __fdividef(1.0f, gm * gm);
-            float qq = (2.0f * gm - 1.0f) * ig2, q1 = tau * tau * ig2;
-            float ec = __fdividef(P.e_cut, T0), iec = __fdividef(T0, P.e_cut);
-            auto gf = [&](float e) { float o = __fdividef(1.0f, 1.0f - e); return 1.0f - qq * e * o + e * e * (q1 + o * o); };
-            float gmax = fmaxf(gf(ec), gf(0.5f)), eps;
-            for (;;) {
-                uint4 m4 = next_block(rng, P.seed_lo, P.seed_hi);
-                eps = __fdividef(1.0f, iec - u01(m4.x) * (iec - 2.0f));
-                if (u01(m4.y) * gmax <= gf(eps)) break;
-                eps = __fdividef(1.0f, iec - u01(m4.z) * (iec - 2.0f));
-                if (u01(m4.w) * gmax <= gf(eps)) break;
-            }
-            float W = eps * T0, Tp = T0 - W, t2m = T0 + 2.0f * kMeF;
-            float c1 = sqrtf(__fdividef(Tp * t2m, T0 * (Tp + 2.0f * kMeF)));
-            float c2 = sqrtf(__fdividef(W * t2m, T0 * (W + 2.0f * kMeF)));
-            q.E = W; q.tag = (tag & ~3u) | CODE_ELECTRON;
-            rotate(q.u, q.v, q.w, 1.0f - c2, phi + 3.14159265358979f);
-            rotate(u, v, w, 1.0f - c1, phi);
-            T = Tp;
-            emit(P, P.q_e_out, sc, cell0 + vox, q, n_sec_e);
-        } else {  // bremsstrahlung (R11)
-            ++n_brems;
-            float Et = T0 + kMeF, lscr = P.lscr[mat], iEt = __fdividef(1.0f, Et);
-            auto Ff = [&](float k) {
-                float Ep = Et - k, rr = Ep * iEt;
-                return (1.0f + rr * rr - (2.0f / 3.0f) * rr) * (fminf(__logf(__fdividef(2.0f * Et * Ep, kMeF * k)), lscr) - 0.5f);
-            };
-            float Fmax = (4.0f / 3.0f) * (fminf(__logf(__fdividef(2.0f * Et * (Et - P.g_cut), kMeF * P.g_cut)), lscr) - 0.5f);
-            float lr = __logf(__fdividef(T0, P.g_cut)), kk;
-            for (;;) {
-                uint4 m4 = next_block(rng, P.seed_lo, P.seed_hi);
-                kk = fminf(P.g_cut * __expf(lr * u01(m4.x)), T0);
-                if (u01(m4.y) * Fmax <= Ff(kk)) break;
-                kk = fminf(P.g_cut * __expf(lr * u01(m4.z)), T0);
-                if (u01(m4.w) * Fmax <= Ff(kk)) break;
-            }
-            q.E = kk; q.tag = (tag & ~3u) | CODE_PHOTON;
-            float sh = __sinf(0.5f * kMeF * iEt);
-            rotate(q.u, q.v, q.w, 2.0f * sh * sh, phi);
-            T = T0 - kk;
-            emit(P, P.q_p_out, sc, cell0 + vox, q, n_sec_g);
-        }
-        ex = (__logf(fmaxf(T, 1e-30f)) - P.lnE0) * P.inv_dln;
+        } else if (L.T <= P.e_cut) terminate();
+        else if (lim == 4) { state = L_HARD; L.smax = Smax; }
     }
-    // ---- warp exit: flush the pending deposit, reduce the counters ---------------------------------------
-    score_flush(sc, P.edep);
-    unsigned long long s_moller = warp_sum(n_moller), s_brems = warp_sum(n_brems), s_se = warp_sum(n_sec_e),
-                       s_sg = warp_sum(n_sec_g), s_red = warp_sum(sc.n_red), s_hist = warp_sum(n_hist),
-                       s_step = warp_sum(n_step);
-    double s_src = warp_sum(e_src), s_esc = warp_sum(e_esc);
+    // ---- exit: reduce the per-thread counters ------------------------------------------------------------------
+    const int sid[SE_COUNT] = {S_ESTEP, S_MOLLER, S_BREMS, S_SEC_E, S_SEC_G, S_HIST, S_ATOMICS};
+#pragma unroll
+    for (int k = 0; k < SE_COUNT; ++k) {
+        unsigned long long s = warp_sum(s_cnt[k * kThreadsE + tid]);
+        if (lane == 0) stat_add(P.stats, sid[k], s);
+    }
+    double s_src = warp_sum(s_led[tid]), s_esc = warp_sum(s_led[kThreadsE + tid]);
     if (lane == 0) {
-        stat_add(P.stats, S_ESTEP, s_step); stat_add(P.stats, S_MOLLER, s_moller); stat_add(P.stats, S_BREMS, s_brems);
-        stat_add(P.stats, S_SEC_E, s_se); stat_add(P.stats, S_SEC_G, s_sg); stat_add(P.stats, S_ATOMICS, s_red);
-        stat_add(P.stats, S_HIST, s_hist);
         if (s_src != 0.0) atomicAdd(P.ledger + LG_SRC, s_src);
         if (s_esc != 0.0) atomicAdd(P.ledger + LG_ESC, s_esc);
     }
