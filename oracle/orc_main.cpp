@@ -47,6 +47,7 @@ struct Stream {
 };
 
 // ------------------------------------------------------------------------------------------------
+constexpr double HINGE_OVERRUN = 0.25;  // DESIGN.md R8
 struct Params { double e_cut, g_cut, e_max; int n_grid; double d_maxs, f_maxe; uint32_t flags; };
 enum { F_NO_HARD = 1, F_NO_MS = 2, F_LOCAL_SEC = 4 };
 
@@ -387,7 +388,13 @@ struct Run {
             }
             double rest = (1.0 - xi) * d;
             double tf = face_dist(p.x, p.d, p.v, ax);
-            bool cross = tf <= rest;
+            // R8: a step cut short by the voxel (d = d_vox) is meant to end on the face; after the deflection the
+            // face may be a little further than planned, so the second leg may run on to it, by at most
+            // HINGE_OVERRUN of its planned length and never beyond the non-geometric limits.  Without this,
+            // about half of the voxel-limited steps stop a hair short of the face and need a tiny extra step.
+            double d_lim = std::min(std::min(P.d_maxs, d_maxe), std::min(d_range, d_event));
+            double reach = std::min((1.0 + HINGE_OVERRUN) * rest, d_lim - xi * d);
+            bool cross = tf <= std::max(reach, rest);
             double legB = cross ? tf : rest;
             for (int a = 0; a < 3; ++a) p.x[a] += legB * p.d[a];
             double d_act = xi * d + legB;

@@ -111,6 +111,7 @@ __device__ __forceinline__ void emit(const RunParams& P, const Queue& q, Score& 
 // else can run, so the rare blocks run with many lanes instead of one or two (profiles/README.md).
 // =================================================================================================
 constexpr int kThreadsE = 128;
+constexpr float kHingeOverrun = 0.25f;  // DESIGN.md R8
 enum LaneState { L_IDLE = 0, L_STEP = 1, L_HARD = 2, L_DONE = 3 };
 enum { SE_STEP = 0, SE_MOLLER, SE_BREMS, SE_SEC_E, SE_SEC_G, SE_HIST, SE_RED, SE_COUNT };
 
@@ -308,17 +309,19 @@ __global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_con
         float R0 = lerp(tm, i0, f0), L0 = lerp(tm + (TE_L - TE_R) * N, i0, f0), Smax = lerp(tm + (TE_SMAX - TE_R) * N, i0, f0);
         uint4 w4 = next_block(L.rng, P.seed_lo, P.seed_hi);
         const float rho = L.rho, irho = f_rcp(rho);
-        float d = fminf(L.tx, fminf(L.ty, L.tz));
-        int lim = 0;
-        float d_maxe = P.f_maxe * L.T * irho * f_rcp(L0);
-        float d_range = fmaxf(R0, 0.0f) * irho;
-        if (P.d_maxs < d) { d = P.d_maxs; lim = 1; }
-        if (d_maxe < d) { d = d_maxe; lim = 2; }
-        if (d_range < d) { d = d_range; lim = 3; }
+        const float d_vox = fminf(L.tx, fminf(L.ty, L.tz));
+        float d_lim = P.d_maxs;  // the non-geometric limits
+        int lim = 1;
+        const float d_maxe = P.f_maxe * L.T * irho * f_rcp(L0);
+        const float d_range = fmaxf(R0, 0.0f) * irho;
+        if (d_maxe < d_lim) { d_lim = d_maxe; lim = 2; }
+        if (d_range < d_lim) { d_lim = d_range; lim = 3; }
         if (!no_hard) {
             float d_event = -kLn2F * f_lg2(u01f(w4.x)) * irho * f_rcp(Smax);
-            if (d_event < d) { d = d_event; lim = 4; }
+            if (d_event < d_lim) { d_lim = d_event; lim = 4; }
         }
+        float d = d_vox;
+        if (d_lim < d) d = d_lim; else lim = 0;
         // ---- random hinge (S5; R7, R8) ---------------------------------------------------------------------
         const float legA = u01f(w4.y) * d;
         L.x = fmaf(legA, L.u, L.x); L.y = fmaf(legA, L.v, L.y); L.z = fmaf(legA, L.w, L.z);
@@ -344,7 +347,9 @@ __global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_con
         float tf = L.tx;
         if (L.ty < tf) { tf = L.ty; ax = 1; }
         if (L.tz < tf) { tf = L.tz; ax = 2; }
-        const bool cross = tf <= rest;
+        // R8: a voxel-limited step may run on to the face by up to kHingeOverrun of the planned second leg, never
+        // beyond the non-geometric limits (removes the tiny catch-up steps after half of the voxel-limited steps)
+        const bool cross = tf <= fmaxf(fminf((1.0f + kHingeOverrun) * rest, d_lim - legA), rest);
         const float legB = cross ? tf : rest;
         L.x = fmaf(legB, L.u, L.x); L.y = fmaf(legB, L.v, L.y); L.z = fmaf(legB, L.w, L.z);
         L.tx = fmaxf(L.tx - legB, 0.0f); L.ty = fmaxf(L.ty - legB, 0.0f); L.tz = fmaxf(L.tz - legB, 0.0f);
