@@ -71,6 +71,7 @@ struct RunParams {
     uint32_t flags;
     float* edep;  // [n_batches][nvox]
     unsigned long long n_total, h_first;  // job size; first primary history of this launch
+    unsigned long long inv_n_total;       // floor(2^64 / n_total), see batch_of
     int n_batches;
     uint32_t seed_lo, seed_hi;
     uint32_t n_in, n_new;     // queued particles to consume, new primaries to generate
@@ -152,6 +153,27 @@ __device__ __forceinline__ void push_record(const Queue& q, uint32_t* overflow, 
     d[1] = make_uint4(__float_as_uint(r.v), __float_as_uint(r.w), __float_as_uint(r.E), r.hist);
     d[2] = make_uint4(r.trk_lo, r.trk_hi, (uint32_t)r.vox, r.tag);
 }
+// Push to one of two queues chosen per lane (first ? qa : qb): one pass over the record stores, two aggregated
+// tail reservations (one per queue, each over the lanes that chose it).
+__device__ __forceinline__ void push_record2(const Queue& qa, const Queue& qb, bool first, uint32_t* overflow, const QRec& r) {
+    const unsigned m = __activemask();
+    const unsigned ma = __ballot_sync(m, first), mb = m & ~ma;
+    const int lane = threadIdx.x & 31;
+    uint32_t base_a = 0, base_b = 0;
+    if (ma && lane == __ffs(ma) - 1) base_a = atomicAdd(qa.count, (uint32_t)__popc(ma));
+    if (mb && lane == __ffs(mb) - 1) base_b = atomicAdd(qb.count, (uint32_t)__popc(mb));
+    if (ma) base_a = __shfl_sync(m, base_a, __ffs(ma) - 1);
+    if (mb) base_b = __shfl_sync(m, base_b, __ffs(mb) - 1);
+    const unsigned mine = first ? ma : mb;
+    const uint32_t idx = (first ? base_a : base_b) + __popc(mine & ((1u << lane) - 1u));
+    const Queue& q = first ? qa : qb;
+    if (idx >= (first ? qa.cap : qb.cap)) { atomicExch(overflow, 1u); return; }
+    uint4* d = (first ? qa.rec : qb.rec) + 3ull * idx;
+    d[0] = make_uint4(__float_as_uint(r.x), __float_as_uint(r.y), __float_as_uint(r.z), __float_as_uint(r.u));
+    d[1] = make_uint4(__float_as_uint(r.v), __float_as_uint(r.w), __float_as_uint(r.E), r.hist);
+    d[2] = make_uint4(r.trk_lo, r.trk_hi, (uint32_t)r.vox, r.tag);
+    (void)q;
+}
 __device__ __forceinline__ QRec load_record(const Queue& q, uint32_t idx) {
     const uint4* s = q.rec + 3ull * idx;
     uint4 a = s[0], b = s[1], c = s[2];
@@ -209,8 +231,13 @@ __device__ __forceinline__ Primary sample_primary(const RunParams& P, uint4 w4) 
     if (b.n_nodes == 1) p.E = b.E_nodes[0];
     else {
         float u0 = u01(w4.x), u1 = u01(w4.y);
-        int j = 0;
-        while (j + 2 < b.n_nodes && u0 >= b.cdf[j + 1]) ++j;
+        // j = number of interior nodes cdf[1 .. n-2] that are <= u0 (the cdf is non-decreasing): the bin the linear
+        // scan "while (j + 2 < n && u0 >= cdf[j + 1]) ++j" stops in, found by bisection
+        int j = 0, hi = b.n_nodes - 2;
+        while (j < hi) {
+            int mid = (j + hi + 1) >> 1;
+            if (u0 >= b.cdf[mid]) j = mid; else hi = mid - 1;
+        }
         float p0 = b.pdf_nodes[j], p1 = b.pdf_nodes[j + 1];
         float q = __fmaf_rn(u1, __fsub_rn(__fmul_rn(p1, p1), __fmul_rn(p0, p0)), __fmul_rn(p0, p0));
         float t = __fdiv_rn(__fmul_rn(u1, __fadd_rn(p0, p1)), __fadd_rn(p0, __fsqrt_rn(q)));
@@ -232,8 +259,14 @@ __device__ __forceinline__ Primary sample_primary(const RunParams& P, uint4 w4) 
     return p;
 }
 
-__device__ __forceinline__ uint32_t batch_of(unsigned long long h, int n_batches, unsigned long long n_total) {
-    return (uint32_t)((h * (unsigned long long)n_batches) / n_total);
+// batch of history h = floor(h * B / N) (R18) without a 64-bit division: inv_n = floor(2^64 / N) gives a quotient that
+// is exact or one too small (h * B < 2^63), corrected by one multiply-compare.
+__device__ __forceinline__ uint32_t batch_of(unsigned long long h, int n_batches, unsigned long long n_total,
+                                             unsigned long long inv_n) {
+    const unsigned long long x = h * (unsigned long long)n_batches;
+    unsigned long long q = __umul64hi(x, inv_n);
+    if (x - q * n_total >= n_total) ++q;
+    return (uint32_t)q;
 }
 
 }  // namespace mcb

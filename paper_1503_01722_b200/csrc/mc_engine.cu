@@ -128,7 +128,9 @@ mc_status upload_tables(mc_ctx* ctx) {
 size_t smem_e(const mc_ctx* c) {  // tables + per-thread counters + per-thread energy ledger
     return (size_t)c->tabs.n_mat * TE_COUNT * c->tabs.N * sizeof(float2) + (size_t)SE_COUNT * kThreadsE * sizeof(uint32_t) + 2 * (size_t)kThreadsE * sizeof(double);
 }
-size_t smem_p(const mc_ctx* c) { return (size_t)(1 + c->tabs.n_mat * TP_COUNT) * c->tabs.N * sizeof(float2); }
+size_t smem_p(const mc_ctx* c) {
+    return (size_t)(1 + c->tabs.n_mat * TP_COUNT) * c->tabs.N * sizeof(float2) + (size_t)SP_COUNT * kThreadsP * sizeof(uint32_t) + 2 * (size_t)kThreadsP * sizeof(double);
+}
 
 mc_status check_beam(mc_ctx* ctx, const mc_beam* b) {
     if (!b) return fail(ctx, MC_ERR_INVALID_ARG, "beam is null");
@@ -213,7 +215,7 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, uint64_t n_total, uint64_t
     CU(cudaFuncSetAttribute(photon_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp));
     int occ_e = 0, occ_p = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_e, electron_kernel, kThreadsE, se));
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, photon_kernel, kThreads, sp));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, photon_kernel, kThreadsP, sp));
     if (occ_e < 1 || occ_p < 1) return fail(ctx, MC_ERR_CUDA, "kernel does not fit on an SM");
     if (ctx->blocks_per_sm > 0) { occ_e = std::min<int>(occ_e, (int)ctx->blocks_per_sm); occ_p = std::min<int>(occ_p, (int)ctx->blocks_per_sm); }
 
@@ -238,6 +240,7 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, uint64_t n_total, uint64_t
     fill_params(ctx, P);
     if ((st = upload_beam(ctx, beam, P.beam)) != MC_OK) return st;
     P.edep = d_edep; P.n_total = n_total; P.n_batches = n_batches;
+    P.inv_n_total = n_total > 1 ? (unsigned long long)((((unsigned __int128)1) << 64) / n_total) : ~0ull;
     P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32);
 
     const bool photon_beam = beam->particle == MC_PHOTON;
@@ -263,13 +266,13 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, uint64_t n_total, uint64_t
         Queue qe_oth{ctx->d_q[1 - cur], ctx->d_counters + C_E_A + (1 - cur), ctx->q_cap};
         Queue qp{ctx->d_q[2], ctx->d_counters + C_P, ctx->q_cap};
         const uint64_t items = (uint64_t)n_in + n_new;
-        const int occ = run_p ? occ_p : occ_e, thr = run_p ? kThreads : kThreadsE;
+        const int occ = run_p ? occ_p : occ_e, thr = run_p ? kThreadsP : kThreadsE;
         int grid = (int)std::min<uint64_t>((uint64_t)ctx->sm_count * occ, (items + thr - 1) / thr);
         grid = std::max(grid, 1);
         CU(cudaEventRecord(ctx->ev[2], s));
         if (run_p) {
             P.q_in = qp; P.q_e_out = qe_cur; P.q_p_out = qp;
-            photon_kernel<<<grid, kThreads, sp, s>>>(P);
+            photon_kernel<<<grid, kThreadsP, sp, s>>>(P);
         } else {
             P.q_in = qe_cur; P.q_e_out = qe_oth; P.q_p_out = qp;
             electron_kernel<<<grid, kThreadsE, se, s>>>(P);

@@ -154,6 +154,7 @@ __global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_con
     const int KH = P.hard_lanes, KR = P.refill_lanes;
 
     int state = L_IDLE;
+    uint32_t n_step_w = 0u;
     ELane L;
     L.x = L.y = L.z = 0.f; L.u = L.v = 0.f; L.w = 1.f; L.T = 0.f; L.ex = 0.f; L.rho = 1.f; L.tx = L.ty = L.tz = 0.f;
     L.acc = 0.f; L.smax = 0.f; L.ix = L.iy = L.iz = L.vox = L.mat = 0; L.tag = 0u; L.rng = {0, 0, 0, 0};
@@ -211,7 +212,7 @@ __global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_con
                     uint4 w4 = next_block(L.rng, P.seed_lo, P.seed_hi);
                     Primary p = sample_primary(P, w4);
                     uint32_t code = P.beam.particle > 0 ? CODE_POSITRON : CODE_ELECTRON;
-                    L.tag = (batch_of(h, P.n_batches, P.n_total) << 2) | code;
+                    L.tag = (batch_of(h, P.n_batches, P.n_total, P.inv_n_total) << 2) | code;
                     float e0 = p.E + (code == CODE_POSITRON ? 2.0f * kMeF : 0.0f);
                     s_led[tid] += (double)e0; bump(SE_HIST);
                     L.x = p.x; L.y = p.y; L.z = p.z; L.u = p.u; L.v = p.v; L.w = p.w; L.T = p.E;
@@ -233,65 +234,80 @@ __global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_con
         }
 
         if (do_hard) {
-            // ---- HARD: thinning against the running-max majorant (R6), then Moller (R10) / bremsstrahlung (R11) ---
+            // ---- HARD: thinning against the running-max majorant (R6), then Moller (R10) / bremsstrahlung (R11).
+            // The two event types share one code path (Philox blocks, rejection loop, rotation of the secondary,
+            // queue push) so that the expensive parts run with all pending lanes, not once per type. -----------
             if (state == L_HARD) {
                 state = L_STEP;
                 const float2* tm = tR + L.mat * mstride;
                 uint4 h4 = next_block(L.rng, P.seed_lo, P.seed_hi);
-                float r = u01f(h4.x) * L.smax;
+                const float r = u01f(h4.x) * L.smax;
                 int i1 = min(max((int)L.ex, 0), N - 2);
                 float f1 = L.ex - (float)i1;
-                float SH = lerp(tm + (TE_SHARD - TE_R) * N, i1, f1);
+                const float SH = lerp(tm + (TE_SHARD - TE_R) * N, i1, f1), SM = lerp(tm + (TE_SM - TE_R) * N, i1, f1);
                 if (r < SH) {
-                    float SM = lerp(tm + (TE_SM - TE_R) * N, i1, f1);
-                    float phi = kTwoPiF * u01f(h4.w), sphi = f_sin(phi), cphi = f_cos(phi);
-                    float T0 = L.T;
+                    const bool mol = r < SM;
+                    const float T0 = L.T;
+                    // per-type constants of the rejection sampling:  Moller: a = T0/e_cut, b = (2g-1)/g^2, c = ((g-1)/g)^2, m = g_max
+                    //                                              brems : a = lg2(T0/g_cut), b = 1/(T0+mc^2), c = L_scr, m = F_max
+                    float ca, cb, cc, cm;
+                    const float Et = T0 + kMeF;
+                    if (mol) {
+                        float tau = T0 * (1.0f / kMeF), gm = tau + 1.0f, ig2 = f_rcp(gm * gm);
+                        cb = (2.0f * gm - 1.0f) * ig2; cc = tau * tau * ig2;
+                        ca = T0 * f_rcp(P.e_cut);
+                        float ec = f_rcp(ca), o = f_rcp(1.0f - ec);
+                        cm = fmaxf(1.0f - cb * ec * o + ec * ec * (cc + o * o), 1.0f - cb + 0.25f * (cc + 4.0f));  // max(g(e_c), g(1/2))
+                    } else {
+                        cb = f_rcp(Et); cc = P.lscr[L.mat];
+                        ca = f_lg2(T0 * f_rcp(P.g_cut));
+                        cm = (4.0f / 3.0f) * (fminf(f_ln(2.0f * Et * (Et - P.g_cut) * f_rcp(kMeF * P.g_cut)), cc) - 0.5f);
+                    }
+                    // one trial: the sampled variable (Moller: eps = W/T0; brems: k) and its acceptance
+                    auto trial = [&](uint32_t w0, uint32_t w1, float& val) {
+                        const float u0 = u01f(w0), u1 = u01f(w1) * cm;
+                        if (mol) {
+                            float e = f_rcp(ca - u0 * (ca - 2.0f)), o = f_rcp(1.0f - e);
+                            val = e;
+                            return u1 <= 1.0f - cb * e * o + e * e * (cc + o * o);
+                        }
+                        float k = fminf(P.g_cut * f_ex2(ca * u0), T0), Ep = Et - k, rr = Ep * cb;
+                        val = k;
+                        return u1 <= (1.0f + rr * rr - (2.0f / 3.0f) * rr) * (fminf(f_ln(2.0f * Et * Ep * f_rcp(kMeF * k)), cc) - 0.5f);
+                    };
+                    float val;
+                    for (;;) {
+                        uint4 m4 = next_block(L.rng, P.seed_lo, P.seed_hi);
+                        if (trial(m4.x, m4.y, val)) break;
+                        if (trial(m4.z, m4.w, val)) break;
+                    }
+                    const float phi = kTwoPiF * u01f(h4.w);
+                    float sphi = f_sin(phi), cphi = f_cos(phi);
                     QRec q; q.x = L.x; q.y = L.y; q.z = L.z; q.u = L.u; q.v = L.v; q.w = L.w; q.hist = L.rng.hist;
                     q.trk_lo = h4.y; q.trk_hi = h4.z; q.vox = L.vox;
-                    if (r < SM) {  // Moller
+                    float omu_q;  // 1 - cos(polar angle) of the secondary
+                    if (mol) {
                         bump(SE_MOLLER);
-                        float tau = T0 * (1.0f / kMeF), gm = tau + 1.0f, ig2 = f_rcp(gm * gm);
-                        float qq = (2.0f * gm - 1.0f) * ig2, q1 = tau * tau * ig2;
-                        float ec = P.e_cut * f_rcp(T0), iec = T0 * f_rcp(P.e_cut);
-                        auto gf = [&](float e) { float o = f_rcp(1.0f - e); return 1.0f - qq * e * o + e * e * (q1 + o * o); };
-                        float gmax = fmaxf(gf(ec), gf(0.5f)), eps;
-                        for (;;) {
-                            uint4 m4 = next_block(L.rng, P.seed_lo, P.seed_hi);
-                            eps = f_rcp(iec - u01f(m4.x) * (iec - 2.0f));
-                            if (u01f(m4.y) * gmax <= gf(eps)) break;
-                            eps = f_rcp(iec - u01f(m4.z) * (iec - 2.0f));
-                            if (u01f(m4.w) * gmax <= gf(eps)) break;
-                        }
-                        float W = eps * T0, Tp = T0 - W, t2m = T0 + 2.0f * kMeF;
-                        float c1 = f_sqrt(Tp * t2m * f_rcp(T0 * (Tp + 2.0f * kMeF)));
-                        float c2 = f_sqrt(W * t2m * f_rcp(T0 * (W + 2.0f * kMeF)));
+                        const float W = val * T0, Tp = T0 - W, t2m = T0 + 2.0f * kMeF;
+                        const float c1 = f_sqrt(Tp * t2m * f_rcp(T0 * (Tp + 2.0f * kMeF)));
+                        omu_q = 1.0f - f_sqrt(W * t2m * f_rcp(T0 * (W + 2.0f * kMeF)));
                         q.E = W; q.tag = (L.tag & ~3u) | CODE_ELECTRON;
-                        rotate_fast(q.u, q.v, q.w, 1.0f - c2, -sphi, -cphi);  // azimuth phi + pi
                         rotate_fast(L.u, L.v, L.w, 1.0f - c1, sphi, cphi);
-                        L.T = Tp;
-                        emit_rec(P.q_e_out, q, SE_SEC_E);
                         face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, L.ix, L.iy, L.iz, L.tx, L.ty, L.tz);
-                    } else {  // bremsstrahlung
+                        sphi = -sphi; cphi = -cphi;  // the delta ray leaves at azimuth phi + pi
+                        L.T = Tp;
+                    } else {
                         bump(SE_BREMS);
-                        float Et = T0 + kMeF, lscr = P.lscr[L.mat], iEt = f_rcp(Et);
-                        auto Ff = [&](float k) {
-                            float Ep = Et - k, rr = Ep * iEt;
-                            return (1.0f + rr * rr - (2.0f / 3.0f) * rr) * (fminf(f_ln(2.0f * Et * Ep * f_rcp(kMeF * k)), lscr) - 0.5f);
-                        };
-                        float Fmax = (4.0f / 3.0f) * (fminf(f_ln(2.0f * Et * (Et - P.g_cut) * f_rcp(kMeF * P.g_cut)), lscr) - 0.5f);
-                        float l2r = f_lg2(T0 * f_rcp(P.g_cut)), kk;
-                        for (;;) {
-                            uint4 m4 = next_block(L.rng, P.seed_lo, P.seed_hi);
-                            kk = fminf(P.g_cut * f_ex2(l2r * u01f(m4.x)), T0);
-                            if (u01f(m4.y) * Fmax <= Ff(kk)) break;
-                            kk = fminf(P.g_cut * f_ex2(l2r * u01f(m4.z)), T0);
-                            if (u01f(m4.w) * Fmax <= Ff(kk)) break;
-                        }
-                        q.E = kk; q.tag = (L.tag & ~3u) | CODE_PHOTON;
-                        float sh = f_sin(0.5f * kMeF * iEt);
-                        rotate_fast(q.u, q.v, q.w, 2.0f * sh * sh, sphi, cphi);
-                        L.T = T0 - kk;
-                        emit_rec(P.q_p_out, q, SE_SEC_G);
+                        const float sh = f_sin(0.5f * kMeF * cb);
+                        omu_q = 2.0f * sh * sh;  // polar angle mc^2 / (T0 + mc^2)
+                        q.E = val; q.tag = (L.tag & ~3u) | CODE_PHOTON;
+                        L.T = T0 - val;
+                    }
+                    rotate_fast(q.u, q.v, q.w, omu_q, sphi, cphi);
+                    if (local_sec) L.acc += q.E;
+                    else {
+                        bump(mol ? SE_SEC_E : SE_SEC_G);
+                        push_record2(P.q_e_out, P.q_p_out, mol, P.counters + C_OVERFLOW, q);
                     }
                     if (L.T <= P.e_cut) terminate();
                     else L.ex = fmaf(f_lg2(L.T), P.ex_a, -P.ex_b);
@@ -300,9 +316,9 @@ __global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_con
             continue;
         }
 
+        n_step_w += (uint32_t)ns;  // warp-uniform: every lane in state L_STEP takes a step now
         if (state != L_STEP) continue;
         // ---- STEP set-up (S4): d = min[d_vox, d_maxs, d_maxe, d_range, d_event] ------------------------------
-        bump(SE_STEP);
         const float2* tm = tR + L.mat * mstride;
         int i0 = min(max((int)L.ex, 0), N - 2);
         float f0 = L.ex - (float)i0;
@@ -393,7 +409,7 @@ __global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_con
     const int sid[SE_COUNT] = {S_ESTEP, S_MOLLER, S_BREMS, S_SEC_E, S_SEC_G, S_HIST, S_ATOMICS};
 #pragma unroll
     for (int k = 0; k < SE_COUNT; ++k) {
-        unsigned long long s = warp_sum(s_cnt[k * kThreadsE + tid]);
+        unsigned long long s = k == SE_STEP ? (unsigned long long)n_step_w : warp_sum(s_cnt[k * kThreadsE + tid]);
         if (lane == 0) stat_add(P.stats, sid[k], s);
     }
     double s_src = warp_sum(s_led[tid]), s_esc = warp_sum(s_led[kThreadsE + tid]);
@@ -405,158 +421,185 @@ __global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_con
 
 // =================================================================================================
 // photon kernel: Woodcock tracking (R3), Compton (R4), pair (R12),
-// photoelectric absorption (R16).  One Philox block serves two flights.
+// photoelectric absorption (R16).  One Philox block serves two flights.  Same warp scheduling as the electron
+// kernel: per iteration a warp runs ONE of  FLY (lanes in L_STEP) / COMPTON (lanes in L_HARD, pending) /
+// REFILL (lanes in L_IDLE), the rare blocks only when enough lanes want them.
 // =================================================================================================
-__global__ void __launch_bounds__(kThreads) photon_kernel(const __grid_constant__ RunParams P) {
+constexpr int kThreadsP = 128;
+enum { SP_FLIGHT = 0, SP_FICT, SP_COMPTON, SP_PAIR, SP_PE, SP_SEC_E, SP_HIST, SP_RED, SP_COUNT };
+
+__global__ void __launch_bounds__(kThreadsP, 6) photon_kernel(const __grid_constant__ RunParams P) {
     extern __shared__ float2 s_tab[];
-    {
-        const int ntab = (1 + P.n_mat * TP_COUNT) * P.N;
-        for (int i = threadIdx.x; i < ntab; i += blockDim.x) s_tab[i] = P.tabP[i];
-    }
+    const int ntab = (1 + P.n_mat * TP_COUNT) * P.N;
+    uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_tab + ntab);              // [SP_COUNT][kThreadsP]
+    double* s_led = reinterpret_cast<double*>(s_cnt + SP_COUNT * kThreadsP);  // [2][kThreadsP]: e_src, e_esc
+    for (int i = threadIdx.x; i < ntab; i += kThreadsP) s_tab[i] = P.tabP[i];
+    const int tid = threadIdx.x;
+#pragma unroll
+    for (int k = 0; k < SP_COUNT; ++k) s_cnt[k * kThreadsP + tid] = 0u;
+    s_led[tid] = 0.0; s_led[kThreadsP + tid] = 0.0;
     __syncthreads();
-    const int lane = threadIdx.x & 31;
+    const int lane = tid & 31;
     const int N = P.N;
     const Geometry& g = P.g;
+    const bool local_sec = P.flags & 4u;
+    const int KC = P.hard_lanes, KR = P.refill_lanes;
+    const float lg_a = kLn2F * P.inv_dlnP, lg_b = P.lnE0P * P.inv_dlnP;  // table coordinate = lg2(E) * lg_a - lg_b
 
-    bool active = false, exhausted = false;
+    int state = L_IDLE;
     float x = 0, y = 0, z = 0, u = 0, v = 0, w = 1, E = 0, lf = 0, maj = 1;
-    int li = 0;
+    int li = 0, vox = 0;
     Rng rng = {0, 0, 0, 0};
-    uint32_t tag = 0, cell0 = 0;
-    Score sc = {0.0f, 0u, 0u};
-    uint32_t n_flight = 0, n_fict = 0, n_compton = 0, n_pair = 0, n_pe = 0, n_sec_e = 0, n_hist = 0;
-    double e_src = 0.0, e_esc = 0.0;
+    uint32_t tag = 0;
+
+    auto bump = [&](int k, uint32_t n) { s_cnt[k * kThreadsP + tid] += n; };
+    auto deposit = [&](int vx, float e) {
+        atomicAdd(P.edep + ((tag >> 2) * (uint32_t)g.nvox + (uint32_t)vx), e);
+        bump(SP_RED, 1u);
+    };
+    auto set_energy = [&]() {  // table coordinate and majorant of the current energy
+        float t = fmaf(f_lg2(E), lg_a, -lg_b);
+        li = min(max((int)t, 0), N - 2); lf = t - (float)li;
+        maj = lerp(s_tab, li, lf);
+    };
+    auto emit_e = [&](const QRec& r) {
+        if (local_sec) { deposit(r.vox, r.E + (((r.tag & 3u) == CODE_POSITRON) ? 2.0f * kMeF : 0.0f)); return; }
+        bump(SP_SEC_E, 1u);
+        push_record(P.q_e_out, P.counters + C_OVERFLOW, r);
+    };
 
     for (;;) {
-        unsigned want = __ballot_sync(kFull, !active && !exhausted);
-        unsigned act = __ballot_sync(kFull, active);
-        if (want == 0u && act == 0u) break;
-        if (want != 0u && (act == 0u || __popc(want) >= P.refill_lanes)) {
-            uint32_t item = claim(P.counters + C_HEAD, want, lane);
-            if (!active && !exhausted) {
-                int vox = 0;
+        const unsigned m_fly = __ballot_sync(kFull, state == L_STEP), m_comp = __ballot_sync(kFull, state == L_HARD),
+                       m_idle = __ballot_sync(kFull, state == L_IDLE);
+        const int nf = __popc(m_fly), nc = __popc(m_comp), ni = __popc(m_idle);
+        if ((nf | nc | ni) == 0) break;
+        const bool do_comp = nc > 0 && (nc >= KC || nc > nf || (nf == 0 && ni == 0));
+        const bool do_refill = !do_comp && ni > 0 && (ni >= KR || nf == 0);
+
+        if (do_refill) {
+            // ---- REFILL (S0, S1) --------------------------------------------------------------------------------
+            uint32_t item = claim(P.counters + C_HEAD, m_idle, lane);
+            if (state == L_IDLE) {
+                bool ok = false;
                 if (item < P.n_in) {
                     QRec r = load_record(P.q_in, item);
                     x = r.x; y = r.y; z = r.z; u = r.u; v = r.v; w = r.w; E = r.E;
                     rng.hist = r.hist; rng.trk_lo = r.trk_lo; rng.trk_hi = r.trk_hi; rng.block = 0;
                     vox = r.vox; tag = r.tag;
-                    active = true;
+                    ok = true;
                 } else if (item < P.n_in + P.n_new) {
                     unsigned long long h = P.h_first + (item - P.n_in);
                     rng.hist = (uint32_t)h; rng.trk_lo = 0; rng.trk_hi = 0; rng.block = 0;
                     uint4 w4 = next_block(rng, P.seed_lo, P.seed_hi);
                     Primary p = sample_primary(P, w4);
-                    tag = (batch_of(h, P.n_batches, P.n_total) << 2) | CODE_PHOTON;
-                    e_src += (double)p.E; ++n_hist;
+                    tag = (batch_of(h, P.n_batches, P.n_total, P.inv_n_total) << 2) | CODE_PHOTON;
+                    s_led[tid] += (double)p.E; bump(SP_HIST, 1u);
                     x = p.x; y = p.y; z = p.z; u = p.u; v = p.v; w = p.w; E = p.E;
                     vox = p.ix + g.nx * (p.iy + g.ny * p.iz);
-                    if (p.inside) active = true; else e_esc += (double)p.E;
-                } else exhausted = true;
-                if (active) {
-                    cell0 = (tag >> 2) * (uint32_t)g.nvox;
-                    if (E < P.g_cut) {  // absorbed where it was born
-                        score_add(sc, P.edep, cell0 + vox, E);
-                        active = false;
-                    } else {
-                        float t = (__logf(E) - P.lnE0P) * P.inv_dlnP;
-                        li = min(max((int)t, 0), N - 2); lf = t - (float)li;
-                        maj = lerp(s_tab, li, lf);
-                    }
+                    if (p.inside) ok = true; else s_led[kThreadsP + tid] += (double)p.E;
+                } else state = L_DONE;
+                if (ok) {
+                    if (E < P.g_cut) deposit(vox, E);  // absorbed where it was born
+                    else { set_energy(); state = L_STEP; }
                 }
             }
-            act = __ballot_sync(kFull, active);
-            if (act == 0u) continue;
+            continue;
         }
-        if (!active) continue;
 
+        if (do_comp) {
+            // ---- COMPTON: Klein-Nishina by the epsilon decomposition (R4) ----------------------------------------
+            if (state == L_HARD) {
+                bump(SP_COMPTON, 1u);
+                const float k0 = E * (1.0f / kMeF), e0 = f_rcp(1.0f + 2.0f * k0), e02 = e0 * e0;
+                const float a1l2 = -f_lg2(e0), a1 = a1l2 * kLn2F, a2 = 0.5f * (1.0f - e02), ik0 = f_rcp(k0);
+                float eps, tt;
+                for (;;) {
+                    uint4 c4 = next_block(rng, P.seed_lo, P.seed_hi);
+                    float u1 = u01f(c4.y);
+                    if (u01f(c4.x) * (a1 + a2) < a1) eps = f_ex2(-a1l2 * u1);
+                    else eps = f_sqrt(fmaf(1.0f - e02, u1, e02));
+                    tt = (1.0f - eps) * f_rcp(eps) * ik0;
+                    float sin2 = tt * (2.0f - tt);
+                    if (u01f(c4.z) <= 1.0f - eps * sin2 * f_rcp(1.0f + eps * eps)) break;
+                }
+                uint4 d4 = next_block(rng, P.seed_lo, P.seed_hi);
+                const float E1 = eps * E, Te = E - E1;
+                const float u0 = u, v0 = v, w0 = w;
+                const float phi = kTwoPiF * u01f(d4.z);
+                rotate_fast(u, v, w, tt, f_sin(phi), f_cos(phi));
+                float dep = 0.0f;
+                if (Te >= P.e_cut || local_sec) {
+                    QRec q; q.x = x; q.y = y; q.z = z; q.hist = rng.hist; q.vox = vox;
+                    float qx = E * u0 - E1 * u, qy = E * v0 - E1 * v, qz = E * w0 - E1 * w;
+                    float inr = f_rsqrt(fmaf(qx, qx, fmaf(qy, qy, qz * qz)));
+                    q.u = qx * inr; q.v = qy * inr; q.w = qz * inr;
+                    q.E = Te; q.trk_lo = d4.x; q.trk_hi = d4.y; q.tag = (tag & ~3u) | CODE_ELECTRON;
+                    emit_e(q);
+                } else dep = Te;  // born below the cut-off: absorbed where it is born (R26)
+                E = E1;
+                if (E < P.g_cut) { dep += E; state = L_IDLE; }
+                else { set_energy(); state = L_STEP; }
+                if (dep > 0.0f) deposit(vox, dep);
+            }
+            continue;
+        }
+
+        if (state != L_STEP) continue;
+        // ---- FLY: up to two Woodcock flights from one Philox block (S2) --------------------------------------------
         uint4 w4 = next_block(rng, P.seed_lo, P.seed_hi);
-        int chan = -1, vox = 0;
-        float rho = 0.0f;
+        int chan = -1;
+        uint32_t n_fl = 0, n_fi = 0;
         const float2* tm = s_tab;
-        float imaj = __fdividef(1.0f, maj);
+        const float imaj = f_rcp(maj);
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
-            float sl = -__logf(u01(k ? w4.z : w4.x)) * imaj;
+            float sl = -kLn2F * f_lg2(u01f(k ? w4.z : w4.x)) * imaj;
             x = fmaf(sl, u, x); y = fmaf(sl, v, y); z = fmaf(sl, w, z);
-            ++n_flight;
+            ++n_fl;
             float gx = (x - g.ox) * g.ihx, gy = (y - g.oy) * g.ihy, gz = (z - g.oz) * g.ihz;
             if (!(gx >= 0.0f && gx < (float)g.nx && gy >= 0.0f && gy < (float)g.ny && gz >= 0.0f && gz < (float)g.nz)) {
-                e_esc += (double)E; active = false; break;
+                s_led[kThreadsP + tid] += (double)E; state = L_IDLE; break;
             }
             vox = (int)gx + g.nx * ((int)gy + g.ny * (int)gz);
             uint2 vd = P.vox[vox];
-            rho = __uint_as_float(vd.x);
+            float rho = __uint_as_float(vd.x);
             tm = s_tab + (1 + (int)vd.y * TP_COUNT) * N;
-            float r = u01(k ? w4.w : w4.y) * maj;
+            float r = u01f(k ? w4.w : w4.y) * maj;
             float mu = rho * lerp(tm + TP_TOT * N, li, lf);
-            if (r > mu) { ++n_fict; continue; }
+            if (r > mu) { ++n_fi; continue; }
             float mc = rho * lerp(tm + TP_C * N, li, lf), mp = rho * lerp(tm + TP_PP * N, li, lf);
             chan = r < mc ? 0 : (r < mc + mp ? 1 : 2);
             break;
         }
-        if (chan < 0) continue;
-        uint32_t cell = cell0 + (uint32_t)vox;
-        if (chan == 2) {  // photoelectric: absorbed locally
-            ++n_pe;
-            score_add(sc, P.edep, cell, E);
-            active = false;
-            continue;
-        }
-        QRec q; q.x = x; q.y = y; q.z = z; q.hist = rng.hist; q.vox = vox;
-        if (chan == 1) {  // pair: both along the photon direction, uniform split
-            ++n_pair;
+        bump(SP_FLIGHT, n_fl);
+        if (n_fi) bump(SP_FICT, n_fi);
+        if (chan == 0) state = L_HARD;  // Compton: pending
+        else if (chan == 2) {           // photoelectric: absorbed locally
+            bump(SP_PE, 1u);
+            deposit(vox, E);
+            state = L_IDLE;
+        } else if (chan == 1) {  // pair: both along the photon direction, uniform split
+            bump(SP_PAIR, 1u);
+            QRec q; q.x = x; q.y = y; q.z = z; q.hist = rng.hist; q.vox = vox;
             uint4 a4 = next_block(rng, P.seed_lo, P.seed_hi);
-            float Tk = E - 2.0f * kMeF, us = u01(a4.z);
+            float Tk = E - 2.0f * kMeF, us = u01f(a4.z);
             q.u = u; q.v = v; q.w = w;
             q.E = us * Tk; q.trk_lo = a4.x; q.trk_hi = a4.y; q.tag = (tag & ~3u) | CODE_ELECTRON;
-            emit(P, P.q_e_out, sc, cell, q, n_sec_e);
+            emit_e(q);
             uint4 b4 = next_block(rng, P.seed_lo, P.seed_hi);
             q.E = Tk - q.E; q.trk_lo = b4.x; q.trk_hi = b4.y; q.tag = (tag & ~3u) | CODE_POSITRON;
-            emit(P, P.q_e_out, sc, cell, q, n_sec_e);
-            active = false;
-            continue;
+            emit_e(q);
+            state = L_IDLE;
         }
-        // Compton: Klein-Nishina by the epsilon decomposition (R4)
-        ++n_compton;
-        float k0 = E * (1.0f / kMeF), e0 = __fdividef(1.0f, 1.0f + 2.0f * k0), e02 = e0 * e0;
-        float a1 = -__logf(e0), a2 = 0.5f * (1.0f - e02), ik0 = __fdividef(1.0f, k0);
-        float eps, tt;
-        for (;;) {
-            uint4 c4 = next_block(rng, P.seed_lo, P.seed_hi);
-            float u1 = u01(c4.y);
-            if (u01(c4.x) * (a1 + a2) < a1) eps = __expf(-a1 * u1);
-            else eps = sqrtf(fmaf(1.0f - e02, u1, e02));
-            tt = __fdividef(1.0f - eps, eps) * ik0;
-            float sin2 = tt * (2.0f - tt);
-            if (u01(c4.z) <= 1.0f - __fdividef(eps * sin2, 1.0f + eps * eps)) break;
-        }
-        uint4 d4 = next_block(rng, P.seed_lo, P.seed_hi);
-        float E1 = eps * E, Te = E - E1;
-        float u0 = u, v0 = v, w0 = w;
-        rotate(u, v, w, tt, kTwoPiF * u01(d4.z));
-        if (Te >= P.e_cut || (P.flags & 4u)) {
-            float qx = E * u0 - E1 * u, qy = E * v0 - E1 * v, qz = E * w0 - E1 * w;
-            float inr = rsqrtf(fmaf(qx, qx, fmaf(qy, qy, qz * qz)));
-            q.u = qx * inr; q.v = qy * inr; q.w = qz * inr;
-            q.E = Te; q.trk_lo = d4.x; q.trk_hi = d4.y; q.tag = (tag & ~3u) | CODE_ELECTRON;
-            emit(P, P.q_e_out, sc, cell, q, n_sec_e);
-        } else {
-            score_add(sc, P.edep, cell, Te);  // born below the cut-off: absorbed where it is born (R26)
-        }
-        E = E1;
-        if (E < P.g_cut) { score_add(sc, P.edep, cell, E); active = false; continue; }
-        float t = (__logf(E) - P.lnE0P) * P.inv_dlnP;
-        li = min(max((int)t, 0), N - 2); lf = t - (float)li;
-        maj = lerp(s_tab, li, lf);
     }
-    score_flush(sc, P.edep);
-    unsigned long long s_fl = warp_sum(n_flight), s_fi = warp_sum(n_fict), s_c = warp_sum(n_compton), s_p = warp_sum(n_pair),
-                       s_pe = warp_sum(n_pe), s_se = warp_sum(n_sec_e), s_red = warp_sum(sc.n_red), s_hist = warp_sum(n_hist);
-    double s_src = warp_sum(e_src), s_esc = warp_sum(e_esc);
+    const int sid[SP_COUNT] = {S_FLIGHT, S_FICT, S_COMPTON, S_PAIR, S_PE, S_SEC_E, S_HIST, S_ATOMICS};
+#pragma unroll
+    for (int k = 0; k < SP_COUNT; ++k) {
+        unsigned long long s = warp_sum(s_cnt[k * kThreadsP + tid]);
+        if (lane == 0) stat_add(P.stats, sid[k], s);
+    }
+    double s_src = warp_sum(s_led[tid]), s_esc = warp_sum(s_led[kThreadsP + tid]);
     if (lane == 0) {
-        stat_add(P.stats, S_FLIGHT, s_fl); stat_add(P.stats, S_FICT, s_fi); stat_add(P.stats, S_COMPTON, s_c);
-        stat_add(P.stats, S_PAIR, s_p); stat_add(P.stats, S_PE, s_pe); stat_add(P.stats, S_SEC_E, s_se);
-        stat_add(P.stats, S_ATOMICS, s_red); stat_add(P.stats, S_HIST, s_hist);
         if (s_src != 0.0) atomicAdd(P.ledger + LG_SRC, s_src);
         if (s_esc != 0.0) atomicAdd(P.ledger + LG_ESC, s_esc);
     }
