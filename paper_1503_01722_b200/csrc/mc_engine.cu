@@ -43,7 +43,7 @@ struct mc_ctx {
     float* d_beam = nullptr;  // E nodes, pdf nodes, cdf: 3 x kMaxNodes
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     // options (M "manually adjusted")
-    int64_t wave_size = 1 << 22, queue_factor = 6, blocks_per_sm = 0, refill_lanes = 8, aggregate = 0, hard_lanes = 8;
+    int64_t wave_size = 1 << 22, queue_factor = 6, blocks_per_sm = 0, refill_lanes = 16, aggregate = 0, hard_lanes = 16;
     mc_stats stats{};
     std::string err;
 };
@@ -125,8 +125,9 @@ mc_status upload_tables(mc_ctx* ctx) {
     return MC_OK;
 }
 
-size_t smem_e(const mc_ctx* c) {  // tables + per-thread counters + per-thread energy ledger
-    return (size_t)c->tabs.n_mat * TE_COUNT * c->tabs.N * sizeof(float2) + (size_t)SE_COUNT * kThreadsE * sizeof(uint32_t) + 2 * (size_t)kThreadsE * sizeof(double);
+size_t smem_e(const mc_ctx* c) {  // tables + per-thread counters + per-thread energy ledger + parked tracks
+    return (size_t)c->tabs.n_mat * TE_COUNT * c->tabs.N * sizeof(float2) + (size_t)SE_COUNT * kThreadsE * sizeof(uint32_t) +
+           2 * (size_t)kThreadsE * sizeof(double) + (size_t)kTrackWords * kSlots * kThreadsE * sizeof(uint32_t);
 }
 size_t smem_p(const mc_ctx* c) {
     return (size_t)(1 + c->tabs.n_mat * TP_COUNT) * c->tabs.N * sizeof(float2) + (size_t)SP_COUNT * kThreadsP * sizeof(uint32_t) + 2 * (size_t)kThreadsP * sizeof(double);

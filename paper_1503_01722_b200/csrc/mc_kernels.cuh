@@ -109,10 +109,16 @@ __device__ __forceinline__ void emit(const RunParams& P, const Queue& q, Score& 
 //   REFILL queue pop / source generation (S0, S1)            — lanes in state L_IDLE
 // Divergent work is deferred until enough lanes of the warp want it (hard_lanes / refill_lanes) or nothing
 // else can run, so the rare blocks run with many lanes instead of one or two (profiles/README.md).
+// Every lane owns kSlots tracks, parked in shared memory (field-major, one bank per lane: conflict-free); a block
+// loads the lane's track that is in the state the block serves, works on it in registers and stores it back.
+// While one track of a lane waits for the HARD block, the lane keeps stepping its other track, so the STEP block
+// runs with nearly all lanes and the rare blocks can wait for nearly full warps.
 // =================================================================================================
-constexpr int kThreadsE = 128;
+constexpr int kThreadsE = 640;  // one CTA per SM: the tables are staged once per SM, 20 warps share them
+constexpr int kSlots = 2;       // tracks per lane, parked in shared memory between the blocks that work on them
 constexpr float kHingeOverrun = 0.25f;  // DESIGN.md R8
 enum LaneState { L_IDLE = 0, L_STEP = 1, L_HARD = 2, L_DONE = 3 };
+constexpr int kTrackWords = 24;
 enum { SE_STEP = 0, SE_MOLLER, SE_BREMS, SE_SEC_E, SE_SEC_G, SE_HIST, SE_RED, SE_COUNT };
 
 // distances along (u,v,w) to the three faces of voxel (ix,iy,iz) the direction points at
@@ -134,11 +140,12 @@ struct ELane {
     Rng rng;
 };
 
-__global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_constant__ RunParams P) {
+__global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_constant__ RunParams P) {
     extern __shared__ float2 s_tab[];
     const int ntab = P.n_mat * TE_COUNT * P.N;
     uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_tab + ntab);           // [SE_COUNT][kThreadsE]
     double* s_led = reinterpret_cast<double*>(s_cnt + SE_COUNT * kThreadsE);  // [2][kThreadsE]: e_src, e_esc
+    uint32_t* s_trk = reinterpret_cast<uint32_t*>(s_led + 2 * kThreadsE);      // [kTrackWords][kSlots][kThreadsE]
     for (int i = threadIdx.x; i < ntab; i += kThreadsE) s_tab[i] = P.tabE[i];
     const int tid = threadIdx.x;
 #pragma unroll
@@ -153,11 +160,47 @@ __global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_con
     const int mstride = TE_COUNT * N;
     const int KH = P.hard_lanes, KR = P.refill_lanes;
 
-    int state = L_IDLE;
+    int state = L_IDLE;            // state of the track being worked on (L)
+    int st[kSlots];                // states of this lane's parked tracks
+#pragma unroll
+    for (int k = 0; k < kSlots; ++k) st[k] = L_IDLE;
     uint32_t n_step_w = 0u;
     ELane L;
     L.x = L.y = L.z = 0.f; L.u = L.v = 0.f; L.w = 1.f; L.T = 0.f; L.ex = 0.f; L.rho = 1.f; L.tx = L.ty = L.tz = 0.f;
     L.acc = 0.f; L.smax = 0.f; L.ix = L.iy = L.iz = L.vox = L.mat = 0; L.tag = 0u; L.rng = {0, 0, 0, 0};
+    auto W = [&](int f, int k) -> uint32_t& { return s_trk[(f * kSlots + k) * kThreadsE + tid]; };
+    auto store_slot = [&](int k) {
+        W(0, k) = __float_as_uint(L.x); W(1, k) = __float_as_uint(L.y); W(2, k) = __float_as_uint(L.z);
+        W(3, k) = __float_as_uint(L.u); W(4, k) = __float_as_uint(L.v); W(5, k) = __float_as_uint(L.w);
+        W(6, k) = __float_as_uint(L.T); W(7, k) = __float_as_uint(L.ex); W(8, k) = __float_as_uint(L.rho);
+        W(9, k) = __float_as_uint(L.tx); W(10, k) = __float_as_uint(L.ty); W(11, k) = __float_as_uint(L.tz);
+        W(12, k) = __float_as_uint(L.acc); W(13, k) = __float_as_uint(L.smax);
+        W(14, k) = (uint32_t)L.ix; W(15, k) = (uint32_t)L.iy; W(16, k) = (uint32_t)L.iz; W(17, k) = (uint32_t)L.vox;
+        W(18, k) = (uint32_t)L.mat; W(19, k) = L.tag;
+        W(20, k) = L.rng.hist; W(21, k) = L.rng.trk_lo; W(22, k) = L.rng.trk_hi; W(23, k) = L.rng.block;
+    };
+    auto load_slot = [&](int k) {
+        L.x = __uint_as_float(W(0, k)); L.y = __uint_as_float(W(1, k)); L.z = __uint_as_float(W(2, k));
+        L.u = __uint_as_float(W(3, k)); L.v = __uint_as_float(W(4, k)); L.w = __uint_as_float(W(5, k));
+        L.T = __uint_as_float(W(6, k)); L.ex = __uint_as_float(W(7, k)); L.rho = __uint_as_float(W(8, k));
+        L.tx = __uint_as_float(W(9, k)); L.ty = __uint_as_float(W(10, k)); L.tz = __uint_as_float(W(11, k));
+        L.acc = __uint_as_float(W(12, k)); L.smax = __uint_as_float(W(13, k));
+        L.ix = (int)W(14, k); L.iy = (int)W(15, k); L.iz = (int)W(16, k); L.vox = (int)W(17, k);
+        L.mat = (int)W(18, k); L.tag = W(19, k);
+        L.rng.hist = W(20, k); L.rng.trk_lo = W(21, k); L.rng.trk_hi = W(22, k); L.rng.block = W(23, k);
+    };
+    // the lane's first parked track in state `want` (-1: none)
+    auto pick = [&](int want) {
+        int k = -1;
+#pragma unroll
+        for (int j = kSlots - 1; j >= 0; --j) if (st[j] == want) k = j;
+        return k;
+    };
+    auto park = [&](int k) {  // put the working track back: only live tracks need their data
+        if (state == L_STEP || state == L_HARD) store_slot(k);
+#pragma unroll
+        for (int j = 0; j < kSlots; ++j) if (j == k) st[j] = state;
+    };
 
     auto bump = [&](int k) { s_cnt[k * kThreadsE + tid] += 1u; };
     auto flush = [&]() {  // one red.global.add.f32 per (track, voxel) visit (S6)
@@ -187,17 +230,19 @@ __global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_con
     };
 
     for (;;) {
-        const unsigned m_step = __ballot_sync(kFull, state == L_STEP), m_hard = __ballot_sync(kFull, state == L_HARD),
-                       m_idle = __ballot_sync(kFull, state == L_IDLE);
+        const int k_step = pick(L_STEP), k_hard = pick(L_HARD), k_idle = pick(L_IDLE);
+        const unsigned m_step = __ballot_sync(kFull, k_step >= 0), m_hard = __ballot_sync(kFull, k_hard >= 0),
+                       m_idle = __ballot_sync(kFull, k_idle >= 0);
         const int ns = __popc(m_step), nh = __popc(m_hard), ni = __popc(m_idle);
         if ((ns | nh | ni) == 0) break;
-        const bool do_hard = nh > 0 && (nh >= KH || nh > ns || (ns == 0 && ni == 0));
+        const bool do_hard = nh > 0 && (nh >= KH || (ns == 0 && ni == 0));
         const bool do_refill = !do_hard && ni > 0 && (ni >= KR || ns == 0);
 
         if (do_refill) {
             // ---- REFILL: queue first, then new primaries (S0, S1) --------------------------------
             uint32_t item = claim(P.counters + C_HEAD, m_idle, lane);
-            if (state == L_IDLE) {
+            if (k_idle >= 0) {
+                state = L_IDLE; L.acc = 0.0f;
                 bool ok = false;
                 if (item < P.n_in) {
                     QRec r = load_record(P.q_in, item);
@@ -229,6 +274,10 @@ __global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_con
                         face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, L.ix, L.iy, L.iz, L.tx, L.ty, L.tz);
                     }
                 }
+                if (state == L_DONE) {  // nothing left to claim: every empty slot of this lane retires
+#pragma unroll
+                    for (int j = 0; j < kSlots; ++j) if (st[j] == L_IDLE) st[j] = L_DONE;
+                } else park(k_idle);
             }
             continue;
         }
@@ -237,7 +286,8 @@ __global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_con
             // ---- HARD: thinning against the running-max majorant (R6), then Moller (R10) / bremsstrahlung (R11).
             // The two event types share one code path (Philox blocks, rejection loop, rotation of the secondary,
             // queue push) so that the expensive parts run with all pending lanes, not once per type. -----------
-            if (state == L_HARD) {
+            if (k_hard >= 0) {
+                load_slot(k_hard);
                 state = L_STEP;
                 const float2* tm = tR + L.mat * mstride;
                 uint4 h4 = next_block(L.rng, P.seed_lo, P.seed_hi);
@@ -312,12 +362,15 @@ __global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_con
                     if (L.T <= P.e_cut) terminate();
                     else L.ex = fmaf(f_lg2(L.T), P.ex_a, -P.ex_b);
                 }
+                park(k_hard);
             }
             continue;
         }
 
         n_step_w += (uint32_t)ns;  // warp-uniform: every lane in state L_STEP takes a step now
-        if (state != L_STEP) continue;
+        if (k_step < 0) continue;
+        load_slot(k_step);
+        state = L_STEP;
         // ---- STEP set-up (S4): d = min[d_vox, d_maxs, d_maxe, d_range, d_event] ------------------------------
         const float2* tm = tR + L.mat * mstride;
         int i0 = min(max((int)L.ex, 0), N - 2);
@@ -404,6 +457,7 @@ __global__ void __launch_bounds__(kThreadsE, 5) electron_kernel(const __grid_con
             }
         } else if (L.T <= P.e_cut) terminate();
         else if (lim == 4) { state = L_HARD; L.smax = Smax; }
+        park(k_step);
     }
     // ---- exit: reduce the per-thread counters ------------------------------------------------------------------
     const int sid[SE_COUNT] = {S_ESTEP, S_MOLLER, S_BREMS, S_SEC_E, S_SEC_G, S_HIST, S_ATOMICS};
