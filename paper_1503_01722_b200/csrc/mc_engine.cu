@@ -43,7 +43,7 @@ struct mc_ctx {
     float* d_beam = nullptr;  // E nodes, pdf nodes, cdf: 3 x kMaxNodes
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     // options (M "manually adjusted")
-    int64_t wave_size = 1 << 22, queue_factor = 6, blocks_per_sm = 0, refill_lanes = 16, aggregate = 0, hard_lanes = 16;
+    int64_t wave_size = 1 << 22, queue_factor = 6, blocks_per_sm = 0, refill_lanes = 32, aggregate = 0, hard_lanes = 32;
     mc_stats stats{};
     std::string err;
 };
@@ -127,10 +127,11 @@ mc_status upload_tables(mc_ctx* ctx) {
 
 size_t smem_e(const mc_ctx* c) {  // tables + per-thread counters + per-thread energy ledger + parked tracks
     return (size_t)c->tabs.n_mat * TE_COUNT * c->tabs.N * sizeof(float2) + (size_t)SE_COUNT * kThreadsE * sizeof(uint32_t) +
-           2 * (size_t)kThreadsE * sizeof(double) + (size_t)kTrackWords * kSlots * kThreadsE * sizeof(uint32_t);
+           2 * (size_t)kThreadsE * sizeof(double) + (size_t)(kTrackWords * kSlots + kSlots + 1) * kThreadsE * sizeof(uint32_t);
 }
 size_t smem_p(const mc_ctx* c) {
-    return (size_t)(1 + c->tabs.n_mat * TP_COUNT) * c->tabs.N * sizeof(float2) + (size_t)SP_COUNT * kThreadsP * sizeof(uint32_t) + 2 * (size_t)kThreadsP * sizeof(double);
+    return (size_t)(1 + c->tabs.n_mat * TP_COUNT) * c->tabs.N * sizeof(float2) + (size_t)SP_COUNT * kThreadsP * sizeof(uint32_t) + 2 * (size_t)kThreadsP * sizeof(double) +
+           (size_t)(kTrackWordsP * kSlotsP + kSlotsP + 1) * kThreadsP * sizeof(uint32_t);
 }
 
 mc_status check_beam(mc_ctx* ctx, const mc_beam* b) {
@@ -595,8 +596,8 @@ mc_status mc_set_option(mc_ctx* ctx, const char* name, int64_t value) {
     if (n == "wave_size") { if (value < 1024 || value > (1ll << 28)) return fail(ctx, MC_ERR_INVALID_ARG, "wave_size in [1024, 2^28]"); ctx->wave_size = value; }
     else if (n == "queue_factor") { if (value < 2 || value > 64) return fail(ctx, MC_ERR_INVALID_ARG, "queue_factor in [2, 64]"); ctx->queue_factor = value; }
     else if (n == "blocks_per_sm") { if (value < 0 || value > 32) return fail(ctx, MC_ERR_INVALID_ARG, "blocks_per_sm in [0, 32]"); ctx->blocks_per_sm = value; }
-    else if (n == "refill_lanes") { if (value < 1 || value > 32) return fail(ctx, MC_ERR_INVALID_ARG, "refill_lanes in [1, 32]"); ctx->refill_lanes = value; }
-    else if (n == "hard_lanes") { if (value < 1 || value > 32) return fail(ctx, MC_ERR_INVALID_ARG, "hard_lanes in [1, 32]"); ctx->hard_lanes = value; }
+    else if (n == "refill_lanes") { if (value < 1 || value > 64) return fail(ctx, MC_ERR_INVALID_ARG, "refill_lanes in [1, 64]"); ctx->refill_lanes = value; }
+    else if (n == "hard_lanes") { if (value < 1 || value > 64) return fail(ctx, MC_ERR_INVALID_ARG, "hard_lanes in [1, 64]"); ctx->hard_lanes = value; }
     else if (n == "aggregate") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "aggregate in {0, 1}"); ctx->aggregate = value; }
     else return fail(ctx, MC_ERR_INVALID_ARG, "unknown option: " + n);
     return MC_OK;

@@ -146,6 +146,8 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
     uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_tab + ntab);           // [SE_COUNT][kThreadsE]
     double* s_led = reinterpret_cast<double*>(s_cnt + SE_COUNT * kThreadsE);  // [2][kThreadsE]: e_src, e_esc
     uint32_t* s_trk = reinterpret_cast<uint32_t*>(s_led + 2 * kThreadsE);      // [kTrackWords][kSlots][kThreadsE]
+    uint32_t* s_st = s_trk + kTrackWords * kSlots * kThreadsE;                 // [kSlots][kThreadsE]: slot states
+    uint32_t* s_asg = s_st + kSlots * kThreadsE;                               // [kThreadsE]: per-warp assignment
     for (int i = threadIdx.x; i < ntab; i += kThreadsE) s_tab[i] = P.tabE[i];
     const int tid = threadIdx.x;
 #pragma unroll
@@ -161,14 +163,15 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
     const int KH = P.hard_lanes, KR = P.refill_lanes;
 
     int state = L_IDLE;            // state of the track being worked on (L)
-    int st[kSlots];                // states of this lane's parked tracks
 #pragma unroll
-    for (int k = 0; k < kSlots; ++k) st[k] = L_IDLE;
+    for (int k = 0; k < kSlots; ++k) s_st[k * kThreadsE + tid] = L_IDLE;
+    const int wbase = tid & ~31;   // first thread of this warp: a warp's kSlots x 32 slots form its track pool
+    int slot = 0;                  // pool slot (k * kThreadsE + owner thread) of the track being worked on
     uint32_t n_step_w = 0u;
     ELane L;
     L.x = L.y = L.z = 0.f; L.u = L.v = 0.f; L.w = 1.f; L.T = 0.f; L.ex = 0.f; L.rho = 1.f; L.tx = L.ty = L.tz = 0.f;
     L.acc = 0.f; L.smax = 0.f; L.ix = L.iy = L.iz = L.vox = L.mat = 0; L.tag = 0u; L.rng = {0, 0, 0, 0};
-    auto W = [&](int f, int k) -> uint32_t& { return s_trk[(f * kSlots + k) * kThreadsE + tid]; };
+    auto W = [&](int f, int sl) -> uint32_t& { return s_trk[f * (kSlots * kThreadsE) + sl]; };
     auto store_slot = [&](int k) {
         W(0, k) = __float_as_uint(L.x); W(1, k) = __float_as_uint(L.y); W(2, k) = __float_as_uint(L.z);
         W(3, k) = __float_as_uint(L.u); W(4, k) = __float_as_uint(L.v); W(5, k) = __float_as_uint(L.w);
@@ -189,19 +192,10 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         L.mat = (int)W(18, k); L.tag = W(19, k);
         L.rng.hist = W(20, k); L.rng.trk_lo = W(21, k); L.rng.trk_hi = W(22, k); L.rng.block = W(23, k);
     };
-    // the lane's first parked track in state `want` (-1: none)
-    auto pick = [&](int want) {
-        int k = -1;
-#pragma unroll
-        for (int j = kSlots - 1; j >= 0; --j) if (st[j] == want) k = j;
-        return k;
+    auto park = [&]() {  // put the working track back into its pool slot: only live tracks need their data
+        if (state == L_STEP || state == L_HARD) store_slot(slot);
+        s_st[slot] = (uint32_t)state;
     };
-    auto park = [&](int k) {  // put the working track back: only live tracks need their data
-        if (state == L_STEP || state == L_HARD) store_slot(k);
-#pragma unroll
-        for (int j = 0; j < kSlots; ++j) if (j == k) st[j] = state;
-    };
-
     auto bump = [&](int k) { s_cnt[k * kThreadsE + tid] += 1u; };
     auto flush = [&]() {  // one red.global.add.f32 per (track, voxel) visit (S6)
         if (L.acc > 0.0f) { atomicAdd(P.edep + (size_t)(L.tag >> 2) * (uint32_t)g.nvox + (uint32_t)L.vox, L.acc); bump(SE_RED); }
@@ -230,18 +224,38 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
     };
 
     for (;;) {
-        const int k_step = pick(L_STEP), k_hard = pick(L_HARD), k_idle = pick(L_IDLE);
-        const unsigned m_step = __ballot_sync(kFull, k_step >= 0), m_hard = __ballot_sync(kFull, k_hard >= 0),
-                       m_idle = __ballot_sync(kFull, k_idle >= 0);
-        const int ns = __popc(m_step), nh = __popc(m_hard), ni = __popc(m_idle);
+        // ---- scheduling: count the pool's tracks by state, choose ONE block, hand its tracks to the lanes ------
+        unsigned ms[kSlots], mh[kSlots], mi[kSlots];
+        int ns = 0, nh = 0, ni = 0;
+#pragma unroll
+        for (int k = 0; k < kSlots; ++k) {
+            const uint32_t sk = s_st[k * kThreadsE + tid];
+            ms[k] = __ballot_sync(kFull, sk == L_STEP); mh[k] = __ballot_sync(kFull, sk == L_HARD);
+            mi[k] = __ballot_sync(kFull, sk == L_IDLE);
+            ns += __popc(ms[k]); nh += __popc(mh[k]); ni += __popc(mi[k]);
+        }
         if ((ns | nh | ni) == 0) break;
-        const bool do_hard = nh > 0 && (nh >= KH || (ns == 0 && ni == 0));
-        const bool do_refill = !do_hard && ni > 0 && (ni >= KR || ns == 0);
-
+        // a rare block runs when it can fill a warp (>= KH / KR tracks), or when it has more tracks than STEP
+        const bool do_hard = nh >= KH || (nh > ns && nh >= ni);
+        const bool do_refill = !do_hard && (ni >= KR || ni > ns);
+        // the r-th track of the chosen state (slot-major, then owner lane) goes to lane r: its owner posts the slot
+        int rank = 0;
+#pragma unroll
+        for (int k = 0; k < kSlots; ++k) {
+            const unsigned m = do_hard ? mh[k] : (do_refill ? mi[k] : ms[k]);
+            const int r = rank + __popc(m & ((1u << lane) - 1u));
+            if (((m >> lane) & 1u) && r < 32) s_asg[wbase + r] = (uint32_t)(k * kThreadsE + tid);
+            rank += __popc(m);
+        }
+        __syncwarp();
+        const int n_work = min(rank, 32);
+        const bool have = lane < n_work;
+        slot = have ? (int)s_asg[wbase + lane] : 0;
+        __syncwarp();
         if (do_refill) {
             // ---- REFILL: queue first, then new primaries (S0, S1) --------------------------------
-            uint32_t item = claim(P.counters + C_HEAD, m_idle, lane);
-            if (k_idle >= 0) {
+            uint32_t item = claim(P.counters + C_HEAD, n_work >= 32 ? kFull : ((1u << n_work) - 1u), lane);
+            if (have) {
                 state = L_IDLE; L.acc = 0.0f;
                 bool ok = false;
                 if (item < P.n_in) {
@@ -274,11 +288,9 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
                         face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, L.ix, L.iy, L.iz, L.tx, L.ty, L.tz);
                     }
                 }
-                if (state == L_DONE) {  // nothing left to claim: every empty slot of this lane retires
-#pragma unroll
-                    for (int j = 0; j < kSlots; ++j) if (st[j] == L_IDLE) st[j] = L_DONE;
-                } else park(k_idle);
+                park();  // L_DONE (nothing left to claim) retires the slot
             }
+            __syncwarp();
             continue;
         }
 
@@ -286,8 +298,8 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
             // ---- HARD: thinning against the running-max majorant (R6), then Moller (R10) / bremsstrahlung (R11).
             // The two event types share one code path (Philox blocks, rejection loop, rotation of the secondary,
             // queue push) so that the expensive parts run with all pending lanes, not once per type. -----------
-            if (k_hard >= 0) {
-                load_slot(k_hard);
+            if (have) {
+                load_slot(slot);
                 state = L_STEP;
                 const float2* tm = tR + L.mat * mstride;
                 uint4 h4 = next_block(L.rng, P.seed_lo, P.seed_hi);
@@ -362,14 +374,15 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
                     if (L.T <= P.e_cut) terminate();
                     else L.ex = fmaf(f_lg2(L.T), P.ex_a, -P.ex_b);
                 }
-                park(k_hard);
+                park();
             }
+            __syncwarp();
             continue;
         }
 
-        n_step_w += (uint32_t)ns;  // warp-uniform: every lane in state L_STEP takes a step now
-        if (k_step < 0) continue;
-        load_slot(k_step);
+        n_step_w += (uint32_t)n_work;  // warp-uniform: n_work tracks take a step now
+        if (!have) { __syncwarp(); continue; }
+        load_slot(slot);
         state = L_STEP;
         // ---- STEP set-up (S4): d = min[d_vox, d_maxs, d_maxe, d_range, d_event] ------------------------------
         const float2* tm = tR + L.mat * mstride;
@@ -457,7 +470,8 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
             }
         } else if (L.T <= P.e_cut) terminate();
         else if (lim == 4) { state = L_HARD; L.smax = Smax; }
-        park(k_step);
+        park();
+        __syncwarp();
     }
     // ---- exit: reduce the per-thread counters ------------------------------------------------------------------
     const int sid[SE_COUNT] = {S_ESTEP, S_MOLLER, S_BREMS, S_SEC_E, S_SEC_G, S_HIST, S_ATOMICS};
@@ -479,14 +493,19 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
 // kernel: per iteration a warp runs ONE of  FLY (lanes in L_STEP) / COMPTON (lanes in L_HARD, pending) /
 // REFILL (lanes in L_IDLE), the rare blocks only when enough lanes want them.
 // =================================================================================================
-constexpr int kThreadsP = 128;
+constexpr int kThreadsP = 640;  // one CTA per SM
+constexpr int kSlotsP = 3;     // tracks per lane in the warp's pool (shared memory)
+constexpr int kTrackWordsP = 13;
 enum { SP_FLIGHT = 0, SP_FICT, SP_COMPTON, SP_PAIR, SP_PE, SP_SEC_E, SP_HIST, SP_RED, SP_COUNT };
 
-__global__ void __launch_bounds__(kThreadsP, 6) photon_kernel(const __grid_constant__ RunParams P) {
+__global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_constant__ RunParams P) {
     extern __shared__ float2 s_tab[];
     const int ntab = (1 + P.n_mat * TP_COUNT) * P.N;
     uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_tab + ntab);              // [SP_COUNT][kThreadsP]
     double* s_led = reinterpret_cast<double*>(s_cnt + SP_COUNT * kThreadsP);  // [2][kThreadsP]: e_src, e_esc
+    uint32_t* s_trk = reinterpret_cast<uint32_t*>(s_led + 2 * kThreadsP);      // [kTrackWordsP][kSlotsP][kThreadsP]
+    uint32_t* s_st = s_trk + kTrackWordsP * kSlotsP * kThreadsP;               // [kSlotsP][kThreadsP]: slot states
+    uint32_t* s_asg = s_st + kSlotsP * kThreadsP;                              // [kThreadsP]: per-warp assignment
     for (int i = threadIdx.x; i < ntab; i += kThreadsP) s_tab[i] = P.tabP[i];
     const int tid = threadIdx.x;
 #pragma unroll
@@ -500,11 +519,32 @@ __global__ void __launch_bounds__(kThreadsP, 6) photon_kernel(const __grid_const
     const int KC = P.hard_lanes, KR = P.refill_lanes;
     const float lg_a = kLn2F * P.inv_dlnP, lg_b = P.lnE0P * P.inv_dlnP;  // table coordinate = lg2(E) * lg_a - lg_b
 
-    int state = L_IDLE;
+    int state = L_IDLE;  // state of the track being worked on
+#pragma unroll
+    for (int k = 0; k < kSlotsP; ++k) s_st[k * kThreadsP + tid] = L_IDLE;
+    const int wbase = tid & ~31;
+    int slot = 0;
     float x = 0, y = 0, z = 0, u = 0, v = 0, w = 1, E = 0, lf = 0, maj = 1;
     int li = 0, vox = 0;
     Rng rng = {0, 0, 0, 0};
     uint32_t tag = 0;
+    auto W = [&](int f, int sl) -> uint32_t& { return s_trk[f * (kSlotsP * kThreadsP) + sl]; };
+    auto store_slot = [&](int sl) {
+        W(0, sl) = __float_as_uint(x); W(1, sl) = __float_as_uint(y); W(2, sl) = __float_as_uint(z);
+        W(3, sl) = __float_as_uint(u); W(4, sl) = __float_as_uint(v); W(5, sl) = __float_as_uint(w);
+        W(6, sl) = __float_as_uint(E); W(7, sl) = (uint32_t)vox; W(8, sl) = tag;
+        W(9, sl) = rng.hist; W(10, sl) = rng.trk_lo; W(11, sl) = rng.trk_hi; W(12, sl) = rng.block;
+    };
+    auto load_slot = [&](int sl) {
+        x = __uint_as_float(W(0, sl)); y = __uint_as_float(W(1, sl)); z = __uint_as_float(W(2, sl));
+        u = __uint_as_float(W(3, sl)); v = __uint_as_float(W(4, sl)); w = __uint_as_float(W(5, sl));
+        E = __uint_as_float(W(6, sl)); vox = (int)W(7, sl); tag = W(8, sl);
+        rng.hist = W(9, sl); rng.trk_lo = W(10, sl); rng.trk_hi = W(11, sl); rng.block = W(12, sl);
+    };
+    auto park = [&]() {
+        if (state == L_STEP || state == L_HARD) store_slot(slot);
+        s_st[slot] = (uint32_t)state;
+    };
 
     auto bump = [&](int k, uint32_t n) { s_cnt[k * kThreadsP + tid] += n; };
     auto deposit = [&](int vx, float e) {
@@ -523,17 +563,37 @@ __global__ void __launch_bounds__(kThreadsP, 6) photon_kernel(const __grid_const
     };
 
     for (;;) {
-        const unsigned m_fly = __ballot_sync(kFull, state == L_STEP), m_comp = __ballot_sync(kFull, state == L_HARD),
-                       m_idle = __ballot_sync(kFull, state == L_IDLE);
-        const int nf = __popc(m_fly), nc = __popc(m_comp), ni = __popc(m_idle);
+        unsigned ms[kSlotsP], mh[kSlotsP], mi[kSlotsP];
+        int nf = 0, nc = 0, ni = 0;
+#pragma unroll
+        for (int k = 0; k < kSlotsP; ++k) {
+            const uint32_t sk = s_st[k * kThreadsP + tid];
+            ms[k] = __ballot_sync(kFull, sk == L_STEP); mh[k] = __ballot_sync(kFull, sk == L_HARD);
+            mi[k] = __ballot_sync(kFull, sk == L_IDLE);
+            nf += __popc(ms[k]); nc += __popc(mh[k]); ni += __popc(mi[k]);
+        }
         if ((nf | nc | ni) == 0) break;
-        const bool do_comp = nc > 0 && (nc >= KC || nc > nf || (nf == 0 && ni == 0));
-        const bool do_refill = !do_comp && ni > 0 && (ni >= KR || nf == 0);
+        const bool do_comp = nc >= KC || (nc > nf && nc >= ni);
+        const bool do_refill = !do_comp && (ni >= KR || ni > nf);
+        int rank = 0;
+#pragma unroll
+        for (int k = 0; k < kSlotsP; ++k) {
+            const unsigned m = do_comp ? mh[k] : (do_refill ? mi[k] : ms[k]);
+            const int r = rank + __popc(m & ((1u << lane) - 1u));
+            if (((m >> lane) & 1u) && r < 32) s_asg[wbase + r] = (uint32_t)(k * kThreadsP + tid);
+            rank += __popc(m);
+        }
+        __syncwarp();
+        const int n_work = min(rank, 32);
+        const bool have = lane < n_work;
+        slot = have ? (int)s_asg[wbase + lane] : 0;
+        __syncwarp();
 
         if (do_refill) {
             // ---- REFILL (S0, S1) --------------------------------------------------------------------------------
-            uint32_t item = claim(P.counters + C_HEAD, m_idle, lane);
-            if (state == L_IDLE) {
+            uint32_t item = claim(P.counters + C_HEAD, n_work >= 32 ? kFull : ((1u << n_work) - 1u), lane);
+            if (have) {
+                state = L_IDLE;
                 bool ok = false;
                 if (item < P.n_in) {
                     QRec r = load_record(P.q_in, item);
@@ -554,15 +614,18 @@ __global__ void __launch_bounds__(kThreadsP, 6) photon_kernel(const __grid_const
                 } else state = L_DONE;
                 if (ok) {
                     if (E < P.g_cut) deposit(vox, E);  // absorbed where it was born
-                    else { set_energy(); state = L_STEP; }
+                    else state = L_STEP;
                 }
+                park();
             }
+            __syncwarp();
             continue;
         }
 
         if (do_comp) {
             // ---- COMPTON: Klein-Nishina by the epsilon decomposition (R4) ----------------------------------------
-            if (state == L_HARD) {
+            if (have) {
+                load_slot(slot);
                 bump(SP_COMPTON, 1u);
                 const float k0 = E * (1.0f / kMeF), e0 = f_rcp(1.0f + 2.0f * k0), e02 = e0 * e0;
                 const float a1l2 = -f_lg2(e0), a1 = a1l2 * kLn2F, a2 = 0.5f * (1.0f - e02), ik0 = f_rcp(k0);
@@ -592,13 +655,18 @@ __global__ void __launch_bounds__(kThreadsP, 6) photon_kernel(const __grid_const
                 } else dep = Te;  // born below the cut-off: absorbed where it is born (R26)
                 E = E1;
                 if (E < P.g_cut) { dep += E; state = L_IDLE; }
-                else { set_energy(); state = L_STEP; }
+                else state = L_STEP;
                 if (dep > 0.0f) deposit(vox, dep);
+                park();
             }
+            __syncwarp();
             continue;
         }
 
-        if (state != L_STEP) continue;
+        if (!have) { __syncwarp(); continue; }
+        load_slot(slot);
+        state = L_STEP;
+        set_energy();
         // ---- FLY: up to two Woodcock flights from one Philox block (S2) --------------------------------------------
         uint4 w4 = next_block(rng, P.seed_lo, P.seed_hi);
         int chan = -1;
@@ -645,6 +713,8 @@ __global__ void __launch_bounds__(kThreadsP, 6) photon_kernel(const __grid_const
             emit_e(q);
             state = L_IDLE;
         }
+        park();
+        __syncwarp();
     }
     const int sid[SP_COUNT] = {S_FLIGHT, S_FICT, S_COMPTON, S_PAIR, S_PE, S_SEC_E, S_HIST, S_ATOMICS};
 #pragma unroll
