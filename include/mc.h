@@ -179,7 +179,8 @@ mc_status mc_set_stream(mc_ctx *ctx, void *cuda_stream);
 /* Tuning knobs ("the number of workitems M ... manually adjusted"):
  * name = "wave_size" (histories admitted per scheduling round), "queue_factor" (queue capacity in waves),
  * "blocks_per_sm", "refill_lanes" (idle lanes per warp that trigger a refill), "hard_lanes" (lanes per warp with a
- * pending hard event that trigger the Moller / bremsstrahlung block), "aggregate" (reserved).  Scheduling only:
+ * pending hard event that trigger the Moller / bremsstrahlung block), "adaptive" (1: the number of new primaries a launch admits is limited by the room left in the
+ * output queues at the measured secondaries-per-primary ratio; 0: always a full wave), "aggregate" (reserved).  Scheduling only:
  * per-history results do not depend on them (R14). */
 mc_status mc_set_option(mc_ctx *ctx, const char *name, int64_t value);
 const char *mc_last_error(const mc_ctx *ctx);

@@ -43,7 +43,7 @@ struct mc_ctx {
     float* d_beam = nullptr;  // E nodes, pdf nodes, cdf: 3 x kMaxNodes
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     // options (M "manually adjusted")
-    int64_t wave_size = 1 << 22, queue_factor = 6, blocks_per_sm = 0, refill_lanes = 32, aggregate = 0, hard_lanes = 32;
+    int64_t wave_size = 1 << 24, queue_factor = 4, blocks_per_sm = 0, refill_lanes = 32, aggregate = 0, hard_lanes = 32, adaptive = 1;
     mc_stats stats{};
     std::string err;
 };
@@ -252,6 +252,7 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, uint64_t n_total, uint64_t
     mc_stats& S = ctx->stats;
     S = mc_stats{};
     double ms_e = 0, ms_p = 0;
+    double m_new_e = 16.0, m_new_p = 16.0;  // secondaries queued per new primary (electron queue, photon queue)
     CU(cudaEventRecord(ctx->ev[0], s));
     while (remaining > 0 || cnt_e[cur] > 0 || cnt_p > 0) {
         bool run_p;
@@ -262,7 +263,15 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, uint64_t n_total, uint64_t
             run_p = avail_p > avail_e;
         }
         uint32_t n_in = run_p ? cnt_p : cnt_e[cur], n_new = 0;
-        if (run_p == photon_beam && n_in < W) n_new = (uint32_t)std::min<uint64_t>(remaining, W - n_in);
+        if (run_p == photon_beam && n_in < W) {
+            // new primaries admitted by this launch: up to a wave, and no more than the output queues can take at
+            // the secondaries-per-primary ratio measured so far (first launch: a probe of cap / 16 histories)
+            const double room_e = (double)ctx->q_cap - (run_p ? cnt_e[cur] : 0u) - (double)n_in;
+            const double room_p = run_p ? 1e30 : (double)ctx->q_cap - cnt_p - (double)n_in;
+            const double fit = ctx->adaptive ? std::max(0.0, std::min(room_e / m_new_e, room_p / m_new_p)) : 1e30;
+            n_new = (uint32_t)std::min<double>((double)std::min<uint64_t>(remaining, W - n_in), fit);
+            if (n_new == 0 && n_in == 0) n_new = (uint32_t)std::min<uint64_t>(remaining, 1024);  // always progress
+        }
         P.n_in = n_in; P.n_new = n_new; P.h_first = h_next;
         Queue qe_cur{ctx->d_q[cur], ctx->d_counters + C_E_A + cur, ctx->q_cap};
         Queue qe_oth{ctx->d_q[1 - cur], ctx->d_counters + C_E_A + (1 - cur), ctx->q_cap};
@@ -293,6 +302,13 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, uint64_t n_total, uint64_t
         if (ctx->h_counters[C_OVERFLOW])
             return fail(ctx, MC_ERR_QUEUE_OVERFLOW, "particle queue overflow: lower option wave_size or raise queue_factor");
         remaining -= n_new; h_next += n_new;
+        if (n_new >= n_in && n_new >= 1024) {  // a launch dominated by primaries: update the measured ratios
+            const double out_e = run_p ? (double)ctx->h_counters[C_E_A + cur] - cnt_e[cur] : (double)ctx->h_counters[C_E_A + (1 - cur)];
+            const double out_p = run_p ? 0.0 : (double)ctx->h_counters[C_P] - cnt_p;
+            const double n_items = (double)n_in + n_new;
+            m_new_e = std::max(0.05, 1.5 * out_e / n_items);
+            m_new_p = std::max(0.05, 1.5 * out_p / n_items);
+        }
         if (run_p) { cnt_p = 0; cnt_e[cur] = ctx->h_counters[C_E_A + cur]; }
         else { cnt_e[cur] = 0; cur = 1 - cur; cnt_e[cur] = ctx->h_counters[C_E_A + cur]; cnt_p = ctx->h_counters[C_P]; }
     }
@@ -598,6 +614,7 @@ mc_status mc_set_option(mc_ctx* ctx, const char* name, int64_t value) {
     else if (n == "blocks_per_sm") { if (value < 0 || value > 32) return fail(ctx, MC_ERR_INVALID_ARG, "blocks_per_sm in [0, 32]"); ctx->blocks_per_sm = value; }
     else if (n == "refill_lanes") { if (value < 1 || value > 64) return fail(ctx, MC_ERR_INVALID_ARG, "refill_lanes in [1, 64]"); ctx->refill_lanes = value; }
     else if (n == "hard_lanes") { if (value < 1 || value > 64) return fail(ctx, MC_ERR_INVALID_ARG, "hard_lanes in [1, 64]"); ctx->hard_lanes = value; }
+    else if (n == "adaptive") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "adaptive in {0, 1}"); ctx->adaptive = value; }
     else if (n == "aggregate") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "aggregate in {0, 1}"); ctx->aggregate = value; }
     else return fail(ctx, MC_ERR_INVALID_ARG, "unknown option: " + n);
     return MC_OK;

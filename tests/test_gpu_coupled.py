@@ -288,19 +288,21 @@ def test_beam_that_misses_and_energy_ledger_of_escapes():
 
 
 def test_queue_overflow_is_reported_never_dropped():
-    """R21: a queue too small for the secondaries of one wave -> MC_ERR_QUEUE_OVERFLOW, no result."""
+    """R21: with admission control off, a queue too small for the secondaries of one wave -> MC_ERR_QUEUE_OVERFLOW
+    and no result; with it on (the default) the scheduler admits fewer primaries per launch and the same tiny
+    queue suffices."""
     cfg = W.config(2)
     eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])
     mc.mc_set_option(eng.ctx, "wave_size", 4096)
     mc.mc_set_option(eng.ctx, "queue_factor", 2)
+    mc.mc_set_option(eng.ctx, "adaptive", 0)
     with pytest.raises(mc.McError) as e:
         eng.run(cfg["beam"], 200000, 1, 10)
     assert e.value.status == mc.MC_ERR_QUEUE_OVERFLOW
-    # and the same context recovers with a sufficient queue
-    mc.mc_set_option(eng.ctx, "queue_factor", 16)
+    mc.mc_set_option(eng.ctx, "adaptive", 1)
     d, _ = eng.run(cfg["beam"], 200000, 1, 10)
     st = eng.stats()
-    assert _ledger(st) < 1e-4 and d.max() > 0
+    assert _ledger(st) < 1e-4 and d.max() > 0 and st["n_histories"] == 200000
     eng.close()
 
 
