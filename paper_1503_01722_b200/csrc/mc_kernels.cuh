@@ -172,15 +172,21 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
     L.x = L.y = L.z = 0.f; L.u = L.v = 0.f; L.w = 1.f; L.T = 0.f; L.ex = 0.f; L.rho = 1.f; L.tx = L.ty = L.tz = 0.f;
     L.acc = 0.f; L.smax = 0.f; L.ix = L.iy = L.iz = L.vox = L.mat = 0; L.tag = 0u; L.rng = {0, 0, 0, 0};
     auto W = [&](int f, int sl) -> uint32_t& { return s_trk[f * (kSlots * kThreadsE) + sl]; };
-    auto store_slot = [&](int k) {
+    // what = 0: a new track, every word; 1: after a step or a hard event that stayed in its voxel; 2: after a step
+    // that crossed into another voxel.  Identity words (tag, history, track id) never change after birth.
+    auto store_slot = [&](int k, int what) {
         W(0, k) = __float_as_uint(L.x); W(1, k) = __float_as_uint(L.y); W(2, k) = __float_as_uint(L.z);
         W(3, k) = __float_as_uint(L.u); W(4, k) = __float_as_uint(L.v); W(5, k) = __float_as_uint(L.w);
-        W(6, k) = __float_as_uint(L.T); W(7, k) = __float_as_uint(L.ex); W(8, k) = __float_as_uint(L.rho);
+        W(6, k) = __float_as_uint(L.T); W(7, k) = __float_as_uint(L.ex);
         W(9, k) = __float_as_uint(L.tx); W(10, k) = __float_as_uint(L.ty); W(11, k) = __float_as_uint(L.tz);
-        W(12, k) = __float_as_uint(L.acc); W(13, k) = __float_as_uint(L.smax);
-        W(14, k) = (uint32_t)L.ix; W(15, k) = (uint32_t)L.iy; W(16, k) = (uint32_t)L.iz; W(17, k) = (uint32_t)L.vox;
-        W(18, k) = (uint32_t)L.mat; W(19, k) = L.tag;
-        W(20, k) = L.rng.hist; W(21, k) = L.rng.trk_lo; W(22, k) = L.rng.trk_hi; W(23, k) = L.rng.block;
+        W(12, k) = __float_as_uint(L.acc); W(23, k) = L.rng.block;
+        if (state == L_HARD) W(13, k) = __float_as_uint(L.smax);
+        if (what != 1) {
+            W(8, k) = __float_as_uint(L.rho);
+            W(14, k) = (uint32_t)L.ix; W(15, k) = (uint32_t)L.iy; W(16, k) = (uint32_t)L.iz; W(17, k) = (uint32_t)L.vox;
+            W(18, k) = (uint32_t)L.mat;
+        }
+        if (what == 0) { W(19, k) = L.tag; W(20, k) = L.rng.hist; W(21, k) = L.rng.trk_lo; W(22, k) = L.rng.trk_hi; }
     };
     auto load_slot = [&](int k) {
         L.x = __uint_as_float(W(0, k)); L.y = __uint_as_float(W(1, k)); L.z = __uint_as_float(W(2, k));
@@ -192,8 +198,8 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         L.mat = (int)W(18, k); L.tag = W(19, k);
         L.rng.hist = W(20, k); L.rng.trk_lo = W(21, k); L.rng.trk_hi = W(22, k); L.rng.block = W(23, k);
     };
-    auto park = [&]() {  // put the working track back into its pool slot: only live tracks need their data
-        if (state == L_STEP || state == L_HARD) store_slot(slot);
+    auto park = [&](int what) {  // put the working track back into its pool slot: only live tracks need their data
+        if (state == L_STEP || state == L_HARD) store_slot(slot, what);
         s_st[slot] = (uint32_t)state;
     };
     auto bump = [&](int k) { s_cnt[k * kThreadsE + tid] += 1u; };
@@ -288,7 +294,7 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
                         face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, L.ix, L.iy, L.iz, L.tx, L.ty, L.tz);
                     }
                 }
-                park();  // L_DONE (nothing left to claim) retires the slot
+                park(0);  // L_DONE (nothing left to claim) retires the slot
             }
             __syncwarp();
             continue;
@@ -374,7 +380,7 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
                     if (L.T <= P.e_cut) terminate();
                     else L.ex = fmaf(f_lg2(L.T), P.ex_a, -P.ex_b);
                 }
-                park();
+                park(1);
             }
             __syncwarp();
             continue;
@@ -470,7 +476,7 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
             }
         } else if (L.T <= P.e_cut) terminate();
         else if (lim == 4) { state = L_HARD; L.smax = Smax; }
-        park();
+        park(cross ? 2 : 1);
         __syncwarp();
     }
     // ---- exit: reduce the per-thread counters ------------------------------------------------------------------
