@@ -307,7 +307,10 @@ def run_engine(args):
     alg, kms = (alg_e, e_ms) if dom == "electron_kernel" else (alg_p, p_ms)
     achieved = alg / (kms * 1e-3) if kms > 0 else 0.0
     roofline = {"bound": "alu", "kernel": dom, "achieved": achieved / 1e12, "peak": issue_peak / 1e12,
-                "unit": "Tinstr/s (thread-instructions)", "frac": achieved / issue_peak, "traffic": None,
+                "unit": "Tinstr/s (thread-instructions)", "frac": achieved / issue_peak,
+                # dram__bytes_read.sum + dram__bytes_write.sum of one launch of that kernel (a wave of primaries) from the
+                # committed ncu --set full capture, profiles/r1b_*_kernel_ncu_full.txt: queue records, not a bound
+                "traffic": {"electron_kernel": 436.7e6, "photon_kernel": 159.9e6}[dom], "traffic_unit": "bytes per launch (ncu capture, profiles/)",
                 "peak_source": f"148 SM x 4 schedulers x 32 lanes x sm_max_mhz ({pk_kind} MEASURED_PEAKS.json clock)",
                 "kernel_ms_per_step": kms / K, "kernel_share_of_step": kms / total_ms if world == 1 else None}
     # scoring roofline: measured red.global.add.f32 peak into a window the size of one batch grid

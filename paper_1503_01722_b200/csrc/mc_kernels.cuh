@@ -1,5 +1,5 @@
-// Transport, scoring and statistics kernels (sm_100a).  One warp lane = one particle track; lanes
-// refill themselves from the input queue / the source while the kernel runs.
+// Transport, scoring and statistics kernels (sm_100a).  Tracks live in per-warp pools in shared memory; per
+// iteration a warp runs ONE block on up to 32 tracks that are in the state the block serves.
 //   electron_kernel : Class II condensed-history steps, d = min[d_vox, d_maxs, d_maxe, d_event]
 //                     (PAPER.md:39), Moller / bremsstrahlung hard events, random-hinge MS deflection,
 //                     CSDA loss through the range table, dose by red.global.add.f32
