@@ -43,7 +43,8 @@ def parse():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="engine", choices=["engine", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config, 1-based (default 2 = configs[1])")
+    ap.add_argument("--config", default="2", help="BASELINE.json config, 1-based (default 2 = configs[1]); p1..p5 = the paper's "
+                    "own five cases (128^3 x 0.25 cm, 2x2 cm^2 field: context beside its Tables 2-3)")
     ap.add_argument("--beam", default=None, choices=[None, "e", "g"], help="configs 4, 5: electron or photon beam")
     ap.add_argument("--histories", type=int, default=0, help="override n_histories (the line then says so)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -102,7 +103,7 @@ def workload(args):
 
 
 def config_dict(cfg, args, extra=None):
-    d = {"workload": f"BASELINE config {args.config}: {cfg['name']}", "n_histories_per_step": cfg["n_histories"],
+    d = {"workload": (f"paper-shaped case {args.config}: " if str(args.config).startswith("p") else f"BASELINE config {args.config}: ") + cfg["name"], "n_histories_per_step": cfg["n_histories"],
          "n_batches": cfg["n_batches"], "dims": [int(x) for x in cfg["phantom"]["dims"]],
          "voxel_cm": float(cfg["phantom"]["voxel_cm"][0]), "e_cut_MeV": cfg["params"]["e_cut_MeV"],
          "g_cut_MeV": cfg["params"]["g_cut_MeV"], "seed": cfg["seed"],

@@ -146,6 +146,21 @@ mc_status mc_set_photon_tables(mc_ctx *ctx, float lnE0, float inv_dln, const flo
 mc_status mc_run(mc_ctx *ctx, const mc_beam *beam, uint64_t n_histories, uint64_t seed, int32_t n_batches,
                  float *dose_out, float *sigma_out);
 
+/* One source particle of a particle list (a phase-space record; PAPER.md:84 leaves the source interface open:
+ * "phase-space file" or a "user ... function").  particle: 0 photon, -1 electron, +1 positron; position in cm in
+ * phantom coordinates; (u, v, w) a unit vector; E kinetic energy in MeV (<= e_max_MeV). */
+typedef struct {
+    float x, y, z, u, v, w, E;
+    int32_t particle;
+} mc_particle;
+
+/* mc_run_particles — as mc_run, but the source is a list: history h is particles[h], transported with track id (0,0)
+ * from Philox block 0 (R13b).  A particle outside the phantom counts as escaped (no re-entry, R3).
+ * particles: n records, HOST or DEVICE memory (a host list is validated and staged; a device list is read in place and
+ * must already satisfy the constraints above).  Other arguments and errors as mc_run. */
+mc_status mc_run_particles(mc_ctx *ctx, const mc_particle *particles, uint64_t n, uint64_t seed, int32_t n_batches,
+                           float *dose_out, float *sigma_out);
+
 /* mc_run_range — the shard of mc_run one GPU of several computes: histories [h_begin, h_end) of a
  * job of n_histories.  edep_out: n_batches*nvox floats (host or device), energy deposited per batch
  * grid in MeV (sum these over shards, then call mc_finalize). */

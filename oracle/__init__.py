@@ -202,6 +202,46 @@ class Oracle:
             return edep, dict(zip(STAT_NAMES, st)), fv, fc
         return edep, dict(zip(STAT_NAMES, st))
 
+    def run_particles_edep(self, particles, n_total, seed, n_batches, h0=0, h1=None):
+        """Particle-list source: `particles` is a structured array (x, y, z, u, v, w, E float32, particle int32)."""
+        h1 = n_total if h1 is None else h1
+        pa = np.ascontiguousarray(particles)
+        assert pa.dtype.itemsize == 32
+        b_lo, b_hi = (h0 * n_batches) // n_total, ((max(h1, h0 + 1) - 1) * n_batches) // n_total
+        edep = np.zeros((b_hi - b_lo + 1, self.nvox))
+        st = np.zeros(lib().orc_n_stats())
+        base = C.cast(C.c_void_p(edep.ctypes.data - b_lo * self.nvox * 8), C.POINTER(C.c_double))
+        rc = lib().orc_run_particles(self._h, C.c_void_p(pa.ctypes.data), C.c_uint64(h0), C.c_uint64(h1), C.c_uint64(n_total),
+                                     C.c_uint64(seed), int(n_batches), base, _dp(st))
+        if rc:
+            raise ValueError(f"orc_run_particles failed ({rc})")
+        return b_lo, edep, dict(zip(STAT_NAMES, st))
+
+    def run_particles(self, particles, seed, n_batches, workers=1):
+        """dose, sigma, stats for a particle list, sharded over `workers` processes by history range."""
+        n = len(particles)
+        global _FORK_ORC
+        edges = np.linspace(0, n, max(1, workers) * 4 + 1).astype(np.int64)
+        jobs = [(particles, n, seed, n_batches, int(edges[i]), int(edges[i + 1])) for i in range(len(edges) - 1)
+                if edges[i + 1] > edges[i]]
+        edep = np.zeros((n_batches, self.nvox))
+        stats = []
+        if workers <= 1:
+            res = [self.run_particles_edep(*j) for j in jobs]
+        else:
+            _FORK_ORC = self
+            try:
+                with mp.get_context("fork").Pool(workers) as pool:
+                    res = pool.map(_shard_particles, jobs, chunksize=1)
+            finally:
+                _FORK_ORC = None
+        for b_lo, part, st in res:
+            edep[b_lo:b_lo + part.shape[0]] += part
+            stats.append(st)
+        st = {k: (max(r[k] for r in stats) if k == "max_ledger_rel" else sum(r[k] for r in stats)) for k in STAT_NAMES}
+        dose, sig = self.finalize(edep, n)
+        return dose, sig, st
+
     def finalize(self, edep, n_total):
         B = edep.shape[0]
         dose, sig = np.zeros(self.nvox), np.zeros(self.nvox)
@@ -294,6 +334,10 @@ def sample_ms(a, n, seed=1):
 
 # -- sharding over host cores -------------------------------------------------------------------
 _FORK_ORC = None  # the parent's Oracle, inherited by forked workers (tables are built once, not per chunk)
+
+
+def _shard_particles(args):
+    return _FORK_ORC.run_particles_edep(*args)
 
 
 def _shard(args):

@@ -460,6 +460,28 @@ struct Run {
         }
     }
 
+    // History h of a particle-list source ("phase-space file"; R13b): the listed particle is the
+    // primary, track id (0,0), stream from block 0; outside the phantom it counts as escaped.
+    void history_listed(uint32_t h, int q, const double x[3], const double d[3], double E) {
+        hist = h; led_src = led_dep = led_esc = 0; first_vox = -1; first_chan = -1;
+        st.n_hist += 1;
+        Particle p; p.q = q; p.E = E; p.trk_lo = 0; p.trk_hi = 0; p.blk0 = 0;
+        for (int a = 0; a < 3; ++a) { p.x[a] = x[a]; p.d[a] = d[a]; }
+        double e0 = E + (q > 0 ? 2.0 * MEC2 : 0.0);
+        led_src += e0; st.e_src += e0;
+        if (!locate(p.x, p.v)) escape(e0);
+        else {
+            stack.clear();
+            stack.push_back(p);
+            while (!stack.empty()) {
+                Particle t = stack.back(); stack.pop_back();
+                if (t.q == 0) photon(t); else electron(t);
+            }
+        }
+        double rel = std::fabs(led_dep + led_esc - led_src) / led_src;
+        if (rel > st.max_ledger_rel) st.max_ledger_rel = rel;
+    }
+
     void history(uint32_t h) {
         hist = h; led_src = led_dep = led_esc = 0; first_vox = -1; first_chan = -1;
         Particle p;
@@ -638,6 +660,28 @@ int orc_run(Ctx* c, const orc_beam* b, uint64_t h0, uint64_t h1, uint64_t n_tota
     return 0;
 }
 int orc_n_stats() { return N_STATS; }
+
+// Particle-list source: histories [h0, h1) are particles[h0 .. h1) (records of 7 floats + int32, as mc_particle).
+struct orc_particle { float x, y, z, u, v, w, E; int32_t particle; };
+int orc_run_particles(Ctx* c, const orc_particle* particles, uint64_t h0, uint64_t h1, uint64_t n_total, uint64_t seed,
+                      int n_batches, double* edep, double* stats_out) {
+    if (!c || !c->have_tables) return 2;
+    if (!particles || n_batches < 1 || n_total >= (1ull << 32) || h1 > n_total || h0 > h1) return 1;
+    Beam B; B.particle = 0; B.shape = 0;
+    Stats st; std::memset(&st, 0, sizeof st);
+    Run run(*c, B, seed, st);
+    size_t nvox = c->mat.size();
+    for (uint64_t h = h0; h < h1; ++h) {
+        const orc_particle& q = particles[h];
+        if (q.E > c->p.e_max) return 3;
+        uint64_t bi = (h * (uint64_t)n_batches) / n_total;
+        run.edep = edep + bi * nvox;
+        double x[3] = {q.x, q.y, q.z}, d[3] = {q.u, q.v, q.w};
+        run.history_listed((uint32_t)h, q.particle == 0 ? 0 : (q.particle > 0 ? 1 : -1), x, d, q.E);
+    }
+    if (stats_out) std::memcpy(stats_out, &st, sizeof st);
+    return 0;
+}
 
 // Dose and batch uncertainty (R17, R18): D_b = E_b/(rho V N_b); mean over batches; standard error.
 int orc_finalize(const Ctx* c, const double* edep, uint64_t n_total, int n_batches, double* dose, double* sigma) {

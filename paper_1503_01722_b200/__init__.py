@@ -29,7 +29,7 @@ TABLE_IDS = {"mu_tot": 0, "mu_C": 1, "mu_pp": 2, "R": 3, "L": 4, "S_hard": 5, "S
 
 # every symbol include/mc.h declares (tests check that the library exports each of them)
 SYMBOLS = ["mc_create", "mc_destroy", "mc_build_tables", "mc_export_table", "mc_export_grid",
-           "mc_set_photon_tables", "mc_run", "mc_run_range", "mc_finalize", "mc_run_atten",
+           "mc_set_photon_tables", "mc_run", "mc_run_particles", "mc_run_range", "mc_finalize", "mc_run_atten",
            "mc_philox_selftest", "mc_bench_red", "mc_get_stats", "mc_set_stream", "mc_set_option",
            "mc_last_error", "mc_version"]
 
@@ -83,6 +83,7 @@ def lib():
         L.mc_export_grid.argtypes = [vp, vp]
         L.mc_set_photon_tables.argtypes = [vp, C.c_float, C.c_float, vp, vp, vp, vp]
         L.mc_run.argtypes = [vp, vp, u64, u64, i32, vp, vp]
+        L.mc_run_particles.argtypes = [vp, vp, u64, u64, i32, vp, vp]
         L.mc_run_range.argtypes = [vp, vp, u64, u64, u64, u64, i32, vp]
         L.mc_finalize.argtypes = [vp, vp, u64, i32, vp, vp]
         L.mc_run_atten.argtypes = [vp, vp, u64, u64, vp, vp]
@@ -201,6 +202,19 @@ def mc_run(ctx, beam, n_histories, seed, n_batches, dose_out, sigma_out):
     b, keep = _beam_struct(beam)
     _check(ctx, lib().mc_run(ctx, C.addressof(b), int(n_histories), int(seed), int(n_batches), _ptr(dose_out),
                              _ptr(sigma_out)))
+
+
+PARTICLE_DTYPE = np.dtype([("x", "f4"), ("y", "f4"), ("z", "f4"), ("u", "f4"), ("v", "f4"), ("w", "f4"), ("E", "f4"),
+                           ("particle", "i4")])  # = mc_particle
+
+
+def mc_run_particles(ctx, particles, seed, n_batches, dose_out, sigma_out, n=None):
+    """particles: numpy structured array of PARTICLE_DTYPE (host) or a CUDA uint8/float tensor holding n such records."""
+    if isinstance(particles, np.ndarray):
+        particles = np.ascontiguousarray(particles, PARTICLE_DTYPE)
+        n = len(particles)
+    _check(ctx, lib().mc_run_particles(ctx, _ptr(particles), int(n), int(seed), int(n_batches), _ptr(dose_out),
+                                       _ptr(sigma_out)))
 
 
 def mc_run_range(ctx, beam, n_histories, h_begin, h_end, seed, n_batches, edep_out):

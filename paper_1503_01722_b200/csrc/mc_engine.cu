@@ -205,8 +205,10 @@ namespace {
 
 // Launch scheduler (workflow Table 1): same-type launches; the queue holding at least one
 // full wave goes first, otherwise the group with the most particles (source included).
-mc_status transport(mc_ctx* ctx, const mc_beam* beam, uint64_t n_total, uint64_t h0, uint64_t h1, uint64_t seed,
-                    int n_batches, float* d_edep) {
+// Source: a beam (primaries sampled inside the transport kernels) or, with beam == nullptr, a device-resident
+// particle list whose entry h is history h (loaded into the queues a wave at a time).
+mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list, uint64_t n_total, uint64_t h0, uint64_t h1,
+                    uint64_t seed, int n_batches, float* d_edep) {
     mc_status st;
     if ((st = ensure_device(ctx)) != MC_OK) return st;
     if ((st = upload_tables(ctx)) != MC_OK) return st;
@@ -240,12 +242,12 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, uint64_t n_total, uint64_t
     RunParams P;
     memset(&P, 0, sizeof P);
     fill_params(ctx, P);
-    if ((st = upload_beam(ctx, beam, P.beam)) != MC_OK) return st;
+    if (beam && (st = upload_beam(ctx, beam, P.beam)) != MC_OK) return st;
     P.edep = d_edep; P.n_total = n_total; P.n_batches = n_batches;
     P.inv_n_total = n_total > 1 ? (unsigned long long)((((unsigned __int128)1) << 64) / n_total) : ~0ull;
     P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32);
 
-    const bool photon_beam = beam->particle == MC_PHOTON;
+    const bool photon_beam = beam && beam->particle == MC_PHOTON;
     uint64_t remaining = n_run, h_next = h0;
     uint32_t cnt_e[2] = {0, 0}, cnt_p = 0;
     int cur = 0;
@@ -255,15 +257,32 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, uint64_t n_total, uint64_t
     double m_new_e = 16.0, m_new_p = 16.0;  // secondaries queued per new primary (electron queue, photon queue)
     CU(cudaEventRecord(ctx->ev[0], s));
     while (remaining > 0 || cnt_e[cur] > 0 || cnt_p > 0) {
+        if (d_list && remaining > 0 && cnt_e[cur] < W && cnt_p < W) {
+            // particle-list source: the next wave of listed particles goes straight into the input queues
+            const uint32_t n_load = (uint32_t)std::min<uint64_t>(remaining, W);
+            P.h_first = h_next; P.n_in = 0; P.n_new = 0;
+            P.q_e_out = Queue{ctx->d_q[cur], ctx->d_counters + C_E_A + cur, ctx->q_cap};
+            P.q_p_out = Queue{ctx->d_q[2], ctx->d_counters + C_P, ctx->q_cap};
+            load_particles_kernel<<<std::min<uint32_t>((n_load + kThreads - 1) / kThreads, (uint32_t)ctx->sm_count * 8), kThreads, 0, s>>>(P, d_list, n_load);
+            CU(cudaGetLastError());
+            CU(cudaMemcpyAsync(ctx->h_counters, ctx->d_counters, C_COUNT * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+            CU(cudaStreamSynchronize(s));
+            ++S.n_kernel_launches;
+            if (ctx->h_counters[C_OVERFLOW]) return fail(ctx, MC_ERR_QUEUE_OVERFLOW, "particle queue overflow while loading the particle list");
+            cnt_e[cur] = ctx->h_counters[C_E_A + cur]; cnt_p = ctx->h_counters[C_P];
+            remaining -= n_load; h_next += n_load;
+            continue;
+        }
         bool run_p;
         if (cnt_p >= W) run_p = true;
         else if (cnt_e[cur] >= W) run_p = false;
         else {
-            uint64_t avail_e = cnt_e[cur] + (photon_beam ? 0 : remaining), avail_p = cnt_p + (photon_beam ? remaining : 0);
+            const uint64_t src = beam ? remaining : 0;  // a particle list feeds the queues, not the kernels
+            uint64_t avail_e = cnt_e[cur] + (photon_beam ? 0 : src), avail_p = cnt_p + (photon_beam ? src : 0);
             run_p = avail_p > avail_e;
         }
         uint32_t n_in = run_p ? cnt_p : cnt_e[cur], n_new = 0;
-        if (run_p == photon_beam && n_in < W) {
+        if (beam && run_p == photon_beam && n_in < W) {
             // new primaries admitted by this launch: up to a wave, and no more than the output queues can take at
             // the secondaries-per-primary ratio measured so far (first launch: a probe of cap / 16 histories)
             const double room_e = (double)ctx->q_cap - (run_p ? cnt_e[cur] : 0u) - (double)n_in;
@@ -489,7 +508,7 @@ mc_status mc_run_range(mc_ctx* ctx, const mc_beam* beam, uint64_t n_histories, u
     if ((st = ensure_device(ctx)) != MC_OK) return st;
     const size_t n = (size_t)n_batches * ctx->g.nvox;
     if ((st = ensure_edep(ctx, n)) != MC_OK) return st;
-    if ((st = transport(ctx, beam, n_histories, h_begin, h_end, seed, n_batches, ctx->d_edep)) != MC_OK) return st;
+    if ((st = transport(ctx, beam, nullptr, n_histories, h_begin, h_end, seed, n_batches, ctx->d_edep)) != MC_OK) return st;
     CU(cudaMemcpyAsync(edep_out, ctx->d_edep, n * sizeof(float), cudaMemcpyDefault, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     return MC_OK;
@@ -518,12 +537,56 @@ mc_status mc_run(mc_ctx* ctx, const mc_beam* beam, uint64_t n_histories, uint64_
     if ((st = ensure_device(ctx)) != MC_OK) return st;
     const size_t nvox = ctx->g.nvox;
     if ((st = ensure_edep(ctx, (size_t)n_batches * nvox)) != MC_OK) return st;
-    if ((st = transport(ctx, beam, n_histories, 0, n_histories, seed, n_batches, ctx->d_edep)) != MC_OK) return st;
+    if ((st = transport(ctx, beam, nullptr, n_histories, 0, n_histories, seed, n_batches, ctx->d_edep)) != MC_OK) return st;
     if ((st = finalize_device(ctx, ctx->d_edep, n_histories, n_batches)) != MC_OK) return st;
     CU(cudaMemcpyAsync(dose_out, ctx->d_dose, nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
     CU(cudaMemcpyAsync(sigma_out, ctx->d_sigma, nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     return MC_OK;
+}
+
+mc_status mc_run_particles(mc_ctx* ctx, const mc_particle* particles, uint64_t n, uint64_t seed, int32_t n_batches, float* dose_out,
+                           float* sigma_out) {
+    if (!ctx) return MC_ERR_INVALID_ARG;
+    if (!ctx->have_tables) return fail(ctx, MC_ERR_STATE, "mc_build_tables has not been called");
+    if (!particles || !dose_out || !sigma_out) return fail(ctx, MC_ERR_INVALID_ARG, "null pointer");
+    if (n == 0 || n >= (1ull << 32)) return fail(ctx, MC_ERR_INVALID_ARG, "n must be in [1, 2^32)");
+    if (n_batches < 2 || (uint64_t)n_batches > n) return fail(ctx, MC_ERR_INVALID_ARG, "n_batches must be in [2, n]");
+    if ((uint64_t)n_batches * (uint64_t)ctx->g.nvox >= (1ull << 32)) return fail(ctx, MC_ERR_INVALID_ARG, "n_batches * nvox must be < 2^32");
+    static_assert(sizeof(mc_particle) == sizeof(ListParticle), "mc_particle layout");
+    mc_status st;
+    if ((st = ensure_device(ctx)) != MC_OK) return st;
+    // the list may be host or device memory: a host list is staged on the device and checked against e_max
+    cudaPointerAttributes at;
+    const bool on_device = cudaPointerGetAttributes(&at, particles) == cudaSuccess && at.type == cudaMemoryTypeDevice;
+    cudaGetLastError();
+    const ListParticle* d_list = reinterpret_cast<const ListParticle*>(particles);
+    ListParticle* staged = nullptr;
+    if (!on_device) {
+        for (uint64_t i = 0; i < n; ++i) {
+            const mc_particle& q = particles[i];
+            if (!(q.E > 0.0f) || !std::isfinite(q.E)) return fail(ctx, MC_ERR_INVALID_ARG, "particle energies must be positive");
+            if (q.E > ctx->params.e_max_MeV) return fail(ctx, MC_ERR_ENERGY_RANGE, "particle energy above e_max_MeV");
+            const float nn = q.u * q.u + q.v * q.v + q.w * q.w;
+            if (!(std::fabs(nn - 1.0f) < 1e-3f)) return fail(ctx, MC_ERR_INVALID_ARG, "particle directions must be unit vectors");
+        }
+        CU(cudaMalloc(&staged, n * sizeof(ListParticle)));
+        cudaError_t e = cudaMemcpyAsync(staged, particles, n * sizeof(ListParticle), cudaMemcpyHostToDevice, ctx->stream);
+        if (e != cudaSuccess) { cudaFree(staged); return fail(ctx, MC_ERR_CUDA, cudaGetErrorString(e)); }
+        d_list = staged;
+    }
+    const size_t nvox = ctx->g.nvox;
+    st = ensure_edep(ctx, (size_t)n_batches * nvox);
+    if (st == MC_OK) st = transport(ctx, nullptr, d_list, n, 0, n, seed, n_batches, ctx->d_edep);
+    if (st == MC_OK) st = finalize_device(ctx, ctx->d_edep, n, n_batches);
+    if (st == MC_OK) {
+        cudaError_t e = cudaMemcpyAsync(dose_out, ctx->d_dose, nvox * sizeof(float), cudaMemcpyDefault, ctx->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(sigma_out, ctx->d_sigma, nvox * sizeof(float), cudaMemcpyDefault, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) st = fail(ctx, MC_ERR_CUDA, cudaGetErrorString(e));
+    } else cudaStreamSynchronize(ctx->stream);
+    if (staged) cudaFree(staged);
+    return st;
 }
 
 mc_status mc_run_atten(mc_ctx* ctx, const mc_beam* beam, uint64_t n, uint64_t seed, int32_t* voxel_out, uint8_t* channel_out) {

@@ -786,6 +786,41 @@ __global__ void __launch_bounds__(kThreads) atten_kernel(const __grid_constant__
 }
 
 // =================================================================================================
+// particle-list source ("phase-space file ... or a user CPU/GPU function"): histories
+// [h_first, h_first + n) are the listed particles themselves.  One thread per particle: locate the voxel (floor
+// rule, R25), book the source / escaped energy, push a queue record (track id (0,0)) to the queue of its type.
+// =================================================================================================
+struct ListParticle { float x, y, z, u, v, w, E; int32_t particle; };  // = mc_particle (include/mc.h)
+__global__ void __launch_bounds__(kThreads) load_particles_kernel(const __grid_constant__ RunParams P, const ListParticle* __restrict__ list,
+                                                                  uint32_t n) {
+    const Geometry& g = P.g;
+    double e_src = 0.0, e_esc = 0.0;
+    uint32_t n_hist = 0;
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const unsigned long long h = P.h_first + i;
+        const ListParticle p = list[h];
+        const uint32_t code = p.particle == 0 ? CODE_PHOTON : (p.particle > 0 ? CODE_POSITRON : CODE_ELECTRON);
+        const float e0 = p.E + (code == CODE_POSITRON ? 2.0f * kMeF : 0.0f);
+        e_src += (double)e0; ++n_hist;
+        float gx = __fmul_rn(__fsub_rn(p.x, g.ox), g.ihx), gy = __fmul_rn(__fsub_rn(p.y, g.oy), g.ihy), gz = __fmul_rn(__fsub_rn(p.z, g.oz), g.ihz);
+        const bool inside = gx >= 0.0f && gx < (float)g.nx && gy >= 0.0f && gy < (float)g.ny && gz >= 0.0f && gz < (float)g.nz;
+        if (!inside) { e_esc += (double)e0; continue; }
+        QRec r; r.x = p.x; r.y = p.y; r.z = p.z; r.u = p.u; r.v = p.v; r.w = p.w; r.E = p.E;
+        r.hist = (uint32_t)h; r.trk_lo = 0u; r.trk_hi = 0u;
+        r.vox = (int)gx + g.nx * ((int)gy + g.ny * (int)gz);
+        r.tag = (batch_of(h, P.n_batches, P.n_total, P.inv_n_total) << 2) | code;
+        push_record2(P.q_e_out, P.q_p_out, code != CODE_PHOTON, P.counters + C_OVERFLOW, r);
+    }
+    e_src = warp_sum(e_src); e_esc = warp_sum(e_esc);
+    unsigned long long nh = warp_sum(n_hist);
+    if ((threadIdx.x & 31) == 0) {
+        stat_add(P.stats, S_HIST, nh);
+        if (e_src != 0.0) atomicAdd(P.ledger + LG_SRC, e_src);
+        if (e_esc != 0.0) atomicAdd(P.ledger + LG_ESC, e_esc);
+    }
+}
+
+// =================================================================================================
 // batch statistics (S9; R17, R18): D_b = E_b / (rho V N_b), mean over batches, standard error of the mean
 // =================================================================================================
 __device__ __forceinline__ double batch_size(unsigned long long n_total, int B, int b) {

@@ -136,10 +136,53 @@ def photon_field():
     return beam(PHOTON, POINT_RECT, spectrum=spectrum_6mv())
 
 
+def paper_slab_phantom(half=False):
+    """The paper's phantoms: 32 cm cube at 0.25 cm voxels (128^3); slab = water 0-2 cm, bone 2-4 cm,
+    lung 4-6 cm, water below; half-slab = the bone and lung layers cover half of the xoy plane (x < 0)."""
+    n, h = 128, 0.25
+    mat = np.zeros((n, n, n), np.uint8)
+    rho = np.ones((n, n, n), np.float32)
+    zc = (np.arange(n) + 0.5) * h
+    xs = slice(0, n // 2) if half else slice(0, n)
+    for iz in range(n):
+        if 2.0 < zc[iz] < 4.0:
+            mat[iz, :, xs] = 1
+            rho[iz, :, xs] = 1.85
+        elif 4.0 < zc[iz] < 6.0:
+            mat[iz, :, xs] = 2
+            rho[iz, :, xs] = 0.26
+    return _phantom((n, n, n), (h, h, h), (-0.5 * n * h, -0.5 * n * h, 0.0), mat, rho)
+
+
+def paper_config(idx):
+    """The five cases of the paper's Tables 2 and 3 with this build's physics: 128^3 x 0.25 cm
+    phantoms, 2x2 cm^2 field at SSD 100 cm, 15 MeV electrons (5e6 histories) or the synthetic 6 MV spectrum (5e8),
+    absorption energies 200 keV (electrons) / 50 keV (photons).  Context beside the paper's timings, not a target.
+    idx: 1 e- water, 2 e- slab, 3 photon water, 4 photon slab, 5 photon half-slab."""
+    names = {1: "p1_15MeV_e_water128", 2: "p2_15MeV_e_slab128", 3: "p3_6MV_g_water128", 4: "p4_6MV_g_slab128",
+             5: "p5_6MV_g_halfslab128"}
+    if idx not in names:
+        raise ValueError("paper config index 1..5")
+    if idx in (1, 3):
+        ph = homogeneous_phantom((128, 128, 128), 0.25)
+    else:
+        ph = paper_slab_phantom(half=(idx == 5))
+    if idx <= 2:
+        bm, n = beam(ELECTRON, POINT_RECT, energy=15.0, field=(2.0, 2.0)), 5 * 10**6
+    else:
+        bm, n = beam(PHOTON, POINT_RECT, spectrum=spectrum_6mv(), field=(2.0, 2.0)), 5 * 10**8
+    return {"phantom": ph, "materials": materials(3), "params": params(e_cut=0.2, g_cut=0.05), "beam": bm,
+            "n_histories": n, "seed": 1, "n_batches": 10, "name": names[idx]}
+
+
 # --- the five BASELINE.json configs -------------------------------------------------------------
 def config(idx, beam_kind=None):
     """Return dict(phantom, materials, params, beam, n_histories, seed, n_batches, name).
-    idx 1..5 as in BASELINE.json `configs` (1-based); configs 4 and 5 take beam_kind 'e' or 'g'."""
+    idx 1..5 as in BASELINE.json `configs` (1-based); configs 4 and 5 take beam_kind 'e' or 'g'.
+    idx 'p1'..'p5': the paper-shaped cases of paper_config()."""
+    if isinstance(idx, str) and idx.startswith("p"):
+        return paper_config(int(idx[1:]))
+    idx = int(idx)
     if idx == 1:
         ph, bm, n, B, name = homogeneous_phantom((20, 20, 20), 0.5), electron_pencil(6.0), 10**5, 10, \
             "c1_6MeV_e_pencil_water20"
@@ -167,3 +210,35 @@ def config(idx, beam_kind=None):
         raise ValueError("config index 1..5")
     return {"phantom": ph, "materials": materials(3), "params": params(), "beam": bm,
             "n_histories": n, "seed": 1, "n_batches": B, "name": name}
+
+
+# --- particle-list ("phase-space") source ---------------------------------------------------------
+PARTICLE_DTYPE = np.dtype([("x", "f4"), ("y", "f4"), ("z", "f4"), ("u", "f4"), ("v", "f4"), ("w", "f4"), ("E", "f4"),
+                           ("particle", "i4")])  # layout of mc_particle (include/mc.h)
+
+
+def phase_space(n, seed=1, field=(6.0, 6.0), ssd=100.0, z=0.0, fractions=(0.90, 0.08, 0.02), e_max=6.0):
+    """Synthetic phase-space list in the plane z: a divergent 6 MV-like beam (PAPER.md:84 names phase-space files as a
+    source; none ships with the paper).  Photons with the triangular spectrum of config 3, contaminant electrons
+    (uniform 0.3..e_max MeV) and a few positrons; positions uniform over `field`, directions from a point at `ssd`
+    with a small Gaussian angular spread.  Input generation only (numpy RNG), no arithmetic of the method."""
+    rng = np.random.default_rng(seed)
+    p = np.zeros(n, PARTICLE_DTYPE)
+    kind = rng.choice(3, size=n, p=np.asarray(fractions) / np.sum(fractions))
+    p["particle"] = np.array([PHOTON, ELECTRON, POSITRON], np.int32)[kind]
+    x = (rng.random(n) - 0.5) * field[0]
+    y = (rng.random(n) - 0.5) * field[1]
+    d = np.stack([x + rng.normal(0, 0.5, n), y + rng.normal(0, 0.5, n), np.full(n, ssd)], axis=1)
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    p["x"], p["y"], p["z"] = x, y, z
+    d32 = d.astype(np.float32).astype(np.float64)
+    d32 /= np.linalg.norm(d32, axis=1, keepdims=True)
+    p["u"], p["v"], p["w"] = d32[:, 0], d32[:, 1], d32[:, 2]
+    # photon energies: triangular pdf 0.25 -> peak at 1.0 -> 0 at 6.0 (inverse CDF), others uniform
+    a, c, b = 0.25, 1.0, 6.0
+    u = rng.random(n)
+    fc = (c - a) / (b - a)
+    eg = np.where(u < fc, a + np.sqrt(u * (b - a) * (c - a)), b - np.sqrt((1 - u) * (b - a) * (b - c)))
+    ee = 0.3 + rng.random(n) * (e_max - 0.3)
+    p["E"] = np.where(kind == 0, eg, ee)
+    return p
