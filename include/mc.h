@@ -195,7 +195,9 @@ mc_status mc_set_stream(mc_ctx *ctx, void *cuda_stream);
  * name = "wave_size" (histories admitted per scheduling round), "queue_factor" (queue capacity in waves),
  * "blocks_per_sm", "refill_lanes" (idle lanes per warp that trigger a refill), "hard_lanes" (lanes per warp with a
  * pending hard event that trigger the Moller / bremsstrahlung block), "adaptive" (1: the number of new primaries a launch admits is limited by the room left in the
- * output queues at the measured secondaries-per-primary ratio; 0: always a full wave), "aggregate" (reserved).  Scheduling only:
+ * output queues at the measured secondaries-per-primary ratio; 0: always a full wave), "aggregate" (1: lanes of a warp that score into the same cell at the same
+ * moment combine into one red.global.add.f32; 0: one per lane; -1, default: 1 for beams entering through fewer than 16
+ * voxel columns, else 0).  Scheduling only:
  * per-history results do not depend on them (R14). */
 mc_status mc_set_option(mc_ctx *ctx, const char *name, int64_t value);
 const char *mc_last_error(const mc_ctx *ctx);

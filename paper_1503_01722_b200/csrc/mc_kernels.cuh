@@ -30,6 +30,20 @@ __device__ __forceinline__ void score_add(Score& s, float* edep, uint32_t idx, f
     s.acc += e;
 }
 
+// Warp-aggregated scoring (PAPER.md:74 scores with one atomic per deposit): the lanes that score at the same moment
+// are grouped by target cell (match.any); the lowest lane of each group sums the group's energies with shuffles and
+// issues ONE red.global.add.f32.  Returns true in the lane that issued it.  Narrow beams put many lanes of a warp on
+// the same few cells (config 1: a pencil beam), where the L2 serialises same-address reductions.
+__device__ __forceinline__ bool red_add_aggregated(float* edep, uint32_t cell, float e) {
+    const unsigned act = __activemask();
+    const unsigned grp = __match_any_sync(act, cell);
+    const int lane = threadIdx.x & 31, leader = __ffs(grp) - 1;
+    float sum = e;
+    for (unsigned m = grp & (grp - 1u); m; m &= m - 1u) sum += __shfl_sync(grp, e, __ffs(m) - 1);  // all but the leader
+    if (lane == leader) atomicAdd(edep + cell, sum);
+    return lane == leader;
+}
+
 // ---- geometry helpers --------------------------------------------------------------------------
 __device__ __forceinline__ float face_dist(const Geometry& g, float x, float y, float z, float u, float v, float w,
                                            int ix, int iy, int iz, int& ax) {
@@ -204,7 +218,11 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
     };
     auto bump = [&](int k) { s_cnt[k * kThreadsE + tid] += 1u; };
     auto flush = [&]() {  // one red.global.add.f32 per (track, voxel) visit (S6)
-        if (L.acc > 0.0f) { atomicAdd(P.edep + (size_t)(L.tag >> 2) * (uint32_t)g.nvox + (uint32_t)L.vox, L.acc); bump(SE_RED); }
+        if (L.acc > 0.0f) {
+            const uint32_t cell = (L.tag >> 2) * (uint32_t)g.nvox + (uint32_t)L.vox;  // n_batches * nvox < 2^32
+            if (P.aggregate) { if (red_add_aggregated(P.edep, cell, L.acc)) bump(SE_RED); }
+            else { atomicAdd(P.edep + cell, L.acc); bump(SE_RED); }
+        }
         L.acc = 0.0f;
     };
     auto emit_rec = [&](const Queue& q, const QRec& r, int stat) {
@@ -554,8 +572,9 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
 
     auto bump = [&](int k, uint32_t n) { s_cnt[k * kThreadsP + tid] += n; };
     auto deposit = [&](int vx, float e) {
-        atomicAdd(P.edep + ((tag >> 2) * (uint32_t)g.nvox + (uint32_t)vx), e);
-        bump(SP_RED, 1u);
+        const uint32_t cell = (tag >> 2) * (uint32_t)g.nvox + (uint32_t)vx;
+        if (P.aggregate) { if (red_add_aggregated(P.edep, cell, e)) bump(SP_RED, 1u); }
+        else { atomicAdd(P.edep + cell, e); bump(SP_RED, 1u); }
     };
     auto set_energy = [&]() {  // table coordinate and majorant of the current energy
         float t = fmaf(f_lg2(E), lg_a, -lg_b);

@@ -134,7 +134,7 @@ def _check(out):
         assert r["n"] > 0
     same, indep = out[1], out[2]
     assert same["mean_diff"] <= 0.01, same
-    if indep["noise"] < 1e-9:  # no randomness left (pencil beam without MS and hard events): sigma = 0 on both sides
+    if indep["noise"] < 1e-6:  # no randomness left (pencil beam without MS and hard events): sigma ~ fp32 rounding only
         assert indep["mean_diff"] <= 1e-3, indep
         return
     assert indep["frac3"] >= 0.99, indep
@@ -312,7 +312,8 @@ def test_scheduling_options_do_not_change_the_result():
     cfg = W.config(4, "e")
     n, B = 100000, 10
     ref = None
-    for opts in ({}, {"wave_size": 8192, "queue_factor": 16}, {"refill_lanes": 1}, {"refill_lanes": 32, "blocks_per_sm": 1}):
+    for opts in ({}, {"wave_size": 8192, "queue_factor": 16}, {"refill_lanes": 1}, {"refill_lanes": 32, "blocks_per_sm": 1},
+                 {"aggregate": 1}, {"aggregate": 0}, {"hard_lanes": 8, "refill_lanes": 48}):
         eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])
         for k, v in opts.items():
             mc.mc_set_option(eng.ctx, k, v)
