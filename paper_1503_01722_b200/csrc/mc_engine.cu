@@ -214,7 +214,7 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
     if ((st = upload_tables(ctx)) != MC_OK) return st;
     const size_t nvox = ctx->g.nvox;
     const size_t se = smem_e(ctx), sp = smem_p(ctx);
-    if (se > 200 * 1024 || sp > 200 * 1024) return fail(ctx, MC_ERR_INVALID_ARG, "tables do not fit in shared memory: lower n_grid");
+    if (se > 227 * 1024 || sp > 227 * 1024) return fail(ctx, MC_ERR_INVALID_ARG, "tables do not fit in shared memory: lower n_grid");
     CU(cudaFuncSetAttribute(electron_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)se));
     CU(cudaFuncSetAttribute(photon_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp));
     int occ_e = 0, occ_p = 0;

@@ -128,7 +128,7 @@ __device__ __forceinline__ void emit(const RunParams& P, const Queue& q, Score& 
 // While one track of a lane waits for the HARD block, the lane keeps stepping its other track, so the STEP block
 // runs with nearly all lanes and the rare blocks can wait for nearly full warps.
 // =================================================================================================
-constexpr int kThreadsE = 640;  // one CTA per SM: the tables are staged once per SM, 20 warps share them
+constexpr int kThreadsE = 768;  // one CTA per SM: the tables are staged once per SM, 24 warps share them
 constexpr int kSlots = 2;       // tracks per lane, parked in shared memory between the blocks that work on them
 constexpr float kHingeOverrun = 0.25f;  // DESIGN.md R8
 enum LaneState { L_IDLE = 0, L_STEP = 1, L_HARD = 2, L_DONE = 3 };
@@ -517,7 +517,7 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
 // kernel: per iteration a warp runs ONE of  FLY (lanes in L_STEP) / COMPTON (lanes in L_HARD, pending) /
 // REFILL (lanes in L_IDLE), the rare blocks only when enough lanes want them.
 // =================================================================================================
-constexpr int kThreadsP = 640;  // one CTA per SM
+constexpr int kThreadsP = 768;  // one CTA per SM
 constexpr int kSlotsP = 3;     // tracks per lane in the warp's pool (shared memory)
 constexpr int kTrackWordsP = 13;
 enum { SP_FLIGHT = 0, SP_FICT, SP_COMPTON, SP_PAIR, SP_PE, SP_SEC_E, SP_HIST, SP_RED, SP_COUNT };
