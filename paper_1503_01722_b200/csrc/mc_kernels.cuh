@@ -517,7 +517,7 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
 // kernel: per iteration a warp runs ONE of  FLY (lanes in L_STEP) / COMPTON (lanes in L_HARD, pending) /
 // REFILL (lanes in L_IDLE), the rare blocks only when enough lanes want them.
 // =================================================================================================
-constexpr int kThreadsP = 768;  // one CTA per SM
+constexpr int kThreadsP = 896;  // one CTA per SM
 constexpr int kSlotsP = 3;     // tracks per lane in the warp's pool (shared memory)
 constexpr int kTrackWordsP = 13;
 enum { SP_FLIGHT = 0, SP_FICT, SP_COMPTON, SP_PAIR, SP_PE, SP_SEC_E, SP_HIST, SP_RED, SP_COUNT };
