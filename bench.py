@@ -311,7 +311,7 @@ def run_engine(args):
                 "unit": "Tinstr/s (thread-instructions)", "frac": achieved / issue_peak,
                 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of that kernel (a wave of primaries) from the
                 # committed ncu --set full capture, profiles/r1b_*_kernel_ncu_full.txt: queue records, not a bound
-                "traffic": {"electron_kernel": 436.7e6, "photon_kernel": 159.9e6}[dom], "traffic_unit": "bytes per launch (ncu capture, profiles/)",
+                "traffic": {"electron_kernel": 435.8e6, "photon_kernel": 160.7e6}[dom], "traffic_unit": "bytes per launch (ncu capture, profiles/)",
                 "peak_source": f"148 SM x 4 schedulers x 32 lanes x sm_max_mhz ({pk_kind} MEASURED_PEAKS.json clock)",
                 "kernel_ms_per_step": kms / K, "kernel_share_of_step": kms / total_ms if world == 1 else None}
     # scoring roofline: measured red.global.add.f32 peak into a window the size of one batch grid
