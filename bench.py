@@ -184,9 +184,16 @@ def run_engine(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the engine has no CPU path)")
+    # one rank per GPU; MC_BENCH_BACKEND=gloo lets the N > 1 code path be exercised on a box with fewer GPUs than
+    # ranks (ranks then share devices and the grids are reduced through the host) — a functional check, not a benchmark
+    backend = os.environ.get("MC_BENCH_BACKEND", "nccl")
+    local = local % torch.cuda.device_count()
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group(backend)
     cfg = workload(args)
     n, B, seed = cfg["n_histories"], cfg["n_batches"], cfg["seed"]
     from paper_1503_01722_b200 import sharding
