@@ -125,13 +125,32 @@ mc_status upload_tables(mc_ctx* ctx) {
     return MC_OK;
 }
 
-size_t smem_e(const mc_ctx* c) {  // tables + per-thread counters + per-thread energy ledger + parked tracks
-    return (size_t)c->tabs.n_mat * TE_COUNT * c->tabs.N * sizeof(float2) + (size_t)SE_COUNT * kThreadsE * sizeof(uint32_t) +
-           2 * (size_t)kThreadsE * sizeof(double) + (size_t)(kTrackWords * kSlots + kSlots + 1) * kThreadsE * sizeof(uint32_t);
+// shared memory of a transport CTA of T threads: tables + per-thread counters + per-thread energy ledger + track pool
+size_t smem_e(const mc_ctx* c, int T) {
+    return (size_t)c->tabs.n_mat * TE_COUNT * c->tabs.N * sizeof(float2) + (size_t)SE_COUNT * T * sizeof(uint32_t) +
+           2 * (size_t)T * sizeof(double) + (size_t)(kTrackWords * kSlots + kSlots + 1) * T * sizeof(uint32_t);
 }
-size_t smem_p(const mc_ctx* c) {
-    return (size_t)(1 + c->tabs.n_mat * TP_COUNT) * c->tabs.N * sizeof(float2) + (size_t)SP_COUNT * kThreadsP * sizeof(uint32_t) + 2 * (size_t)kThreadsP * sizeof(double) +
-           (size_t)(kTrackWordsP * kSlotsP + kSlotsP + 1) * kThreadsP * sizeof(uint32_t);
+size_t smem_p(const mc_ctx* c, int T) {
+    return (size_t)(1 + c->tabs.n_mat * TP_COUNT) * c->tabs.N * sizeof(float2) + (size_t)SP_COUNT * T * sizeof(uint32_t) +
+           2 * (size_t)T * sizeof(double) + (size_t)(kTrackWordsP * kSlotsP + kSlotsP + 1) * T * sizeof(uint32_t);
+}
+constexpr size_t kSmemMax = 227 * 1024;  // opt-in dynamic shared memory per CTA on sm_100
+using TransportKernel = void (*)(const RunParams);
+struct KernelChoice { TransportKernel fn; int threads; size_t smem; };
+// the largest CTA whose tables + pools fit (more materials or a finer grid leave less room for the pools)
+bool choose_electron_kernel(const mc_ctx* c, KernelChoice& k) {
+    const int T[3] = {768, 512, 256};
+    const TransportKernel fn[3] = {electron_kernel<768>, electron_kernel<512>, electron_kernel<256>};
+    for (int i = 0; i < 3; ++i)
+        if (smem_e(c, T[i]) <= kSmemMax) { k = KernelChoice{fn[i], T[i], smem_e(c, T[i])}; return true; }
+    return false;
+}
+bool choose_photon_kernel(const mc_ctx* c, KernelChoice& k) {
+    const int T[3] = {896, 768, 512};
+    const TransportKernel fn[3] = {photon_kernel<896>, photon_kernel<768>, photon_kernel<512>};
+    for (int i = 0; i < 3; ++i)
+        if (smem_p(c, T[i]) <= kSmemMax) { k = KernelChoice{fn[i], T[i], smem_p(c, T[i])}; return true; }
+    return false;
 }
 
 mc_status check_beam(mc_ctx* ctx, const mc_beam* b) {
@@ -213,13 +232,15 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
     if ((st = ensure_device(ctx)) != MC_OK) return st;
     if ((st = upload_tables(ctx)) != MC_OK) return st;
     const size_t nvox = ctx->g.nvox;
-    const size_t se = smem_e(ctx), sp = smem_p(ctx);
-    if (se > 227 * 1024 || sp > 227 * 1024) return fail(ctx, MC_ERR_INVALID_ARG, "tables do not fit in shared memory: lower n_grid");
-    CU(cudaFuncSetAttribute(electron_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)se));
-    CU(cudaFuncSetAttribute(photon_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp));
+    KernelChoice ke, kp;
+    if (!choose_electron_kernel(ctx, ke) || !choose_photon_kernel(ctx, kp))
+        return fail(ctx, MC_ERR_INVALID_ARG, "tables do not fit in shared memory: lower n_grid (n_mats * n_grid is too large)");
+    const size_t se = ke.smem, sp = kp.smem;
+    CU(cudaFuncSetAttribute(ke.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)se));
+    CU(cudaFuncSetAttribute(kp.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp));
     int occ_e = 0, occ_p = 0;
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_e, electron_kernel, kThreadsE, se));
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, photon_kernel, kThreadsP, sp));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_e, ke.fn, ke.threads, se));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, kp.fn, kp.threads, sp));
     if (occ_e < 1 || occ_p < 1) return fail(ctx, MC_ERR_CUDA, "kernel does not fit on an SM");
     if (ctx->blocks_per_sm > 0) { occ_e = std::min<int>(occ_e, (int)ctx->blocks_per_sm); occ_p = std::min<int>(occ_p, (int)ctx->blocks_per_sm); }
 
@@ -304,16 +325,16 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
         Queue qe_oth{ctx->d_q[1 - cur], ctx->d_counters + C_E_A + (1 - cur), ctx->q_cap};
         Queue qp{ctx->d_q[2], ctx->d_counters + C_P, ctx->q_cap};
         const uint64_t items = (uint64_t)n_in + n_new;
-        const int occ = run_p ? occ_p : occ_e, thr = run_p ? kThreadsP : kThreadsE;
+        const int occ = run_p ? occ_p : occ_e, thr = run_p ? kp.threads : ke.threads;
         int grid = (int)std::min<uint64_t>((uint64_t)ctx->sm_count * occ, (items + thr - 1) / thr);
         grid = std::max(grid, 1);
         CU(cudaEventRecord(ctx->ev[2], s));
         if (run_p) {
             P.q_in = qp; P.q_e_out = qe_cur; P.q_p_out = qp;
-            photon_kernel<<<grid, kThreadsP, sp, s>>>(P);
+            kp.fn<<<grid, kp.threads, sp, s>>>(P);
         } else {
             P.q_in = qe_cur; P.q_e_out = qe_oth; P.q_p_out = qp;
-            electron_kernel<<<grid, kThreadsE, se, s>>>(P);
+            ke.fn<<<grid, ke.threads, se, s>>>(P);
         }
         CU(cudaGetLastError());
         CU(cudaEventRecord(ctx->ev[3], s));

@@ -128,7 +128,8 @@ __device__ __forceinline__ void emit(const RunParams& P, const Queue& q, Score& 
 // While one track of a lane waits for the HARD block, the lane keeps stepping its other track, so the STEP block
 // runs with nearly all lanes and the rare blocks can wait for nearly full warps.
 // =================================================================================================
-constexpr int kThreadsE = 768;  // one CTA per SM: the tables are staged once per SM, 24 warps share them
+// One CTA per SM (the tables are staged once per SM).  kThreadsE = CTA size: 768 (24 warps) when tables + pools fit in
+// the 227 KB of shared memory, else 512 or 256 (more materials / finer grids); instantiated in mc_engine.cu.
 constexpr int kSlots = 2;       // tracks per lane, parked in shared memory between the blocks that work on them
 constexpr float kHingeOverrun = 0.25f;  // DESIGN.md R8
 enum LaneState { L_IDLE = 0, L_STEP = 1, L_HARD = 2, L_DONE = 3 };
@@ -154,6 +155,7 @@ struct ELane {
     Rng rng;
 };
 
+template <int kThreadsE>
 __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_constant__ RunParams P) {
     extern __shared__ float2 s_tab[];
     const int ntab = P.n_mat * TE_COUNT * P.N;
@@ -517,11 +519,12 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
 // kernel: per iteration a warp runs ONE of  FLY (lanes in L_STEP) / COMPTON (lanes in L_HARD, pending) /
 // REFILL (lanes in L_IDLE), the rare blocks only when enough lanes want them.
 // =================================================================================================
-constexpr int kThreadsP = 896;  // one CTA per SM
+// kThreadsP = CTA size of the photon kernel: 896 (28 warps), 768 or 512 by what fits (one CTA per SM)
 constexpr int kSlotsP = 3;     // tracks per lane in the warp's pool (shared memory)
 constexpr int kTrackWordsP = 13;
 enum { SP_FLIGHT = 0, SP_FICT, SP_COMPTON, SP_PAIR, SP_PE, SP_SEC_E, SP_HIST, SP_RED, SP_COUNT };
 
+template <int kThreadsP>
 __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_constant__ RunParams P) {
     extern __shared__ float2 s_tab[];
     const int ntab = (1 + P.n_mat * TP_COUNT) * P.N;

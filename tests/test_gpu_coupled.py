@@ -326,3 +326,27 @@ def test_scheduling_options_do_not_change_the_result():
             assert key == ref[1], opts
             assert np.allclose(d, ref[0], rtol=1e-4, atol=1e-6 * ref[0].max()), opts
         eng.close()
+
+
+def test_more_materials_pick_a_smaller_cta_and_give_the_same_histories():
+    """8 materials x 256 nodes leave less shared memory for the track pools: the engine falls back to smaller CTAs
+    (DESIGN.md "Kernels").  Materials the phantom does not use change nothing: same counters, same dose."""
+    cfg = W.config(4, "e")
+    n, B = 200000, 10
+    mats8 = W.materials(3) + [W.water(), W.bone(), W.lung(), W.water(), W.bone()]
+    res = []
+    for mats in (cfg["materials"], mats8):
+        eng = mc.Engine(cfg["phantom"], mats, cfg["params"])
+        d, _ = eng.run(cfg["beam"], n, 6, B)
+        st = eng.stats()
+        assert _ledger(st) < 1e-4
+        res.append((d, (st["n_electron_steps"], st["n_photon_flights"], st["n_moller"], st["n_brems"], st["n_compton"])))
+        eng.close()
+    assert res[0][1] == res[1][1]
+    assert np.allclose(res[0][0], res[1][0], rtol=1e-4, atol=1e-6 * res[0][0].max())
+    # beyond what any CTA size can hold: a clear error, not a crash
+    eng = mc.Engine(cfg["phantom"], mats8, W.params(n_grid=1024))
+    with pytest.raises(mc.McError) as e:
+        eng.run(cfg["beam"], 1000, 1, 2)
+    assert e.value.status == mc.MC_ERR_INVALID_ARG and "shared memory" in str(e.value)
+    eng.close()
