@@ -43,6 +43,7 @@ def test_struct_layouts_match_the_header():
     assert C.sizeof(mc._Material) == 40
     assert C.sizeof(mc._Beam) == 64
     assert C.sizeof(mc._Stats) == 13 * 8 + 6 * 8
+    assert mc.PARTICLE_DTYPE.itemsize == 32 and W.PARTICLE_DTYPE == mc.PARTICLE_DTYPE  # mc_particle
 
 
 def test_create_rejects_bad_arguments():
@@ -195,4 +196,23 @@ def test_set_photon_tables_round_trip():
     got = mc.mc_export_photon_tables(eng.ctx, 3)
     for k in ("mu_maj", "mu_tot", "mu_C", "mu_pp"):
         assert np.array_equal(got[k], t2[k])
+    eng.close()
+
+
+def test_run_particles_argument_validation_before_any_device_work():
+    import numpy as np
+    ph = W.homogeneous_phantom((4, 4, 4), 0.5)
+    eng = mc.Engine(ph)
+    p = W.phase_space(16, seed=1, field=(1.0, 1.0))
+    d, s = np.zeros(64, np.float32), np.zeros(64, np.float32)
+    with pytest.raises(mc.McError) as e:  # tables first
+        mc.mc_run_particles(eng.ctx, p, 1, 2, d, s)
+    assert e.value.status == mc.MC_ERR_STATE
+    mc.mc_build_tables(eng.ctx, W.materials(1), W.params())
+    with pytest.raises(mc.McError) as e:  # n_batches > n
+        mc.mc_run_particles(eng.ctx, p, 1, 17, d, s)
+    assert e.value.status == mc.MC_ERR_INVALID_ARG
+    with pytest.raises(mc.McError) as e:  # n_batches < 2
+        mc.mc_run_particles(eng.ctx, p, 1, 1, d, s)
+    assert e.value.status == mc.MC_ERR_INVALID_ARG
     eng.close()
