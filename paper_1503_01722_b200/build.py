@@ -22,7 +22,7 @@ def build(force=False, verbose=False):
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(s) for s in DEPS):
         return LIB
     cmd = [NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-           "-prec-div=false", "-prec-sqrt=false", "-Xcompiler", "-fPIC,-O2,-Wall", "-shared", "-cudart", "shared", "-o", LIB] + SRC
+           "-prec-div=false", "-prec-sqrt=false", "-Xcompiler", "-fPIC,-O2,-Wall,-pthread", "-shared", "-cudart", "shared", "-o", LIB] + SRC
     if verbose:
         cmd[1:1] = ["-Xptxas", "-v"]
     subprocess.check_call(cmd)

@@ -7,6 +7,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <thread>
 
 namespace mcb {
 namespace {
@@ -173,6 +174,18 @@ double k1_transport(const Mat& m, double T) {
     return kNa * 2 * kPi * kRe * kRe * s / (gam * gam * beta2 * beta2);
 }
 
+// fn(i) for i in [0, n) on a few host threads (the nodes of a table are independent; the build is part of the
+// end-to-end time of a fresh context)
+template <class F> void parallel_for(int n, F fn) {
+    int nt = (int)std::min<unsigned>(std::max(1u, std::thread::hardware_concurrency()), 8u);
+    nt = std::min(nt, std::max(1, n / 8));
+    if (nt <= 1) { for (int i = 0; i < n; ++i) fn(i); return; }
+    std::vector<std::thread> th;
+    for (int t = 0; t < nt; ++t)
+        th.emplace_back([=]() { for (int i = t; i < n; i += nt) fn(i); });
+    for (auto& x : th) x.join();
+}
+
 }  // namespace
 
 std::string build_tables(const std::vector<MaterialSpec>& specs, const TableParams& p,
@@ -207,28 +220,28 @@ std::string build_tables(const std::vector<MaterialSpec>& specs, const TablePara
         Mat m = prepare(specs[mi]);
         out.lscr.push_back((float)m.l_scr);
         auto L = [&](double T) { return l_col(m, T, p.e_cut) + l_rad(m, T, p.g_cut); };
-        std::vector<double> range(N, 0.0);
-        double run_max = 0;
-        for (int j = 0; j < N; ++j) {
+        std::vector<double> range(N, 0.0), s_hard(N, 0.0), segv(N, 0.0);
+        parallel_for(N, [&](int j) {
             double k = E[j] / kMe, pe = 0, pp = 0;
             for (const auto& e : m.el) { pe += e.w / e.A * pe_atom(e.Z, k); pp += e.w / e.A * pair_atom(e.Z, k); }
             double muC = m.n_el * kn_total(k), muP = kNa * pp;
             mu_tot[mi][j] = muC + muP + kNa * pe;
             double sM = m.n_el * moller_total(E[j], p.e_cut);
-            double sH = sM + brems_total(m, E[j], p.g_cut);
-            run_max = std::max(run_max, sH);
+            s_hard[j] = sM + brems_total(m, E[j], p.g_cut);
             out.t[T_MU_TOT][mi][j] = (float)mu_tot[mi][j];
             out.t[T_MU_C][mi][j] = (float)muC;
             out.t[T_MU_PP][mi][j] = (float)muP;
             out.t[T_L][mi][j] = (float)L(E[j]);
             out.t[T_S_MOLLER][mi][j] = (float)sM;
-            out.t[T_S_HARD][mi][j] = (float)sH;
-            out.t[T_S_MAX][mi][j] = (float)run_max;
+            out.t[T_S_HARD][mi][j] = (float)s_hard[j];
             out.t[T_K1][mi][j] = (float)k1_transport(m, E[j]);
-        }
-        auto seg = [&](int j) { return integrate([&](double lt) { double T = std::exp(lt); return T / L(T); }, std::log(E[j]), std::log(E[j + 1]), 1); };
-        for (int j = out.k_cut; j + 1 < N; ++j) range[j + 1] = range[j] + seg(j);
-        for (int j = out.k_cut - 1; j >= 0; --j) range[j] = range[j + 1] - seg(j);
+            // range integral over the segment [node j, node j + 1]
+            if (j + 1 < N) segv[j] = integrate([&](double lt) { double T = std::exp(lt); return T / L(T); }, std::log(E[j]), std::log(E[j + 1]), 1);
+        });
+        double run_max = 0;
+        for (int j = 0; j < N; ++j) { run_max = std::max(run_max, s_hard[j]); out.t[T_S_MAX][mi][j] = (float)run_max; }
+        for (int j = out.k_cut; j + 1 < N; ++j) range[j + 1] = range[j] + segv[j];
+        for (int j = out.k_cut - 1; j >= 0; --j) range[j] = range[j + 1] - segv[j];
         for (int j = 0; j < N; ++j) out.t[T_RANGE][mi][j] = (float)range[j];
         // fp32 rounding must not break the dominance Sigma_max >= Sigma_hard nor monotonicity of R
         for (int j = 0; j < N; ++j) {
