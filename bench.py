@@ -307,6 +307,7 @@ def run_engine(args):
     # ---- rooflines (rank 0's kernels) ----------------------------------------------------------------------
     pk, pk_kind = peaks()
     issue_peak = SM_COUNT * SCHEDULERS_PER_SM * LANES * pk["sm_max_mhz"] * 1e6  # thread-instructions / s
+    issue_measured = max(mc.mc_bench_issue(eng.ctx, 4096) for _ in range(3))  # FFMA micro-benchmark on this GPU
     e_ms, p_ms = acc["electron_kernel_ms"], acc["photon_kernel_ms"]
     alg_e = acc["n_electron_steps"] * INSTR_PER["e_step"] + (acc["n_moller"] + acc["n_brems"]) * INSTR_PER["hard_event"]
     alg_p = acc["n_photon_flights"] * INSTR_PER["photon_flight"] + \
@@ -320,6 +321,8 @@ def run_engine(args):
                 # committed ncu --set full capture, profiles/r1b_*_kernel_ncu_full.txt: queue records, not a bound
                 "traffic": {"electron_kernel": 435.8e6, "photon_kernel": 160.7e6}[dom], "traffic_unit": "bytes per launch (ncu capture, profiles/)",
                 "peak_source": f"148 SM x 4 schedulers x 32 lanes x sm_max_mhz ({pk_kind} MEASURED_PEAKS.json clock)",
+                "peak_measured": issue_measured / 1e12, "frac_of_measured": achieved / issue_measured,
+                "peak_measured_source": "mc_bench_issue: 2 x 1024-thread CTAs per SM, 8 independent FFMA chains per thread, best of 3",
                 "kernel_ms_per_step": kms / K, "kernel_share_of_step": kms / total_ms if world == 1 else None}
     # scoring roofline: measured red.global.add.f32 peak into a window the size of one batch grid
     red_ms = min(mc.mc_bench_red(eng.ctx, nvox, 64, 0, SM_COUNT * 8) for _ in range(3))

@@ -188,6 +188,10 @@ mc_status mc_philox_selftest(const uint32_t *ctr, const uint32_t *key, int32_t n
 mc_status mc_bench_red(mc_ctx *ctx, uint32_t n_cells, int32_t per_thread, int32_t mode, int32_t blocks,
                        double *ms_out);
 
+/* mc_bench_issue — measures the transport roofline's denominator: 2 x 1024-thread CTAs per SM each run iters x 64
+ * independent FFMAs per thread; *thread_instr_per_s (host) = FFMA thread-instructions per second achieved. */
+mc_status mc_bench_issue(mc_ctx *ctx, int32_t iters, double *thread_instr_per_s);
+
 mc_status mc_get_stats(const mc_ctx *ctx, mc_stats *out);
 /* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); 0 = default stream. */
 mc_status mc_set_stream(mc_ctx *ctx, void *cuda_stream);

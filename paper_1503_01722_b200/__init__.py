@@ -30,7 +30,7 @@ TABLE_IDS = {"mu_tot": 0, "mu_C": 1, "mu_pp": 2, "R": 3, "L": 4, "S_hard": 5, "S
 # every symbol include/mc.h declares (tests check that the library exports each of them)
 SYMBOLS = ["mc_create", "mc_destroy", "mc_build_tables", "mc_export_table", "mc_export_grid",
            "mc_set_photon_tables", "mc_run", "mc_run_particles", "mc_run_range", "mc_finalize", "mc_run_atten",
-           "mc_philox_selftest", "mc_bench_red", "mc_get_stats", "mc_set_stream", "mc_set_option",
+           "mc_philox_selftest", "mc_bench_red", "mc_bench_issue", "mc_get_stats", "mc_set_stream", "mc_set_option",
            "mc_last_error", "mc_version"]
 
 
@@ -89,6 +89,7 @@ def lib():
         L.mc_run_atten.argtypes = [vp, vp, u64, u64, vp, vp]
         L.mc_philox_selftest.argtypes = [vp, vp, i32, vp]
         L.mc_bench_red.argtypes = [vp, u32, i32, i32, i32, vp]
+        L.mc_bench_issue.argtypes = [vp, i32, vp]
         L.mc_get_stats.argtypes = [vp, vp]
         L.mc_set_stream.argtypes = [vp, vp]
         L.mc_set_option.argtypes = [vp, C.c_char_p, C.c_int64]
@@ -244,6 +245,12 @@ def mc_bench_red(ctx, n_cells, per_thread, mode, blocks):
     ms = C.c_double()
     _check(ctx, lib().mc_bench_red(ctx, int(n_cells), int(per_thread), int(mode), int(blocks), C.addressof(ms)))
     return ms.value
+
+
+def mc_bench_issue(ctx, iters=4096):
+    r = C.c_double()
+    _check(ctx, lib().mc_bench_issue(ctx, int(iters), C.addressof(r)))
+    return r.value
 
 
 def mc_get_stats(ctx):

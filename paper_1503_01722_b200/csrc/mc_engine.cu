@@ -686,6 +686,23 @@ mc_status mc_bench_red(mc_ctx* ctx, uint32_t n_cells, int32_t per_thread, int32_
     return MC_OK;
 }
 
+mc_status mc_bench_issue(mc_ctx* ctx, int32_t iters, double* thread_instr_per_s) {
+    if (!ctx || !thread_instr_per_s || iters <= 0) return MC_ERR_INVALID_ARG;
+    mc_status st;
+    if ((st = ensure_device(ctx)) != MC_OK) return st;
+    const int blocks = ctx->sm_count * 2;
+    issue_bench_kernel<<<blocks, 1024, 0, ctx->stream>>>(ctx->d_dose, 16);  // warm-up
+    cudaEventRecord(ctx->ev[2], ctx->stream);
+    issue_bench_kernel<<<blocks, 1024, 0, ctx->stream>>>(ctx->d_dose, iters);
+    cudaEventRecord(ctx->ev[3], ctx->stream);
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    float ms = 0;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, ctx->ev[2], ctx->ev[3]);
+    if (e != cudaSuccess || !(ms > 0)) return fail(ctx, MC_ERR_CUDA, std::string("mc_bench_issue: ") + cudaGetErrorString(e));
+    *thread_instr_per_s = (double)blocks * 1024.0 * (double)iters * 64.0 / (ms * 1e-3);
+    return MC_OK;
+}
+
 mc_status mc_get_stats(const mc_ctx* ctx, mc_stats* out) {
     if (!ctx || !out) return MC_ERR_INVALID_ARG;
     *out = ctx->stats;

@@ -902,4 +902,20 @@ __global__ void __launch_bounds__(kThreads) red_bench_kernel(float* grid, uint32
     }
 }
 
+// Issue-rate micro-benchmark (transport roofline): 8 independent FFMA chains per thread,
+// `iters` x 64 FFMA each; 1024 threads per CTA keep every scheduler supplied.  Reports thread-instructions / s.
+__global__ void __launch_bounds__(1024) issue_bench_kernel(float* out, int iters) {
+    float a0 = threadIdx.x * 1e-3f, a1 = a0 + 1.f, a2 = a0 + 2.f, a3 = a0 + 3.f, a4 = a0 + 4.f, a5 = a0 + 5.f, a6 = a0 + 6.f, a7 = a0 + 7.f;
+    const float m = 0.999f, c = 1e-3f;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            a0 = fmaf(a0, m, c); a1 = fmaf(a1, m, c); a2 = fmaf(a2, m, c); a3 = fmaf(a3, m, c);
+            a4 = fmaf(a4, m, c); a5 = fmaf(a5, m, c); a6 = fmaf(a6, m, c); a7 = fmaf(a7, m, c);
+        }
+    }
+    float r = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+    if (r == 123456.f) out[0] = r;  // never true: keeps the chains alive
+}
+
 }  // namespace mcb
