@@ -210,16 +210,47 @@ def run_engine(args):
     edep = torch.empty(B * nvox, dtype=torch.float32, device="cuda") if world > 1 else None
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
 
-    def step():
+    # N > 1: the one exchange of the sharded job (sum of the ranks' per-batch grids).
+    #   peer      (default) every rank leaves its grids in its context's buffer, maps the other ranks' buffers once
+    #             through CUDA IPC and reads them in place in mc_finalize_multi (over NVLink): no all-reduce, no copy
+    #   allreduce NCCL all-reduce of the grids, then mc_finalize (also the fallback if the peers cannot be mapped)
+    exchange, peers = "single GPU", None
+    if world > 1:
+        exchange = os.environ.get("MC_BENCH_EXCHANGE", "peer")
+        if exchange == "peer":
+            ok = 1
+            try:
+                own = mc.mc_edep_buffer(eng.ctx, B)
+                handles = [None] * world
+                dist.all_gather_object(handles, mc.mc_ipc_get_handle(own))
+                peers = [own if r == rank else mc.mc_ipc_open_handle(handles[r]) for r in range(world)]
+            except Exception as exc:  # noqa: BLE001  (any failure -> every rank falls back together)
+                print(f"rank {rank}: peer mapping failed ({exc}); falling back to all-reduce", file=sys.stderr)
+                ok = 0
+            flag = torch.tensor([ok], device="cuda" if backend == "nccl" else "cpu")
+            dist.all_reduce(flag, op=dist.ReduceOp.MIN)
+            if int(flag.item()) == 0:
+                exchange, peers = "allreduce (peer mapping failed)", None
+
+    def step(dose_out=None, sigma_out=None, e=None):
+        e = e or eng
+        d_out, s_out = (dose, sigma) if dose_out is None else (dose_out, sigma_out)
         if world == 1:
-            mc.mc_run(eng.ctx, cfg["beam"], n, seed, B, dose, sigma)
-        else:  # shard = contiguous history range; one exchange: sum of the per-batch grids
+            mc.mc_run(e.ctx, cfg["beam"], n, seed, B, d_out, s_out)
+        elif peers is not None and e is eng:
+            mc.mc_run_range(e.ctx, cfg["beam"], n_job, h_lo, h_hi, seed, B, peers[rank])  # shard stays in place
+            st = mc.mc_get_stats(e.ctx)
+            dist.barrier()                                   # every rank's grids are complete
+            mc.mc_finalize_multi(e.ctx, peers, n_job, B, d_out, s_out)
+            dist.barrier()                                   # nobody overwrites its grids while a peer still reads
+            return st
+        else:
             def run_range(nj, a, b):
-                mc.mc_run_range(eng.ctx, cfg["beam"], nj, a, b, seed, B, edep)
+                mc.mc_run_range(e.ctx, cfg["beam"], nj, a, b, seed, B, edep)
                 return edep
             sharding.run_sharded(rank, world, n, run_range, dist.all_reduce,
-                                 lambda g, nj: mc.mc_finalize(eng.ctx, g, nj, B, dose, sigma))
-        return mc.mc_get_stats(eng.ctx)
+                                 lambda g, nj: mc.mc_finalize(e.ctx, g, nj, B, d_out, s_out))
+        return mc.mc_get_stats(e.ctx)
 
     def sync_all():
         torch.cuda.synchronize()
@@ -259,14 +290,7 @@ def run_engine(args):
         ph = cfg["phantom"]
 
         def host_step(e):
-            if world == 1:
-                mc.mc_run(e.ctx, cfg["beam"], n, seed, B, h_dose, h_sigma)
-            else:
-                def run_range(nj, a, b):
-                    mc.mc_run_range(e.ctx, cfg["beam"], nj, a, b, seed, B, edep)
-                    return edep
-                sharding.run_sharded(rank, world, n, run_range, dist.all_reduce,
-                                     lambda g, nj: mc.mc_finalize(e.ctx, g, nj, B, h_dose, h_sigma))
+            step(h_dose, h_sigma, e)
 
         def timed(fn, reps):
             fn()
@@ -338,7 +362,7 @@ def run_engine(args):
                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
                "data": "synthetic",
                "config": config_dict(cfg, args, {"l2": "256 MiB fill between timed steps (L2 flush)",
-                                                 "parallelism": f"history ranges x{world}, all-reduce of batch grids" if world > 1 else "single GPU"}),
+                                                 "parallelism": f"history ranges x{world}, exchange: {exchange}" if world > 1 else "single GPU"}),
                "e_steps_per_s": acc["n_electron_steps"] * world / (total_ms * 1e-3),
                "photon_flights_per_s": acc["n_photon_flights"] * world / (total_ms * 1e-3),
                "per_history": {"e_steps": acc["n_electron_steps"] / (n * K), "photon_flights": acc["n_photon_flights"] / (n * K),
@@ -358,6 +382,11 @@ def run_engine(args):
         if world == 1 and not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(cfg)
         print(json.dumps(out))
+    if peers is not None:
+        dist.barrier()
+        for r in range(world):
+            if r != rank:
+                mc.mc_ipc_close_handle(peers[r])
     eng.close()
     if world > 1:
         dist.destroy_process_group()

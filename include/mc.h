@@ -170,6 +170,24 @@ mc_status mc_run_range(mc_ctx *ctx, const mc_beam *beam, uint64_t n_histories, u
 mc_status mc_finalize(mc_ctx *ctx, const float *edep, uint64_t n_histories, int32_t n_batches,
                       float *dose_out, float *sigma_out);
 
+/* Fused exchange + statistics for the sharded job: instead of summing the ranks' grids with an
+ * all-reduce and then calling mc_finalize, every rank (or one) reads all grids in place, over NVLink for a peer's.
+ *   mc_edep_buffer     the context's own [n_batches][nvox] grid buffer (device memory, plain cudaMalloc: exportable);
+ *                      pass it as edep_out of mc_run_range to leave the shard's grids there without a copy.
+ *   mc_ipc_get_handle  CUDA IPC handle (64 bytes) of a device buffer, to be sent to the other ranks by any means.
+ *   mc_ipc_open_handle maps another process's buffer into this one (peer access is enabled as needed);
+ *   mc_ipc_close_handle unmaps it.
+ *   mc_finalize_multi  dose and sigma of the SUM of n_grids (1..16) grids: edep_grids[r] = device-accessible pointer to
+ *                      n_batches*nvox floats (own, or opened with mc_ipc_open_handle); edep_grids itself is a HOST array.
+ * The caller orders the calls across ranks (all shards finished before any rank finalizes; nobody reuses its buffer
+ * before all have finalized), e.g. with torch.distributed.barrier(). */
+mc_status mc_edep_buffer(mc_ctx *ctx, int32_t n_batches, float **out);
+mc_status mc_finalize_multi(mc_ctx *ctx, const float *const *edep_grids, int32_t n_grids, uint64_t n_histories,
+                            int32_t n_batches, float *dose_out, float *sigma_out);
+mc_status mc_ipc_get_handle(const void *dev_ptr, uint8_t handle[64]);
+mc_status mc_ipc_open_handle(const uint8_t handle[64], void **dev_ptr);
+mc_status mc_ipc_close_handle(void *dev_ptr);
+
 /* mc_run_atten — attenuation-only mode (R20): photon primaries only; per history the
  * linear voxel index of the first real interaction (-1 = left the phantom or never interacted) and its
  * channel (0 Compton, 1 pair, 2 photoelectric, 255 none).  fp32 arithmetic contract: bit-exact

@@ -29,7 +29,8 @@ TABLE_IDS = {"mu_tot": 0, "mu_C": 1, "mu_pp": 2, "R": 3, "L": 4, "S_hard": 5, "S
 
 # every symbol include/mc.h declares (tests check that the library exports each of them)
 SYMBOLS = ["mc_create", "mc_destroy", "mc_build_tables", "mc_export_table", "mc_export_grid",
-           "mc_set_photon_tables", "mc_run", "mc_run_particles", "mc_run_range", "mc_finalize", "mc_run_atten",
+           "mc_set_photon_tables", "mc_run", "mc_run_particles", "mc_run_range", "mc_finalize", "mc_edep_buffer",
+           "mc_finalize_multi", "mc_ipc_get_handle", "mc_ipc_open_handle", "mc_ipc_close_handle", "mc_run_atten",
            "mc_philox_selftest", "mc_bench_red", "mc_bench_issue", "mc_get_stats", "mc_set_stream", "mc_set_option",
            "mc_last_error", "mc_version"]
 
@@ -86,6 +87,11 @@ def lib():
         L.mc_run_particles.argtypes = [vp, vp, u64, u64, i32, vp, vp]
         L.mc_run_range.argtypes = [vp, vp, u64, u64, u64, u64, i32, vp]
         L.mc_finalize.argtypes = [vp, vp, u64, i32, vp, vp]
+        L.mc_edep_buffer.argtypes = [vp, i32, C.POINTER(vp)]
+        L.mc_finalize_multi.argtypes = [vp, vp, i32, u64, i32, vp, vp]
+        L.mc_ipc_get_handle.argtypes = [vp, vp]
+        L.mc_ipc_open_handle.argtypes = [vp, C.POINTER(vp)]
+        L.mc_ipc_close_handle.argtypes = [vp]
         L.mc_run_atten.argtypes = [vp, vp, u64, u64, vp, vp]
         L.mc_philox_selftest.argtypes = [vp, vp, i32, vp]
         L.mc_bench_red.argtypes = [vp, u32, i32, i32, i32, vp]
@@ -110,6 +116,8 @@ def _ptr(buf):
     """Raw address of a numpy array or a torch tensor (host or CUDA)."""
     if buf is None:
         return None
+    if isinstance(buf, int):
+        return buf
     if isinstance(buf, np.ndarray):
         assert buf.flags["C_CONTIGUOUS"]
         return buf.ctypes.data
@@ -226,6 +234,38 @@ def mc_run_range(ctx, beam, n_histories, h_begin, h_end, seed, n_batches, edep_o
 
 def mc_finalize(ctx, edep, n_histories, n_batches, dose_out, sigma_out):
     _check(ctx, lib().mc_finalize(ctx, _ptr(edep), int(n_histories), int(n_batches), _ptr(dose_out), _ptr(sigma_out)))
+
+
+def mc_edep_buffer(ctx, n_batches):
+    """Device address (int) of the context's own [n_batches][nvox] grid buffer."""
+    p = C.c_void_p()
+    _check(ctx, lib().mc_edep_buffer(ctx, int(n_batches), C.byref(p)))
+    return p.value
+
+
+def mc_finalize_multi(ctx, grids, n_histories, n_batches, dose_out, sigma_out):
+    """grids: device addresses (ints) or CUDA tensors, one [n_batches][nvox] grid per rank."""
+    addr = [g if isinstance(g, int) else _ptr(g) for g in grids]
+    arr = (C.c_void_p * len(addr))(*addr)
+    _check(ctx, lib().mc_finalize_multi(ctx, C.addressof(arr), len(addr), int(n_histories), int(n_batches), _ptr(dose_out),
+                                        _ptr(sigma_out)))
+
+
+def mc_ipc_get_handle(dev_ptr):
+    h = (C.c_uint8 * 64)()
+    _check(None, lib().mc_ipc_get_handle(C.c_void_p(int(dev_ptr)), C.addressof(h)))
+    return bytes(h)
+
+
+def mc_ipc_open_handle(handle):
+    h = (C.c_uint8 * 64).from_buffer_copy(handle)
+    p = C.c_void_p()
+    _check(None, lib().mc_ipc_open_handle(C.addressof(h), C.byref(p)))
+    return p.value
+
+
+def mc_ipc_close_handle(dev_ptr):
+    _check(None, lib().mc_ipc_close_handle(C.c_void_p(int(dev_ptr))))
 
 
 def mc_run_atten(ctx, beam, n, seed, voxel_out, channel_out=None):

@@ -551,7 +551,7 @@ mc_status mc_run_range(mc_ctx* ctx, const mc_beam* beam, uint64_t n_histories, u
     const size_t n = (size_t)n_batches * ctx->g.nvox;
     if ((st = ensure_edep(ctx, n)) != MC_OK) return st;
     if ((st = transport(ctx, beam, nullptr, n_histories, h_begin, h_end, seed, n_batches, ctx->d_edep)) != MC_OK) return st;
-    CU(cudaMemcpyAsync(edep_out, ctx->d_edep, n * sizeof(float), cudaMemcpyDefault, ctx->stream));
+    if (edep_out != ctx->d_edep) CU(cudaMemcpyAsync(edep_out, ctx->d_edep, n * sizeof(float), cudaMemcpyDefault, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     return MC_OK;
 }
@@ -568,6 +568,60 @@ mc_status mc_finalize(mc_ctx* ctx, const float* edep, uint64_t n_histories, int3
     CU(cudaMemcpyAsync(dose_out, ctx->d_dose, nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
     CU(cudaMemcpyAsync(sigma_out, ctx->d_sigma, nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
+    return MC_OK;
+}
+
+mc_status mc_edep_buffer(mc_ctx* ctx, int32_t n_batches, float** out) {
+    if (!ctx || !out || n_batches < 1) return MC_ERR_INVALID_ARG;
+    mc_status st;
+    if ((st = ensure_device(ctx)) != MC_OK) return st;
+    if ((st = ensure_edep(ctx, (size_t)n_batches * ctx->g.nvox)) != MC_OK) return st;
+    *out = ctx->d_edep;
+    return MC_OK;
+}
+
+mc_status mc_finalize_multi(mc_ctx* ctx, const float* const* edep_grids, int32_t n_grids, uint64_t n_histories, int32_t n_batches,
+                            float* dose_out, float* sigma_out) {
+    if (!ctx) return MC_ERR_INVALID_ARG;
+    if (!edep_grids || n_grids < 1 || n_grids > kMaxGrids || !dose_out || !sigma_out || n_batches < 2 || n_histories < (uint64_t)n_batches)
+        return fail(ctx, MC_ERR_INVALID_ARG, "mc_finalize_multi arguments (1 <= n_grids <= 16)");
+    mc_status st;
+    if ((st = ensure_device(ctx)) != MC_OK) return st;
+    GridList gl;
+    gl.n = n_grids;
+    for (int r = 0; r < kMaxGrids; ++r) gl.g[r] = r < n_grids ? edep_grids[r] : nullptr;
+    for (int r = 0; r < n_grids; ++r) if (!gl.g[r]) return fail(ctx, MC_ERR_INVALID_ARG, "mc_finalize_multi: null grid");
+    const int nvox = ctx->g.nvox;
+    const double vol = (double)ctx->g.hx * (double)ctx->g.hy * (double)ctx->g.hz;
+    const int grid = std::min(ctx->sm_count * 8, (nvox + kThreads - 1) / kThreads);
+    finalize_multi_kernel<<<grid, kThreads, n_batches * sizeof(double), ctx->stream>>>(gl, ctx->d_vox, nvox, n_batches, n_histories, vol,
+                                                                                       ctx->d_dose, ctx->d_sigma);
+    CU(cudaGetLastError());
+    ++ctx->stats.n_kernel_launches;
+    CU(cudaMemcpyAsync(dose_out, ctx->d_dose, (size_t)nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
+    CU(cudaMemcpyAsync(sigma_out, ctx->d_sigma, (size_t)nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return MC_OK;
+}
+
+mc_status mc_ipc_get_handle(const void* dev_ptr, uint8_t handle[64]) {
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "cudaIpcMemHandle_t is 64 bytes");
+    if (!dev_ptr || !handle) return MC_ERR_INVALID_ARG;
+    cudaIpcMemHandle_t h;
+    if (cudaIpcGetMemHandle(&h, const_cast<void*>(dev_ptr)) != cudaSuccess) { cudaGetLastError(); return MC_ERR_CUDA; }
+    memcpy(handle, &h, 64);
+    return MC_OK;
+}
+mc_status mc_ipc_open_handle(const uint8_t handle[64], void** dev_ptr) {
+    if (!handle || !dev_ptr) return MC_ERR_INVALID_ARG;
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle, 64);
+    if (cudaIpcOpenMemHandle(dev_ptr, h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) { cudaGetLastError(); return MC_ERR_CUDA; }
+    return MC_OK;
+}
+mc_status mc_ipc_close_handle(void* dev_ptr) {
+    if (!dev_ptr) return MC_ERR_INVALID_ARG;
+    if (cudaIpcCloseMemHandle(dev_ptr) != cudaSuccess) { cudaGetLastError(); return MC_ERR_CUDA; }
     return MC_OK;
 }
 

@@ -867,6 +867,33 @@ __global__ void __launch_bounds__(kThreads) finalize_kernel(const float* __restr
     }
 }
 
+// Fused exchange + statistics for the sharded job: the per-batch energy of a
+// voxel is the SUM over the ranks' grids, read in place — grids[r] may be this device's memory or a peer's, mapped
+// through CUDA IPC / peer access, in which case the loads travel over NVLink.  One pass: no all-reduce, no summed copy.
+constexpr int kMaxGrids = 16;
+struct GridList { const float* g[kMaxGrids]; int n; };
+__global__ void __launch_bounds__(kThreads) finalize_multi_kernel(const __grid_constant__ GridList grids, const uint2* __restrict__ vox,
+                                                                  int nvox, int B, unsigned long long n_total, double voxel_volume,
+                                                                  float* __restrict__ dose, float* __restrict__ sigma) {
+    extern __shared__ double s_inv_nb[];
+    for (int b = threadIdx.x; b < B; b += blockDim.x) s_inv_nb[b] = 1.0 / batch_size(n_total, B, b);
+    __syncthreads();
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < nvox; i += gridDim.x * blockDim.x) {
+        const double inv_mass = 1.0 / ((double)__uint_as_float(vox[i].x) * voxel_volume);
+        double mean = 0.0, sq = 0.0;
+        for (int b = 0; b < B; ++b) {
+            double e = 0.0;
+            for (int r = 0; r < grids.n; ++r) e += (double)__ldg(grids.g[r] + (size_t)b * nvox + i);
+            const double d = e * inv_mass * s_inv_nb[b];
+            mean += d; sq += d * d;
+        }
+        mean /= B;
+        const double ss = fmax(sq - (double)B * mean * mean, 0.0);  // sum of squared deviations from the mean
+        dose[i] = (float)mean;
+        sigma[i] = B > 1 ? (float)sqrt(ss / ((double)B * (B - 1))) : 0.0f;
+    }
+}
+
 // total of a float array in fp64 (energy ledger: deposited energy = sum of the batch grids)
 __global__ void __launch_bounds__(kThreads) sum_kernel(const float* __restrict__ a, size_t n, double* out) {
     double s = 0.0;
