@@ -213,14 +213,19 @@ mc_status mc_bench_issue(mc_ctx *ctx, int32_t iters, double *thread_instr_per_s)
 mc_status mc_get_stats(const mc_ctx *ctx, mc_stats *out);
 /* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); 0 = default stream. */
 mc_status mc_set_stream(mc_ctx *ctx, void *cuda_stream);
-/* Tuning knobs ("the number of workitems M ... manually adjusted"):
- * name = "wave_size" (histories admitted per scheduling round), "queue_factor" (queue capacity in waves),
- * "blocks_per_sm", "refill_lanes" (idle lanes per warp that trigger a refill), "hard_lanes" (lanes per warp with a
- * pending hard event that trigger the Moller / bremsstrahlung block), "adaptive" (1: the number of new primaries a launch admits is limited by the room left in the
- * output queues at the measured secondaries-per-primary ratio; 0: always a full wave), "aggregate" (1: lanes of a warp that score into the same cell at the same
- * moment combine into one red.global.add.f32; 0: one per lane; -1, default: 1 for beams entering through fewer than 16
- * voxel columns, else 0).  Scheduling only:
- * per-history results do not depend on them (R14). */
+/* Tuning knobs ("the number of workitems M ... manually adjusted").  Scheduling only: per-history results
+ * do not depend on them (R14).
+ *   "wave_size"     histories admitted per launch at most (default 2^24)
+ *   "queue_factor"  capacity of each particle queue in waves (default 4)
+ *   "adaptive"      1 (default): the number of new primaries a launch admits is limited by the room left in the output
+ *                   queues at the measured secondaries-per-primary ratio; 0: always a full wave
+ *   "hard_lanes"    tracks of a warp's pool that must wait for the hard-event / Compton block before the warp runs it
+ *                   (default 32 = a full warp; the block also runs when it has more tracks than the step block)
+ *   "refill_lanes"  empty slots of a warp's pool that trigger a refill from the queue / the source (default 32)
+ *   "blocks_per_sm" cap on the CTAs per SM (0 = as many as fit; the transport kernels use one)
+ *   "aggregate"     1: lanes of a warp that score into the same cell at the same moment combine into one
+ *                   red.global.add.f32; 0: one per lane; -1 (default): 1 for beams entering through fewer than 16
+ *                   voxel columns, else 0 */
 mc_status mc_set_option(mc_ctx *ctx, const char *name, int64_t value);
 const char *mc_last_error(const mc_ctx *ctx);
 const char *mc_version(void);
