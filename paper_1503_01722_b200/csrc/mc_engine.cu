@@ -45,6 +45,8 @@ struct mc_ctx {
     // options (M "manually adjusted")
     int64_t wave_size = 1 << 24, queue_factor = 4, blocks_per_sm = 0, refill_lanes = 32, aggregate = -1, hard_lanes = 32, adaptive = 1;
     mc_stats stats{};
+    // secondaries-per-primary ratios measured by the last run, reused when the next run has the same kind of beam
+    double beam_key = -1.0, last_m_e = 16.0, last_m_p = 16.0;
     std::string err;
 };
 
@@ -296,7 +298,10 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
     mc_stats& S = ctx->stats;
     S = mc_stats{};
     double ms_e = 0, ms_p = 0;
-    double m_new_e = 16.0, m_new_p = 16.0;  // secondaries queued per new primary (electron queue, photon queue)
+    // secondaries queued per new primary (electron queue, photon queue): measured while running; the first launch of a
+    // context is a probe (16 assumed), later runs with the same kind of beam start from the last measurement
+    const double key = beam ? (double)beam->particle * 1e3 + (double)beam->E_nodes_MeV[beam->n_nodes - 1] : -2.0;
+    double m_new_e = key == ctx->beam_key ? ctx->last_m_e : 16.0, m_new_p = key == ctx->beam_key ? ctx->last_m_p : 16.0;
     CU(cudaEventRecord(ctx->ev[0], s));
     while (remaining > 0 || cnt_e[cur] > 0 || cnt_p > 0) {
         if (d_list && remaining > 0 && cnt_e[cur] < W && cnt_p < W) {
@@ -369,6 +374,7 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
             const double n_items = (double)n_in + n_new;
             m_new_e = std::max(0.05, 1.5 * out_e / n_items);
             m_new_p = std::max(0.05, 1.5 * out_p / n_items);
+            ctx->beam_key = key; ctx->last_m_e = m_new_e; ctx->last_m_p = m_new_p;
         }
         if (run_p) { cnt_p = 0; cnt_e[cur] = ctx->h_counters[C_E_A + cur]; }
         else { cnt_e[cur] = 0; cur = 1 - cur; cnt_e[cur] = ctx->h_counters[C_E_A + cur]; cnt_p = ctx->h_counters[C_P]; }
