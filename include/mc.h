@@ -122,7 +122,8 @@ void mc_destroy(mc_ctx *ctx);
 
 /* mc_build_tables — closed-form physics tables per material on a uniform ln E grid, the photon
  * Woodcock majorant from the phantom.  Re-callable.
- * Errors: a voxel's material index >= n_mats, bad cut-offs / grid -> MC_ERR_INVALID_ARG. */
+ * n_mats: 1..16 (tables and track pools share the 227 KB of shared memory: 3 materials x 256 nodes run on the largest CTAs,
+ * 16 materials need n_grid <= 128).  Errors: a voxel's material index >= n_mats, bad cut-offs / grid -> MC_ERR_INVALID_ARG. */
 mc_status mc_build_tables(mc_ctx *ctx, const mc_material *mats, int32_t n_mats, const mc_params *params);
 
 /* Table access, fp32 as used on the device.  which: 0 mu_tot 1 mu_C 2 mu_pp (cm^2/g) 3 R (g/cm^2)

@@ -10,7 +10,7 @@
 
 namespace mcb {
 
-constexpr int MAX_MAT = 8;
+constexpr int MAX_MAT = 16;  // the paper's database holds 16 materials
 constexpr float kMeF = 0.51099895f;
 constexpr float kTwoPiF = 6.28318530717958647692f;
 

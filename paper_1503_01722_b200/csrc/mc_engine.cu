@@ -478,7 +478,7 @@ void mc_destroy(mc_ctx* ctx) {
 
 mc_status mc_build_tables(mc_ctx* ctx, const mc_material* mats, int32_t n_mats, const mc_params* params) {
     if (!ctx) return MC_ERR_INVALID_ARG;
-    if (!mats || !params || n_mats <= 0 || n_mats > MAX_MAT) return fail(ctx, MC_ERR_INVALID_ARG, "materials / params (n_mats must be 1..8)");
+    if (!mats || !params || n_mats <= 0 || n_mats > MAX_MAT) return fail(ctx, MC_ERR_INVALID_ARG, "materials / params (n_mats must be 1..16)");
     if (!(params->d_maxs_cm > 0) || !(params->f_maxe > 0) || !(params->f_maxe <= 1)) return fail(ctx, MC_ERR_INVALID_ARG, "d_maxs_cm must be > 0 and f_maxe in (0, 1]");
     std::vector<double> rho_max(n_mats, 0.0);
     for (size_t i = 0; i < ctx->h_mat.size(); ++i) {

@@ -344,6 +344,12 @@ def test_more_materials_pick_a_smaller_cta_and_give_the_same_histories():
         eng.close()
     assert res[0][1] == res[1][1]
     assert np.allclose(res[0][0], res[1][0], rtol=1e-4, atol=1e-6 * res[0][0].max())
+    # 16 materials (the size of the paper's database) on a 128-node grid
+    mats16 = mats8 + mats8
+    eng = mc.Engine(cfg["phantom"], mats16, W.params(n_grid=128))
+    d16, _ = eng.run(cfg["beam"], n, 6, B)
+    assert _ledger(eng.stats()) < 1e-4 and abs(d16.sum() / res[0][0].sum() - 1.0) < 0.01
+    eng.close()
     # beyond what any CTA size can hold: a clear error, not a crash
     eng = mc.Engine(cfg["phantom"], mats8, W.params(n_grid=1024))
     with pytest.raises(mc.McError) as e:
