@@ -8,6 +8,7 @@
 // asymptote; restricted-L identity L_col + int W dsigma_M = S_col and ESTAR-like water values;
 // Moller / brems totals vs independent quadrature; chi-square of the KN, Moller, brems samplers;
 // exp(-mu x) attenuation; CSDA range; per-history energy ledger; MS mean cosine.
+// Sources: beams (R13) and particle lists (R13b, orc_run_particles).  Hinge vs voxel face: reading R8 (HINGE_OVERRUN).
 // Coupled dose: "parity unpinned" by any external number (no dose value in the paper is
 // reproducible here: gDPM, XCOM data and the 6 MV spectrum are missing) — DESIGN.md says so.
 #include "orc_physics.h"
