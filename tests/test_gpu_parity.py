@@ -130,3 +130,17 @@ def test_user_supplied_photon_tables_drive_the_attenuation_mode():
     ovox, och, _ = orc.run_atten(bm, n, 5, tabs)
     assert np.array_equal(vox, ovox) and np.array_equal(ch, och)
     eng.close()
+
+
+def test_roofline_micro_benchmarks_report_plausible_peaks():
+    """mc_bench_issue / mc_bench_red are the measured denominators of bench.py's two rooflines."""
+    ph = W.homogeneous_phantom((8, 8, 8), 0.5)
+    eng = mc.Engine(ph, W.materials(1), W.params())
+    issue = max(mc.mc_bench_issue(eng.ctx, 2048) for _ in range(2))
+    assert 1.5e13 < issue < 4.5e13          # thread-instructions / s; nominal 148 x 4 x 32 x 1.965 GHz = 3.7e13
+    ms = min(mc.mc_bench_red(eng.ctx, 223260, 64, 0, 148 * 8) for _ in range(2))
+    rate = 148 * 8 * 256 * 64 / (ms * 1e-3)
+    assert 2e10 < rate < 1e12               # reds / s into a window the size of one batch grid
+    ms_hot = mc.mc_bench_red(eng.ctx, 223260, 64, 1, 148 * 8)
+    assert ms_hot > 0
+    eng.close()
