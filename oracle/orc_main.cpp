@@ -302,13 +302,16 @@ struct Run {
             st.n_compton += 1;
             double k0 = p.E / MEC2, e0 = 1.0 / (1.0 + 2.0 * k0), a1 = std::log(1.0 / e0), a2 = 0.5 * (1.0 - e0 * e0);
             double eps, tt;
-            for (;;) {
-                s.next();
-                if (s.u(0) * (a1 + a2) < a1) eps = std::exp(-a1 * s.u(1));
-                else eps = std::sqrt(e0 * e0 + (1.0 - e0 * e0) * s.u(1));
+            // two trials per Philox block (words 0,1 then 2,3), as for Moller and bremsstrahlung (R15): the first word
+            // picks the branch of the epsilon decomposition AND, rescaled to (0,1) inside the branch, samples it
+            for (int k = 2;; ++k) {
+                if (k == 2) { s.next(); k = 0; }
+                double r = s.u(2 * k) * (a1 + a2);
+                if (r < a1) eps = std::exp(-r);  // = e0^(r/a1)
+                else eps = std::sqrt(e0 * e0 + (1.0 - e0 * e0) * (r - a1) / a2);
                 tt = (1.0 - eps) / (k0 * eps);
                 double sin2 = tt * (2.0 - tt);
-                if (s.u(2) <= 1.0 - eps * sin2 / (1.0 + eps * eps)) break;
+                if (s.u(2 * k + 1) <= 1.0 - eps * sin2 / (1.0 + eps * eps)) break;
             }
             s.next();
             double phi = 2.0 * PI * s.u(2), cost = 1.0 - tt;
@@ -713,11 +716,12 @@ void orc_sample_kn(double E, uint64_t n, uint64_t seed, double* out) {
     for (uint64_t i = 0; i < n; ++i) {
         Stream s; s.h = (uint32_t)i; s.seed_lo = (uint32_t)seed; s.seed_hi = (uint32_t)(seed >> 32); s.trk_lo = s.trk_hi = 0; s.block = 0;
         double k0 = E / MEC2, e0 = 1.0 / (1.0 + 2.0 * k0), a1 = std::log(1.0 / e0), a2 = 0.5 * (1.0 - e0 * e0), eps, tt;
-        for (;;) {
-            s.next();
-            if (s.u(0) * (a1 + a2) < a1) eps = std::exp(-a1 * s.u(1)); else eps = std::sqrt(e0 * e0 + (1.0 - e0 * e0) * s.u(1));
+        for (int k = 2;; ++k) {
+            if (k == 2) { s.next(); k = 0; }
+            double r = s.u(2 * k) * (a1 + a2);
+            if (r < a1) eps = std::exp(-r); else eps = std::sqrt(e0 * e0 + (1.0 - e0 * e0) * (r - a1) / a2);
             tt = (1.0 - eps) / (k0 * eps);
-            if (s.u(2) <= 1.0 - eps * tt * (2.0 - tt) / (1.0 + eps * eps)) break;
+            if (s.u(2 * k + 1) <= 1.0 - eps * tt * (2.0 - tt) / (1.0 + eps * eps)) break;
         }
         s.next();
         double d0[3] = {0.6, 0.0, 0.8}, d1[3] = {0.6, 0.0, 0.8};

@@ -656,16 +656,21 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
                 load_slot(slot);
                 bump(SP_COMPTON, 1u);
                 const float k0 = E * (1.0f / kMeF), e0 = f_rcp(1.0f + 2.0f * k0), e02 = e0 * e0;
-                const float a1l2 = -f_lg2(e0), a1 = a1l2 * kLn2F, a2 = 0.5f * (1.0f - e02), ik0 = f_rcp(k0);
+                const float a1 = -f_lg2(e0) * kLn2F, a2 = 0.5f * (1.0f - e02), ik0 = f_rcp(k0);
                 float eps, tt;
+                const float ia2 = f_rcp(a2);
+                // one trial from two words: the first picks the branch and, rescaled inside it, samples epsilon (R15)
+                auto trial = [&](uint32_t wa, uint32_t wb) {
+                    const float r = u01f(wa) * (a1 + a2);
+                    eps = r < a1 ? f_ex2(-r * kLog2eF) : f_sqrt(fmaf((1.0f - e02) * ia2, r - a1, e02));
+                    tt = (1.0f - eps) * f_rcp(eps) * ik0;
+                    const float sin2 = tt * (2.0f - tt);
+                    return u01f(wb) <= 1.0f - eps * sin2 * f_rcp(1.0f + eps * eps);
+                };
                 for (;;) {
                     uint4 c4 = next_block(rng, P.seed_lo, P.seed_hi);
-                    float u1 = u01f(c4.y);
-                    if (u01f(c4.x) * (a1 + a2) < a1) eps = f_ex2(-a1l2 * u1);
-                    else eps = f_sqrt(fmaf(1.0f - e02, u1, e02));
-                    tt = (1.0f - eps) * f_rcp(eps) * ik0;
-                    float sin2 = tt * (2.0f - tt);
-                    if (u01f(c4.z) <= 1.0f - eps * sin2 * f_rcp(1.0f + eps * eps)) break;
+                    if (trial(c4.x, c4.y)) break;
+                    if (trial(c4.z, c4.w)) break;
                 }
                 uint4 d4 = next_block(rng, P.seed_lo, P.seed_hi);
                 const float E1 = eps * E, Te = E - E1;
