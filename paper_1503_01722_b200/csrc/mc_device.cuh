@@ -225,6 +225,10 @@ __device__ __forceinline__ void rotate_fast(float& u, float& v, float& w, float 
 
 // ---- source (R13), arithmetic contract ----------------------------------------------------------
 struct Primary { float x, y, z, u, v, w, E; bool inside; int ix, iy, iz; };
+// kExact = true: the fp32 arithmetic contract (IEEE-rounded division and square root), used by the attenuation-only mode
+// where the result must be bit-exact; kExact = false: the same formulas with single MUFU reciprocal / rsqrt for the
+// transport kernels (the primary then differs from the contract's in the last bits only).
+template <bool kExact = true>
 __device__ __forceinline__ Primary sample_primary(const RunParams& P, uint4 w4) {
     const BeamDev& b = P.beam;
     Primary p;
@@ -240,7 +244,9 @@ __device__ __forceinline__ Primary sample_primary(const RunParams& P, uint4 w4) 
         }
         float p0 = b.pdf_nodes[j], p1 = b.pdf_nodes[j + 1];
         float q = __fmaf_rn(u1, __fsub_rn(__fmul_rn(p1, p1), __fmul_rn(p0, p0)), __fmul_rn(p0, p0));
-        float t = __fdiv_rn(__fmul_rn(u1, __fadd_rn(p0, p1)), __fadd_rn(p0, __fsqrt_rn(q)));
+        float t;
+        if (kExact) t = __fdiv_rn(__fmul_rn(u1, __fadd_rn(p0, p1)), __fadd_rn(p0, __fsqrt_rn(q)));
+        else t = u1 * (p0 + p1) * f_rcp(p0 + f_sqrt(q));
         p.E = __fmaf_rn(t, __fsub_rn(b.E_nodes[j + 1], b.E_nodes[j]), b.E_nodes[j]);
     }
     if (b.shape == 0) {
@@ -249,8 +255,14 @@ __device__ __forceinline__ Primary sample_primary(const RunParams& P, uint4 w4) 
         float fx = __fmul_rn(__fsub_rn(u01(w4.z), 0.5f), b.fx), fy = __fmul_rn(__fsub_rn(u01(w4.w), 0.5f), b.fy);
         p.x = __fadd_rn(b.ex, fx); p.y = __fadd_rn(b.ey, fy); p.z = b.ez;
         float n2 = __fmaf_rn(fx, fx, __fmaf_rn(fy, fy, __fmul_rn(b.ssd, b.ssd)));
-        float nr = __fsqrt_rn(n2);
-        p.u = __fdiv_rn(fx, nr); p.v = __fdiv_rn(fy, nr); p.w = __fdiv_rn(b.ssd, nr);
+        if (kExact) {
+            float nr = __fsqrt_rn(n2);
+            p.u = __fdiv_rn(fx, nr); p.v = __fdiv_rn(fy, nr); p.w = __fdiv_rn(b.ssd, nr);
+        } else {
+            float inr = f_rsqrt(n2);
+            inr = inr * fmaf(-0.5f * n2, inr * inr, 1.5f);  // one Newton step: unit vector to ~1e-7
+            p.u = fx * inr; p.v = fy * inr; p.w = b.ssd * inr;
+        }
     }
     float gx = __fmul_rn(__fsub_rn(p.x, P.g.ox), P.g.ihx), gy = __fmul_rn(__fsub_rn(p.y, P.g.oy), P.g.ihy),
           gz = __fmul_rn(__fsub_rn(p.z, P.g.oz), P.g.ihz);

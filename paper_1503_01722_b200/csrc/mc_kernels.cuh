@@ -295,7 +295,7 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
                     unsigned long long h = P.h_first + (item - P.n_in);
                     L.rng.hist = (uint32_t)h; L.rng.trk_lo = 0; L.rng.trk_hi = 0; L.rng.block = 0;
                     uint4 w4 = next_block(L.rng, P.seed_lo, P.seed_hi);
-                    Primary p = sample_primary(P, w4);
+                    Primary p = sample_primary<false>(P, w4);
                     uint32_t code = P.beam.particle > 0 ? CODE_POSITRON : CODE_ELECTRON;
                     L.tag = (batch_of(h, P.n_batches, P.n_total, P.inv_n_total) << 2) | code;
                     float e0 = p.E + (code == CODE_POSITRON ? 2.0f * kMeF : 0.0f);
@@ -633,7 +633,7 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
                     unsigned long long h = P.h_first + (item - P.n_in);
                     rng.hist = (uint32_t)h; rng.trk_lo = 0; rng.trk_hi = 0; rng.block = 0;
                     uint4 w4 = next_block(rng, P.seed_lo, P.seed_hi);
-                    Primary p = sample_primary(P, w4);
+                    Primary p = sample_primary<false>(P, w4);
                     tag = (batch_of(h, P.n_batches, P.n_total, P.inv_n_total) << 2) | CODE_PHOTON;
                     s_led[tid] += (double)p.E; bump(SP_HIST, 1u);
                     x = p.x; y = p.y; z = p.z; u = p.u; v = p.v; w = p.w; E = p.E;
