@@ -58,6 +58,8 @@ def lib():
         _lib.orc_contract_ln.argtypes = [C.c_float]
         _lib.orc_destroy.argtypes = [C.c_void_p]
         _lib.orc_set_flags.argtypes = [C.c_void_p, C.c_uint32]
+        _lib.orc_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_double]
+        _lib.orc_rotate.argtypes = [C.POINTER(C.c_double), C.c_double, C.c_double, C.POINTER(C.c_double)]
     return _lib
 
 
@@ -141,6 +143,11 @@ class Oracle:
         self._params["flags"] = int(flags)
         lib().orc_set_flags(self._h, int(flags))
 
+    def set_option(self, name, value):
+        """Run-time switches of the readings: hinge_overrun (R8, default 0.25), ms_carry (R8b, default 1)."""
+        if lib().orc_set_option(self._h, name.encode(), float(value)):
+            raise ValueError(f"orc_set_option({name}, {value}) failed")
+
     # -- tables / closed forms ---------------------------------------------------------------
     def grid(self):
         o = np.zeros(4)
@@ -201,6 +208,22 @@ class Oracle:
         if first:
             return edep, dict(zip(STAT_NAMES, st)), fv, fc
         return edep, dict(zip(STAT_NAMES, st))
+
+    def run_probe(self, beam, n, seed, h0=0):
+        """Per-history probe of the primary electron track (orc_run_probe): dict of arrays + stats."""
+        b, keep = _beam_struct(beam)
+        npb = lib().orc_n_probe()
+        o = np.zeros((n, npb))
+        st = np.zeros(lib().orc_n_stats())
+        rc = lib().orc_run_probe(self._h, C.byref(b), C.c_uint64(h0), C.c_uint64(h0 + n), C.c_uint64(max(h0 + n, 1)),
+                                 C.c_uint64(seed), _dp(o), _dp(st))
+        if rc:
+            raise ValueError(f"orc_run_probe failed ({rc})")
+        out = {"first_hard": o[:, 0].astype(int), "T_first": o[:, 1], "pos": o[:, 2:5], "dir": o[:, 5:8], "path": o[:, 8],
+               "steps": o[:, 9], "T_end": o[:, 10], "escaped": o[:, 11].astype(int), "path_first": o[:, 12],
+               "fict_before_first": o[:, 13], "q_sampled": o[:, 14], "q_travelled": o[:, 15],
+               "annih_sum": o[:, 16:19], "annih_mu": o[:, 19]}
+        return out, dict(zip(STAT_NAMES, st))
 
     def run_particles_edep(self, particles, n_total, seed, n_batches, h0=0, h1=None):
         """Particle-list source: `particles` is a structured array (x, y, z, u, v, w, E float32, particle int32)."""
@@ -324,6 +347,20 @@ def sample_moller(T0, e_cut, n, seed=1):
     o = np.zeros((n, 3))
     lib().orc_sample_moller(C.c_double(T0), C.c_double(e_cut), C.c_uint64(n), C.c_uint64(seed), _dp(o))
     return o
+
+
+def sample_iso(n, seed=1):
+    o = np.zeros((n, 3))
+    lib().orc_sample_iso(C.c_uint64(n), C.c_uint64(seed), _dp(o))
+    return o
+
+
+def rotate(d, mu, phi):
+    """The transport code's direction rotation (R25): d rotated by polar cosine mu and azimuth phi."""
+    di = (C.c_double * 3)(*[float(x) for x in d])
+    o = (C.c_double * 3)()
+    lib().orc_rotate(di, float(mu), float(phi), o)
+    return np.array(o[:])
 
 
 def sample_ms(a, n, seed=1):

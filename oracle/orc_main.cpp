@@ -7,8 +7,11 @@
 // differential cross section, Thomson limit, tabulated water values; pair branch continuity and
 // asymptote; restricted-L identity L_col + int W dsigma_M = S_col and ESTAR-like water values;
 // Moller / brems totals vs independent quadrature; chi-square of the KN, Moller, brems samplers;
-// exp(-mu x) attenuation; CSDA range; per-history energy ledger; MS mean cosine.
-// Sources: beams (R13) and particle lists (R13b, orc_run_particles).  Hinge vs voxel face: reading R8 (HINGE_OVERRUN).
+// exp(-mu x) attenuation; CSDA range; per-history energy ledger; MS mean cosine; hard-event rate and first-event
+// spectrum against the quadrature of Sigma/L; <cos> of the primary after a given energy loss against exp(-int K1/L dT)
+// (one voxel and on a 0.25 cm grid: hinge rule R8 + MS carry R8b); rotation at the poles; annihilation isotropy.
+// Every sampler is ONE function, called by transport and by the orc_sample_* pin entries alike.
+// Sources: beams (R13) and particle lists (R13b, orc_run_particles).  Hinge vs voxel face: readings R8 / R8b (orc_set_option).
 // Coupled dose: "parity unpinned" by any external number (no dose value in the paper is
 // reproducible here: gDPM, XCOM data and the 6 MV spectrum are missing) — DESIGN.md says so.
 #include "orc_physics.h"
@@ -48,7 +51,6 @@ struct Stream {
 };
 
 // ------------------------------------------------------------------------------------------------
-constexpr double HINGE_OVERRUN = 0.25;  // DESIGN.md R8
 struct Params { double e_cut, g_cut, e_max; int n_grid; double d_maxs, f_maxe; uint32_t flags; };
 enum { F_NO_HARD = 1, F_NO_MS = 2, F_LOCAL_SEC = 4 };
 
@@ -70,6 +72,9 @@ struct Ctx {
     std::vector<double> mu_maj;  // 1/cm
     int N = 0, k_cut = 0;
     double lnE0 = 0, dln = 0;
+    // run-time options of the readings (orc_set_option): tests A/B them, the engine has the same switches
+    double hinge_overrun = 0.25;  // DESIGN.md R8: the second leg may run on to the face by this fraction of its planned length
+    int ms_carry = 1;             // DESIGN.md R8b: the MS path of a step = planned path + (actual - planned) path of the previous steps
     std::string err;
 };
 
@@ -147,6 +152,94 @@ static void build_tables(Ctx& c) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// Samplers and kinematics.  ONE function each: the transport code (Run::photon / Run::electron) and the
+// orc_sample_* entry points of the chi-square / moment / conservation pins call the same code.
+// Rejection loops take a fresh Philox block per two trials (words 0,1 then 2,3; R15).
+
+// rotate direction d by polar cosine mu and azimuth phi (R25: polar-axis branch near +-z)
+static void rotate_dir(double d[3], double mu, double phi) {
+    double st_ = std::sqrt(std::max(0.0, 1.0 - mu * mu)), cp = std::cos(phi), sp = std::sin(phi);
+    double s2 = 1.0 - d[2] * d[2];
+    double nx_, ny_, nz_;
+    if (s2 < 1e-10) {
+        double sg = d[2] >= 0 ? 1.0 : -1.0;
+        nx_ = st_ * cp; ny_ = st_ * sp; nz_ = sg * mu;
+    } else {
+        double s = std::sqrt(s2);
+        nx_ = d[0] * mu + st_ * (d[0] * d[2] * cp - d[1] * sp) / s;
+        ny_ = d[1] * mu + st_ * (d[1] * d[2] * cp + d[0] * sp) / s;
+        nz_ = d[2] * mu - st_ * s * cp;
+    }
+    double n = std::sqrt(nx_ * nx_ + ny_ * ny_ + nz_ * nz_);
+    d[0] = nx_ / n; d[1] = ny_ / n; d[2] = nz_ / n;
+}
+
+// Klein-Nishina by the epsilon decomposition (R4): eps = E'/E and tt = 1 - cos(theta).  The first word of a
+// trial picks the branch of the decomposition AND, rescaled to (0,1) inside the branch, samples it.
+struct KNSample { double eps, tt; };
+static KNSample sample_kn(Stream& s, double E) {
+    double k0 = E / MEC2, e0 = 1.0 / (1.0 + 2.0 * k0), a1 = std::log(1.0 / e0), a2 = 0.5 * (1.0 - e0 * e0);
+    KNSample o;
+    for (int k = 2;; ++k) {
+        if (k == 2) { s.next(); k = 0; }
+        double r = s.u(2 * k) * (a1 + a2);
+        if (r < a1) o.eps = std::exp(-r);  // = e0^(r/a1)
+        else o.eps = std::sqrt(e0 * e0 + (1.0 - e0 * e0) * (r - a1) / a2);
+        o.tt = (1.0 - o.eps) / (k0 * o.eps);
+        double sin2 = o.tt * (2.0 - o.tt);
+        if (s.u(2 * k + 1) <= 1.0 - o.eps * sin2 / (1.0 + o.eps * o.eps)) break;
+    }
+    return o;
+}
+// Compton kinematics: photon direction d rotated in place by (1 - tt, phi); recoil electron direction from
+// momentum conservation, E d0 - E' d' normalised.
+static void compton_kinematics(double E, const KNSample& kn, double phi, double d[3], double de[3]) {
+    double d0[3] = {d[0], d[1], d[2]}, E1 = kn.eps * E, n = 0;
+    rotate_dir(d, 1.0 - kn.tt, phi);
+    for (int a = 0; a < 3; ++a) { de[a] = E * d0[a] - E1 * d[a]; n += de[a] * de[a]; }
+    n = std::sqrt(n);
+    for (int a = 0; a < 3; ++a) de[a] /= n;
+}
+// Moller (R10): eps = W/T0 from the 1/eps^2 proposal on [e_cut/T0, 1/2], rejection g(eps)/max(g(eps_c), g(1/2)).
+static double sample_moller(Stream& s, double T0, double e_cut) {
+    double tau = T0 / MEC2, g = tau + 1.0, q = (2.0 * g - 1.0) / (g * g), q1 = (g - 1.0) / g;
+    q1 *= q1;
+    double ec = e_cut / T0;
+    auto gf = [&](double e) { return 1.0 - q * e / (1.0 - e) + e * e * (q1 + 1.0 / ((1.0 - e) * (1.0 - e))); };
+    double gmax = std::max(gf(ec), gf(0.5)), eps;
+    for (int k = 2;; ++k) {
+        if (k == 2) { s.next(); k = 0; }
+        eps = 1.0 / (1.0 / ec - s.u(2 * k) * (1.0 / ec - 2.0));
+        if (s.u(2 * k + 1) * gmax <= gf(eps)) break;
+    }
+    return eps;
+}
+// polar cosines of the primary (c1) and of the delta ray (c2) after a Moller event with energy transfer W
+static void moller_angles(double T0, double W, double& c1, double& c2) {
+    c1 = std::sqrt((T0 - W) * (T0 + 2.0 * MEC2) / (T0 * (T0 - W + 2.0 * MEC2)));
+    c2 = std::sqrt(W * (T0 + 2.0 * MEC2) / (T0 * (W + 2.0 * MEC2)));
+}
+// Bremsstrahlung photon energy (R11): k = g_cut (T0/g_cut)^u, rejection F(k)/F_max.
+static double sample_brems(Stream& s, const Material& M, double T0, double g_cut) {
+    double Et = T0 + MEC2;
+    auto Ff = [&](double k) { double Ep = Et - k, rr = Ep / Et; return (1.0 + rr * rr - 2.0 * rr / 3.0) * (std::min(std::log(2.0 * Et * Ep / (MEC2 * k)), M.Lscr) - 0.5); };
+    double Fmax = (4.0 / 3.0) * (std::min(std::log(2.0 * Et * (Et - g_cut) / (MEC2 * g_cut)), M.Lscr) - 0.5), kk;
+    for (int k = 2;; ++k) {
+        if (k == 2) { s.next(); k = 0; }
+        kk = g_cut * std::pow(T0 / g_cut, s.u(2 * k));
+        if (s.u(2 * k + 1) * Fmax <= Ff(kk)) break;
+    }
+    return kk;
+}
+// Multiple scattering, Gaussian on the sphere (R7): 1 - cos(theta) for strength am = 1 - exp(-K1 rho d), uniform u.
+static double sample_ms_omu(double am, double u) { return -am * std::log(1.0 - u * (1.0 - std::exp(-2.0 / am))); }
+// Isotropic direction from two uniforms (annihilation photons, R9).
+static void iso_direction(double u_mu, double u_phi, double d[3]) {
+    double mu = 2.0 * u_mu - 1.0, phi = 2.0 * PI * u_phi, sn = std::sqrt(1.0 - mu * mu);
+    d[0] = sn * std::cos(phi); d[1] = sn * std::sin(phi); d[2] = mu;
+}
+
+// ------------------------------------------------------------------------------------------------
 struct Beam {
     int particle, shape;
     double entry[3], axis[3], ssd, field[2];
@@ -170,6 +263,7 @@ struct Stats {  // doubles so that the Python side can read one flat array
     double max_ledger_rel;
 };
 constexpr int N_STATS = sizeof(Stats) / sizeof(double);
+constexpr int N_PROBE = 20;
 
 struct Run {
     const Ctx& c;
@@ -180,6 +274,7 @@ struct Run {
     std::vector<Particle> stack;
     uint32_t hist = 0;
     int32_t first_vox = -1; int first_chan = -1;  // first real interaction of a primary photon
+    double* probe = nullptr;  // optional per-history record of the primary electron track (N_PROBE doubles, see orc_run_probe)
     double led_src = 0, led_dep = 0, led_esc = 0;
     Run(const Ctx& c_, const Beam& b_, uint64_t s, Stats& st_) : c(c_), b(b_), seed(s), edep(nullptr), st(st_) {}
 
@@ -212,24 +307,6 @@ struct Run {
             return;
         }
         stack.push_back(p);
-    }
-
-    // rotate direction d by polar cosine mu and azimuth phi (R25: polar-axis branch near +-z)
-    static void rotate(double d[3], double mu, double phi) {
-        double st_ = std::sqrt(std::max(0.0, 1.0 - mu * mu)), cp = std::cos(phi), sp = std::sin(phi);
-        double s2 = 1.0 - d[2] * d[2];
-        double nx_, ny_, nz_;
-        if (s2 < 1e-10) {
-            double sg = d[2] >= 0 ? 1.0 : -1.0;
-            nx_ = st_ * cp; ny_ = st_ * sp; nz_ = sg * mu;
-        } else {
-            double s = std::sqrt(s2);
-            nx_ = d[0] * mu + st_ * (d[0] * d[2] * cp - d[1] * sp) / s;
-            ny_ = d[1] * mu + st_ * (d[1] * d[2] * cp + d[0] * sp) / s;
-            nz_ = d[2] * mu - st_ * s * cp;
-        }
-        double n = std::sqrt(nx_ * nx_ + ny_ * ny_ + nz_ * nz_);
-        d[0] = nx_ / n; d[1] = ny_ / n; d[2] = nz_ / n;
     }
 
     // ---- source (R13): block 0 of track (0,0): w0 bin, w1 in-bin energy, w2 x, w3 y ----------
@@ -300,29 +377,11 @@ struct Run {
             }
             // Compton: Klein-Nishina by the epsilon decomposition (R4)
             st.n_compton += 1;
-            double k0 = p.E / MEC2, e0 = 1.0 / (1.0 + 2.0 * k0), a1 = std::log(1.0 / e0), a2 = 0.5 * (1.0 - e0 * e0);
-            double eps, tt;
-            // two trials per Philox block (words 0,1 then 2,3), as for Moller and bremsstrahlung (R15): the first word
-            // picks the branch of the epsilon decomposition AND, rescaled to (0,1) inside the branch, samples it
-            for (int k = 2;; ++k) {
-                if (k == 2) { s.next(); k = 0; }
-                double r = s.u(2 * k) * (a1 + a2);
-                if (r < a1) eps = std::exp(-r);  // = e0^(r/a1)
-                else eps = std::sqrt(e0 * e0 + (1.0 - e0 * e0) * (r - a1) / a2);
-                tt = (1.0 - eps) / (k0 * eps);
-                double sin2 = tt * (2.0 - tt);
-                if (s.u(2 * k + 1) <= 1.0 - eps * sin2 / (1.0 + eps * eps)) break;
-            }
+            KNSample kn = sample_kn(s, p.E);
             s.next();
-            double phi = 2.0 * PI * s.u(2), cost = 1.0 - tt;
-            double d0[3] = {p.d[0], p.d[1], p.d[2]};
-            double E1 = eps * p.E;
-            rotate(p.d, cost, phi);
+            double E1 = kn.eps * p.E;
             Particle e = p; e.q = -1; e.blk0 = 0; e.E = p.E - E1; e.trk_lo = s.w[0]; e.trk_hi = s.w[1];
-            double n = 0;
-            for (int a = 0; a < 3; ++a) { e.d[a] = p.E * d0[a] - E1 * p.d[a]; n += e.d[a] * e.d[a]; }
-            n = std::sqrt(n);
-            for (int a = 0; a < 3; ++a) e.d[a] /= n;
+            compton_kinematics(p.E, kn, 2.0 * PI * s.u(2), p.d, e.d);
             push(e);
             p.E = E1;
             if (p.E < c.p.g_cut) { deposit(p.v, p.E, true); return; }
@@ -347,17 +406,26 @@ struct Run {
     void electron(Particle p) {
         Stream s = stream(p);
         const Params& P = c.p;
+        const bool primary = probe && p.trk_lo == 0 && p.trk_hi == 0;  // per-history probe of the primary track (pins)
+        double path = 0, nstep = 0, q_used = 0, q_act = 0;
+        double ms_carry = 0;  // R8b: scattering power (K1 rho x path) travelled but not yet sampled (< 0: sampled ahead)
+        auto finish = [&](int reason) {
+            if (!primary) return;
+            for (int a = 0; a < 3; ++a) { probe[2 + a] = p.x[a]; probe[5 + a] = p.d[a]; }
+            probe[8] = path; probe[9] = nstep; probe[10] = p.E; probe[11] = reason; probe[14] = q_used; probe[15] = q_act;
+        };
         for (;;) {
             if (p.E <= P.e_cut) {
+                finish(0);
                 deposit(p.v, p.E, true);
                 if (p.q > 0) {  // annihilation at rest: two back-to-back 0.511 MeV photons (R9)
                     s.next();
-                    double mu = 2.0 * s.u(2) - 1.0, phi = 2.0 * PI * s.u(3), sn = std::sqrt(1.0 - mu * mu);
                     Particle g = p; g.q = 0; g.blk0 = 0; g.E = MEC2; g.trk_lo = s.w[0]; g.trk_hi = s.w[1];
-                    g.d[0] = sn * std::cos(phi); g.d[1] = sn * std::sin(phi); g.d[2] = mu;
+                    iso_direction(s.u(2), s.u(3), g.d);
                     s.next();
                     Particle g2 = g; g2.trk_lo = s.w[0]; g2.trk_hi = s.w[1];
                     for (int a = 0; a < 3; ++a) g2.d[a] = -g.d[a];
+                    if (primary) { for (int a = 0; a < 3; ++a) probe[16 + a] = g.d[a] + g2.d[a]; probe[19] = g.d[2]; }
                     push(g); push(g2);
                 }
                 return;
@@ -378,31 +446,37 @@ struct Run {
             if (d_maxe < d) { d = d_maxe; lim = 2; }
             if (d_range < d) { d = d_range; lim = 3; }
             if (d_event < d) { d = d_event; lim = 4; }
-            (&st.lim_vox)[lim] += 1; st.n_estep += 1;
+            (&st.lim_vox)[lim] += 1; st.n_estep += 1; nstep += 1;
             // random hinge (R7, R8)
             double xi = s.u(1);
             for (int a = 0; a < 3; ++a) p.x[a] += xi * d * p.d[a];
+            double k1rho = 0;
             if (!(P.flags & F_NO_MS)) {
                 double Tmid = inv_range(c, t.R, R0 - 0.5 * rho * d);
-                double am = 1.0 - std::exp(-lerp_tab(c, t.K1, Tmid) * rho * d);
-                if (am > 0.0) {
-                    double omu = -am * std::log(1.0 - s.u(2) * (1.0 - std::exp(-2.0 / am)));
-                    rotate(p.d, 1.0 - omu, 2.0 * PI * s.u(3));
-                }
+                k1rho = lerp_tab(c, t.K1, Tmid) * rho;
+                // R8b: the angle is sampled for the planned path d plus the path travelled but not yet sampled for
+                // (the previous steps ended early at a face or ran on to it); never a negative path
+                double tq = k1rho * d + (c.ms_carry ? ms_carry : 0.0);
+                double tu = std::max(tq, 0.0);
+                ms_carry = tq - tu;
+                q_used += tu;
+                double am = 1.0 - std::exp(-tu);
+                if (am > 0.0) rotate_dir(p.d, 1.0 - sample_ms_omu(am, s.u(2)), 2.0 * PI * s.u(3));
             }
             double rest = (1.0 - xi) * d;
             double tf = face_dist(p.x, p.d, p.v, ax);
             // R8: a step cut short by the voxel (d = d_vox) is meant to end on the face; after the deflection the
             // face may be a little further than planned, so the second leg may run on to it, by at most
-            // HINGE_OVERRUN of its planned length and never beyond the non-geometric limits.  Without this,
+            // hinge_overrun of its planned length and never beyond the non-geometric limits.  Without this,
             // about half of the voxel-limited steps stop a hair short of the face and need a tiny extra step.
             double d_lim = std::min(std::min(P.d_maxs, d_maxe), std::min(d_range, d_event));
-            double reach = std::min((1.0 + HINGE_OVERRUN) * rest, d_lim - xi * d);
+            double reach = std::min((1.0 + c.hinge_overrun) * rest, d_lim - xi * d);
             bool cross = tf <= std::max(reach, rest);
             double legB = cross ? tf : rest;
             for (int a = 0; a < 3; ++a) p.x[a] += legB * p.d[a];
             double d_act = xi * d + legB;
-            st.path_e += d_act;
+            st.path_e += d_act; path += d_act;
+            ms_carry += k1rho * (d_act - d); q_act += k1rho * d_act;
             // a range-limited step that stayed in the voxel ends exactly at the cut-off
             double T1 = (lim == 3 && !cross) ? P.e_cut : inv_range(c, t.R, R0 - rho * d_act);
             deposit(p.v, T - T1, false);
@@ -411,7 +485,7 @@ struct Run {
                 int dir = p.d[ax] > 0 ? 1 : -1;
                 p.v[ax] += dir;
                 p.x[ax] = c.org[ax] + (p.v[ax] + (dir > 0 ? 0 : 1)) * c.h[ax];  // snap to the face
-                if (!inside(p.v)) { escape(p.E + (p.q > 0 ? 2.0 * MEC2 : 0.0)); return; }
+                if (!inside(p.v)) { finish(1); escape(p.E + (p.q > 0 ? 2.0 * MEC2 : 0.0)); return; }
                 continue;
             }
             if (lim != 4 || p.E <= P.e_cut) continue;
@@ -419,45 +493,25 @@ struct Run {
             s.next();
             double r = s.u(0) * Smax;
             double SM = lerp_tab(c, t.S_M, p.E), SH = lerp_tab(c, t.S_hard, p.E);
-            if (r >= SH) continue;  // fictitious
+            if (r >= SH) { if (primary && probe[0] == 0) probe[13] += 1; continue; }  // fictitious
             uint32_t id_lo = s.w[1], id_hi = s.w[2];
             double phi = 2.0 * PI * s.u(3);
             double T0 = p.E;
+            if (primary && probe[0] == 0) { probe[0] = r < SM ? 1 : 2; probe[1] = T0; probe[12] = path; }
             if (r < SM) {  // Moller (R10)
                 st.n_moller += 1;
-                double tau = T0 / MEC2, g = tau + 1.0, q = (2.0 * g - 1.0) / (g * g), q1 = (g - 1.0) / g;
-                q1 *= q1;
-                double ec = P.e_cut / T0;
-                auto gf = [&](double e) { return 1.0 - q * e / (1.0 - e) + e * e * (q1 + 1.0 / ((1.0 - e) * (1.0 - e))); };
-                double gmax = std::max(gf(ec), gf(0.5));
-                double eps;
-                for (int k = 2;; ++k) {
-                    if (k == 2) { s.next(); k = 0; }
-                    eps = 1.0 / (1.0 / ec - s.u(2 * k) * (1.0 / ec - 2.0));
-                    if (s.u(2 * k + 1) * gmax <= gf(eps)) break;
-                }
-                double W = eps * T0;
-                double c1 = std::sqrt((T0 - W) * (T0 + 2.0 * MEC2) / (T0 * (T0 - W + 2.0 * MEC2)));
-                double c2 = std::sqrt(W * (T0 + 2.0 * MEC2) / (T0 * (W + 2.0 * MEC2)));
+                double W = sample_moller(s, T0, P.e_cut) * T0, c1, c2;
+                moller_angles(T0, W, c1, c2);
                 Particle e = p; e.q = -1; e.blk0 = 0; e.E = W; e.trk_lo = id_lo; e.trk_hi = id_hi;
-                rotate(e.d, c2, phi + PI);
-                rotate(p.d, c1, phi);
+                rotate_dir(e.d, c2, phi + PI);
+                rotate_dir(p.d, c1, phi);
                 p.E = T0 - W;
                 push(e);
             } else {  // bremsstrahlung (R11)
                 st.n_brems += 1;
-                const Material& M = c.mats[c.mat[vi]];
-                double Et = T0 + MEC2;
-                auto Ff = [&](double k) { double Ep = Et - k, rr = Ep / Et; return (1.0 + rr * rr - 2.0 * rr / 3.0) * (std::min(std::log(2.0 * Et * Ep / (MEC2 * k)), M.Lscr) - 0.5); };
-                double Fmax = (4.0 / 3.0) * (std::min(std::log(2.0 * Et * (Et - P.g_cut) / (MEC2 * P.g_cut)), M.Lscr) - 0.5);
-                double kk;
-                for (int k = 2;; ++k) {
-                    if (k == 2) { s.next(); k = 0; }
-                    kk = P.g_cut * std::pow(T0 / P.g_cut, s.u(2 * k));
-                    if (s.u(2 * k + 1) * Fmax <= Ff(kk)) break;
-                }
+                double kk = sample_brems(s, c.mats[c.mat[vi]], T0, P.g_cut);
                 Particle g = p; g.q = 0; g.blk0 = 0; g.E = kk; g.trk_lo = id_lo; g.trk_hi = id_hi;
-                rotate(g.d, std::cos(MEC2 / Et), phi);
+                rotate_dir(g.d, std::cos(MEC2 / (T0 + MEC2)), phi);
                 p.E = T0 - kk;
                 push(g);
             }
@@ -709,75 +763,98 @@ int orc_finalize(const Ctx* c, const double* edep, uint64_t n_total, int n_batch
     return 0;
 }
 
-// ---- samplers exposed one interaction at a time, for the chi-square / conservation pins ----
-// Each draws from history stream h = i (track 0) exactly as the transport code does.
+// ---- samplers exposed one interaction at a time, for the chi-square / moment / conservation pins ----
+// Each entry draws from history stream h = i (track 0) and calls the SAME sampler function the transport code calls.
+static Stream pin_stream(uint64_t i, uint64_t seed) {
+    Stream s; s.h = (uint32_t)i; s.seed_lo = (uint32_t)seed; s.seed_hi = (uint32_t)(seed >> 32); s.trk_lo = s.trk_hi = 0; s.block = 0;
+    return s;
+}
 // KN: out[4*i+0]=eps, [1]=cos(theta_photon), [2]=dot(electron dir, incoming), [3]=|p_in - p_g - p_e|/p_in residual
 void orc_sample_kn(double E, uint64_t n, uint64_t seed, double* out) {
     for (uint64_t i = 0; i < n; ++i) {
-        Stream s; s.h = (uint32_t)i; s.seed_lo = (uint32_t)seed; s.seed_hi = (uint32_t)(seed >> 32); s.trk_lo = s.trk_hi = 0; s.block = 0;
-        double k0 = E / MEC2, e0 = 1.0 / (1.0 + 2.0 * k0), a1 = std::log(1.0 / e0), a2 = 0.5 * (1.0 - e0 * e0), eps, tt;
-        for (int k = 2;; ++k) {
-            if (k == 2) { s.next(); k = 0; }
-            double r = s.u(2 * k) * (a1 + a2);
-            if (r < a1) eps = std::exp(-r); else eps = std::sqrt(e0 * e0 + (1.0 - e0 * e0) * (r - a1) / a2);
-            tt = (1.0 - eps) / (k0 * eps);
-            if (s.u(2 * k + 1) <= 1.0 - eps * tt * (2.0 - tt) / (1.0 + eps * eps)) break;
-        }
+        Stream s = pin_stream(i, seed);
+        KNSample kn = sample_kn(s, E);
         s.next();
-        double d0[3] = {0.6, 0.0, 0.8}, d1[3] = {0.6, 0.0, 0.8};
-        Run::rotate(d1, 1.0 - tt, 2.0 * PI * s.u(2));
-        double E1 = eps * E, Te = E - E1, pe = std::sqrt(Te * (Te + 2.0 * MEC2));
-        double ed[3], nn = 0;
-        for (int a = 0; a < 3; ++a) { ed[a] = E * d0[a] - E1 * d1[a]; nn += ed[a] * ed[a]; }
-        nn = std::sqrt(nn);
+        const double d0[3] = {0.6, 0.0, 0.8};
+        double d1[3] = {0.6, 0.0, 0.8}, ed[3];
+        compton_kinematics(E, kn, 2.0 * PI * s.u(2), d1, ed);
+        double E1 = kn.eps * E, Te = E - E1, pe = std::sqrt(Te * (Te + 2.0 * MEC2));
         double res = 0, dot = 0;
-        for (int a = 0; a < 3; ++a) { double r = E * d0[a] - E1 * d1[a] - pe * ed[a] / nn; res += r * r; dot += ed[a] / nn * d0[a]; }
-        out[4 * i] = eps; out[4 * i + 1] = d0[0] * d1[0] + d0[1] * d1[1] + d0[2] * d1[2]; out[4 * i + 2] = dot; out[4 * i + 3] = std::sqrt(res) / E;
+        for (int a = 0; a < 3; ++a) { double r = E * d0[a] - E1 * d1[a] - pe * ed[a]; res += r * r; dot += ed[a] * d0[a]; }
+        out[4 * i] = kn.eps; out[4 * i + 1] = d0[0] * d1[0] + d0[1] * d1[1] + d0[2] * d1[2]; out[4 * i + 2] = dot; out[4 * i + 3] = std::sqrt(res) / E;
     }
 }
 // Moller: out[3*i+0]=eps, [1]=cos theta primary, [2]=cos theta delta
 void orc_sample_moller(double T0, double e_cut, uint64_t n, uint64_t seed, double* out) {
     for (uint64_t i = 0; i < n; ++i) {
-        Stream s; s.h = (uint32_t)i; s.seed_lo = (uint32_t)seed; s.seed_hi = (uint32_t)(seed >> 32); s.trk_lo = s.trk_hi = 0; s.block = 0;
-        double tau = T0 / MEC2, g = tau + 1.0, q = (2.0 * g - 1.0) / (g * g), q1 = (g - 1.0) / g; q1 *= q1;
-        double ec = e_cut / T0;
-        auto gf = [&](double e) { return 1.0 - q * e / (1.0 - e) + e * e * (q1 + 1.0 / ((1.0 - e) * (1.0 - e))); };
-        double gmax = std::max(gf(ec), gf(0.5)), eps;
-        for (int k = 2;; ++k) {
-            if (k == 2) { s.next(); k = 0; }
-            eps = 1.0 / (1.0 / ec - s.u(2 * k) * (1.0 / ec - 2.0));
-            if (s.u(2 * k + 1) * gmax <= gf(eps)) break;
-        }
-        double W = eps * T0;
+        Stream s = pin_stream(i, seed);
+        double eps = sample_moller(s, T0, e_cut);
         out[3 * i] = eps;
-        out[3 * i + 1] = std::sqrt((T0 - W) * (T0 + 2.0 * MEC2) / (T0 * (T0 - W + 2.0 * MEC2)));
-        out[3 * i + 2] = std::sqrt(W * (T0 + 2.0 * MEC2) / (T0 * (W + 2.0 * MEC2)));
+        moller_angles(T0, eps * T0, out[3 * i + 1], out[3 * i + 2]);
     }
 }
 // brems photon energy k for material m of ctx
 void orc_sample_brems(const Ctx* c, int m, double T0, uint64_t n, uint64_t seed, double* out) {
-    const Material& M = c->mats[m];
-    double g_cut = c->p.g_cut;
     for (uint64_t i = 0; i < n; ++i) {
-        Stream s; s.h = (uint32_t)i; s.seed_lo = (uint32_t)seed; s.seed_hi = (uint32_t)(seed >> 32); s.trk_lo = s.trk_hi = 0; s.block = 0;
-        double Et = T0 + MEC2;
-        auto Ff = [&](double k) { double Ep = Et - k, rr = Ep / Et; return (1.0 + rr * rr - 2.0 * rr / 3.0) * (std::min(std::log(2.0 * Et * Ep / (MEC2 * k)), M.Lscr) - 0.5); };
-        double Fmax = (4.0 / 3.0) * (std::min(std::log(2.0 * Et * (Et - g_cut) / (MEC2 * g_cut)), M.Lscr) - 0.5), kk;
-        for (int k = 2;; ++k) {
-            if (k == 2) { s.next(); k = 0; }
-            kk = g_cut * std::pow(T0 / g_cut, s.u(2 * k));
-            if (s.u(2 * k + 1) * Fmax <= Ff(kk)) break;
-        }
-        out[i] = kk;
+        Stream s = pin_stream(i, seed);
+        out[i] = sample_brems(s, c->mats[m], T0, c->p.g_cut);
     }
 }
-// MS polar cosine for a given a = 1 - exp(-K1 rho d)
+// MS polar cosine for a given a = 1 - exp(-K1 rho d) (word 2 of the step block, as in transport)
 void orc_sample_ms(double am, uint64_t n, uint64_t seed, double* out) {
     for (uint64_t i = 0; i < n; ++i) {
-        Stream s; s.h = (uint32_t)i; s.seed_lo = (uint32_t)seed; s.seed_hi = (uint32_t)(seed >> 32); s.trk_lo = s.trk_hi = 0; s.block = 0;
+        Stream s = pin_stream(i, seed);
         s.next();
-        out[i] = 1.0 + am * std::log(1.0 - s.u(2) * (1.0 - std::exp(-2.0 / am)));
+        out[i] = 1.0 - sample_ms_omu(am, s.u(2));
     }
+}
+// annihilation photon direction (words 2, 3 of the block, as in transport): out[3*i..] = unit vector
+void orc_sample_iso(uint64_t n, uint64_t seed, double* out) {
+    for (uint64_t i = 0; i < n; ++i) {
+        Stream s = pin_stream(i, seed);
+        s.next();
+        iso_direction(s.u(2), s.u(3), out + 3 * i);
+    }
+}
+// the direction rotation of the transport code (R25), one call
+void orc_rotate(const double* d, double mu, double phi, double* out) {
+    out[0] = d[0]; out[1] = d[1]; out[2] = d[2];
+    rotate_dir(out, mu, phi);
+}
+// run-time switches of the readings R8 / R8b (defaults: hinge_overrun 0.25, ms_carry 1)
+int orc_set_option(Ctx* c, const char* name, double value) {
+    if (!c || !name) return 1;
+    std::string n(name);
+    if (n == "hinge_overrun") { if (!(value >= 0.0 && value <= 1.0)) return 1; c->hinge_overrun = value; }
+    else if (n == "ms_carry") c->ms_carry = value != 0.0;
+    else return 1;
+    return 0;
+}
+int orc_n_probe() { return N_PROBE; }
+// Per-history probe of the PRIMARY electron / positron track, for the transport-level pins (hard-event rate, MS in
+// transport, hinge rule).  Runs histories [h0, h1) like orc_run (dose goes to a scratch grid) and writes N_PROBE doubles
+// per history: [0] first real hard event (0 none, 1 Moller, 2 bremsstrahlung), [1] kinetic energy at that event,
+// [2..4] final position, [5..7] final direction, [8] path length, [9] steps, [10] final kinetic energy,
+// [11] end (0 absorbed at the cut-off, 1 left the phantom), [12] path length at the first hard event,
+// [13] fictitious candidates before it, [14] sum of the scattering powers the MS angles were sampled for,
+// [15] sum of K1 rho x path actually travelled, [16..18] sum of the two annihilation-photon directions (positron),
+// [19] z direction cosine of the first annihilation photon.
+int orc_run_probe(Ctx* c, const orc_beam* b, uint64_t h0, uint64_t h1, uint64_t n_total, uint64_t seed, double* out, double* stats_out) {
+    if (!c || !c->have_tables) return 2;
+    if (!b || !out || n_total >= (1ull << 32) || h1 > n_total || h0 > h1 || b->n_nodes < 1) return 1;
+    Beam B; to_beam(b, B);
+    for (double E : B.E) if (E > c->p.e_max) return 3;
+    Stats st; std::memset(&st, 0, sizeof st);
+    Run run(*c, B, seed, st);
+    std::vector<double> scratch(c->mat.size(), 0.0);
+    run.edep = scratch.data();
+    for (uint64_t h = h0; h < h1; ++h) {
+        run.probe = out + (h - h0) * N_PROBE;
+        for (int k = 0; k < N_PROBE; ++k) run.probe[k] = 0.0;
+        run.history((uint32_t)h);
+    }
+    if (stats_out) std::memcpy(stats_out, &st, sizeof st);
+    return 0;
 }
 // primaries only: energy, position, direction (7 doubles per history) — source pins
 void orc_sample_source(Ctx* c, const orc_beam* b, uint64_t n, uint64_t seed, double* out) {
