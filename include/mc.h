@@ -4,7 +4,7 @@
  *   - a voxelised phantom, "each voxel was assigned to a density value and a material type"
  *     (§2.1)                                            -> mc_create
  *   - "physics data needed by oclMC based on a user-defined material composition", cut-offs and
- *     maximum step sizes are user defined    -> mc_build_tables / mc_set_tables
+ *     maximum step sizes are user defined    -> mc_build_tables / mc_set_photon_tables
  *   - a point source with an energy or spectrum, a field at the surface, an SSD;
  *     result "in a unit of MeV/g per source particle" with its uncertainty sigma_D
  *                                                                     -> mc_run
@@ -226,7 +226,12 @@ mc_status mc_set_stream(mc_ctx *ctx, void *cuda_stream);
  *   "blocks_per_sm" cap on the CTAs per SM (0 = as many as fit; the transport kernels use one)
  *   "aggregate"     1: lanes of a warp that score into the same cell at the same moment combine into one
  *                   red.global.add.f32; 0: one per lane; -1 (default): 1 for beams entering through fewer than 16
- *                   voxel columns, else 0 */
+ *                   voxel columns, else 0
+ * Readings of the method (R8, R8b; the oracle has the same two switches, used by A/B tests):
+ *   "hinge_overrun_pct"  the second leg of a voxel-limited step may run on to the face by this percentage of its
+ *                   planned length (default 25; 0 = the plain rule)
+ *   "ms_carry"      1 (default): the multiple-scattering angle of a step is sampled for the planned path plus the path
+ *                   travelled but not yet sampled for (steps a voxel face cut short or lengthened); 0: planned path only */
 mc_status mc_set_option(mc_ctx *ctx, const char *name, int64_t value);
 const char *mc_last_error(const mc_ctx *ctx);
 const char *mc_version(void);

@@ -83,6 +83,8 @@ struct RunParams {
     int hard_lanes;           // lanes of a warp that must hold a pending hard event before the warp runs that block
     // table coordinate <-> energy in base 2: ex = lg2(T) * ex_a - ex_b;  T = ex2(ex * t_a + t_b)
     float ex_a, ex_b, t_a, t_b;
+    float hinge_overrun;      // DESIGN.md R8
+    int ms_carry;             // DESIGN.md R8b
 };
 
 // ---- Philox4x32-10 -----------------------------------------------------------------------------

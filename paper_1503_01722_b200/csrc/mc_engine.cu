@@ -44,6 +44,7 @@ struct mc_ctx {
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     // options (M "manually adjusted")
     int64_t wave_size = 1 << 24, queue_factor = 4, blocks_per_sm = 0, refill_lanes = 32, aggregate = -1, hard_lanes = 32, adaptive = 1;
+    int64_t hinge_overrun_pct = 25, ms_carry = 1;  // readings R8 / R8b; the oracle has the same switches
     mc_stats stats{};
     // secondaries-per-primary ratios measured by the last run, reused when the next run has the same kind of beam
     double beam_key = -1.0, last_m_e = 16.0, last_m_p = 16.0;
@@ -218,6 +219,7 @@ void fill_params(const mc_ctx* ctx, RunParams& P) {
     const double ln2 = 0.69314718055994530942, log2e = 1.44269504088896340736;
     P.ex_a = (float)(ln2 / t.dln); P.ex_b = (float)(t.lnE0 / t.dln);
     P.t_a = (float)(t.dln * log2e); P.t_b = (float)(t.lnE0 * log2e);
+    P.hinge_overrun = 0.01f * (float)ctx->hinge_overrun_pct; P.ms_carry = (int)ctx->ms_carry;
 }
 
 }  // namespace
@@ -798,6 +800,8 @@ mc_status mc_set_option(mc_ctx* ctx, const char* name, int64_t value) {
     else if (n == "hard_lanes") { if (value < 1 || value > 64) return fail(ctx, MC_ERR_INVALID_ARG, "hard_lanes in [1, 64]"); ctx->hard_lanes = value; }
     else if (n == "adaptive") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "adaptive in {0, 1}"); ctx->adaptive = value; }
     else if (n == "aggregate") { if (value < -1 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "aggregate in {-1, 0, 1}"); ctx->aggregate = value; }
+    else if (n == "hinge_overrun_pct") { if (value < 0 || value > 100) return fail(ctx, MC_ERR_INVALID_ARG, "hinge_overrun_pct in [0, 100]"); ctx->hinge_overrun_pct = value; }
+    else if (n == "ms_carry") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "ms_carry in {0, 1}"); ctx->ms_carry = value; }
     else return fail(ctx, MC_ERR_INVALID_ARG, "unknown option: " + n);
     return MC_OK;
 }

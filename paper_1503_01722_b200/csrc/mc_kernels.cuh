@@ -131,7 +131,6 @@ __device__ __forceinline__ void emit(const RunParams& P, const Queue& q, Score& 
 // One CTA per SM (the tables are staged once per SM).  kThreadsE = CTA size: 768 (24 warps) when tables + pools fit in
 // the 227 KB of shared memory, else 512 or 256 (more materials / finer grids); instantiated in mc_engine.cu.
 constexpr int kSlots = 2;       // tracks per lane, parked in shared memory between the blocks that work on them
-constexpr float kHingeOverrun = 0.25f;  // DESIGN.md R8
 enum LaneState { L_IDLE = 0, L_STEP = 1, L_HARD = 2, L_DONE = 3 };
 constexpr int kTrackWords = 24;
 enum { SE_STEP = 0, SE_MOLLER, SE_BREMS, SE_SEC_E, SE_SEC_G, SE_HIST, SE_RED, SE_COUNT };
@@ -150,6 +149,7 @@ __device__ __forceinline__ void face_all(const Geometry& g, float x, float y, fl
 
 struct ELane {
     float x, y, z, u, v, w, T, ex, rho, tx, ty, tz, acc, smax;
+    float msc;  // R8b: scattering power travelled but not yet sampled for (< 0: sampled ahead)
     int ix, iy, iz, vox, mat;
     uint32_t tag;
     Rng rng;
@@ -186,14 +186,14 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
     uint32_t n_step_w = 0u;
     ELane L;
     L.x = L.y = L.z = 0.f; L.u = L.v = 0.f; L.w = 1.f; L.T = 0.f; L.ex = 0.f; L.rho = 1.f; L.tx = L.ty = L.tz = 0.f;
-    L.acc = 0.f; L.smax = 0.f; L.ix = L.iy = L.iz = L.vox = L.mat = 0; L.tag = 0u; L.rng = {0, 0, 0, 0};
+    L.acc = 0.f; L.smax = 0.f; L.msc = 0.f; L.ix = L.iy = L.iz = L.vox = L.mat = 0; L.tag = 0u; L.rng = {0, 0, 0, 0};
     auto W = [&](int f, int sl) -> uint32_t& { return s_trk[f * (kSlots * kThreadsE) + sl]; };
     // what = 0: a new track, every word; 1: after a step or a hard event that stayed in its voxel; 2: after a step
     // that crossed into another voxel.  Identity words (tag, history, track id) never change after birth.
     auto store_slot = [&](int k, int what) {
         W(0, k) = __float_as_uint(L.x); W(1, k) = __float_as_uint(L.y); W(2, k) = __float_as_uint(L.z);
         W(3, k) = __float_as_uint(L.u); W(4, k) = __float_as_uint(L.v); W(5, k) = __float_as_uint(L.w);
-        W(6, k) = __float_as_uint(L.T); W(7, k) = __float_as_uint(L.ex);
+        W(6, k) = __float_as_uint(L.T); W(7, k) = __float_as_uint(L.msc);
         W(9, k) = __float_as_uint(L.tx); W(10, k) = __float_as_uint(L.ty); W(11, k) = __float_as_uint(L.tz);
         W(12, k) = __float_as_uint(L.acc); W(23, k) = L.rng.block;
         if (state == L_HARD) W(13, k) = __float_as_uint(L.smax);
@@ -207,11 +207,12 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
     auto load_slot = [&](int k) {
         L.x = __uint_as_float(W(0, k)); L.y = __uint_as_float(W(1, k)); L.z = __uint_as_float(W(2, k));
         L.u = __uint_as_float(W(3, k)); L.v = __uint_as_float(W(4, k)); L.w = __uint_as_float(W(5, k));
-        L.T = __uint_as_float(W(6, k)); L.ex = __uint_as_float(W(7, k)); L.rho = __uint_as_float(W(8, k));
+        L.T = __uint_as_float(W(6, k)); L.msc = __uint_as_float(W(7, k)); L.rho = __uint_as_float(W(8, k));
         L.tx = __uint_as_float(W(9, k)); L.ty = __uint_as_float(W(10, k)); L.tz = __uint_as_float(W(11, k));
         L.acc = __uint_as_float(W(12, k)); L.smax = __uint_as_float(W(13, k));
         L.ix = (int)W(14, k); L.iy = (int)W(15, k); L.iz = (int)W(16, k); L.vox = (int)W(17, k);
         L.mat = (int)W(18, k); L.tag = W(19, k);
+        L.ex = fmaf(f_lg2(L.T), P.ex_a, -P.ex_b);  // table coordinate of T (not stored)
         L.rng.hist = W(20, k); L.rng.trk_lo = W(21, k); L.rng.trk_hi = W(22, k); L.rng.block = W(23, k);
     };
     auto park = [&](int what) {  // put the working track back into its pool slot: only live tracks need their data
@@ -282,7 +283,7 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
             // ---- REFILL: queue first, then new primaries (S0, S1) --------------------------------
             uint32_t item = claim(P.counters + C_HEAD, n_work >= 32 ? kFull : ((1u << n_work) - 1u), lane);
             if (have) {
-                state = L_IDLE; L.acc = 0.0f;
+                state = L_IDLE; L.acc = 0.0f; L.msc = 0.0f;
                 bool ok = false;
                 if (item < P.n_in) {
                     QRec r = load_record(P.q_in, item);
@@ -436,10 +437,14 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         const float xl = rho * L0 * f_rcp(L.T);  // fractional energy loss per unit path at constant L (search guess only)
         const float rd = rho * d;
         bool turned = false;
+        float k1rho = 0.0f;
         if (!no_ms) {
             float em = inv_range_coord(tm, fmaf(-0.5f, rd, R0), fmaf(f_lg2(fmaf(-0.5f * d, xl, 1.0f)), P.ex_a, L.ex), k_cut, N);
             int im = min(max((int)em, 0), N - 2);
-            float t = lerp(tm + (TE_K1 - TE_R) * N, im, em - (float)im) * rd;
+            k1rho = lerp(tm + (TE_K1 - TE_R) * N, im, em - (float)im) * rho;
+            // R8b: sample for the planned path plus the path travelled but not yet sampled for; never a negative path
+            const float tq = fmaf(k1rho, d, P.ms_carry ? L.msc : 0.0f), t = fmaxf(tq, 0.0f);
+            L.msc = tq - t;
             float am = t < 1e-3f ? t * (1.0f - 0.5f * t) : 1.0f - f_exp(-t);
             if (am > 0.0f) {
                 float omu = -am * kLn2F * f_lg2(1.0f - u01f(w4.z) * (1.0f - f_exp(-2.0f * f_rcp(am))));
@@ -457,11 +462,12 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         if (L.tz < tf) { tf = L.tz; ax = 2; }
         // R8: a voxel-limited step may run on to the face by up to kHingeOverrun of the planned second leg, never
         // beyond the non-geometric limits (removes the tiny catch-up steps after half of the voxel-limited steps)
-        const bool cross = tf <= fmaxf(fminf((1.0f + kHingeOverrun) * rest, d_lim - legA), rest);
+        const bool cross = tf <= fmaxf(fminf((1.0f + P.hinge_overrun) * rest, d_lim - legA), rest);
         const float legB = cross ? tf : rest;
         L.x = fmaf(legB, L.u, L.x); L.y = fmaf(legB, L.v, L.y); L.z = fmaf(legB, L.w, L.z);
         L.tx = fmaxf(L.tx - legB, 0.0f); L.ty = fmaxf(L.ty - legB, 0.0f); L.tz = fmaxf(L.tz - legB, 0.0f);
         const float d_act = legA + legB;
+        L.msc = fmaf(k1rho, d_act - d, L.msc);
         // ---- CSDA loss through the range table (S6; R5) + scoring ------------------------------------------
         float T1, ex1;
         if (lim == 3 && !cross) { T1 = P.e_cut; ex1 = (float)k_cut; }
