@@ -114,7 +114,8 @@ typedef struct {
 } mc_stats;
 
 /* mc_create — copy the phantom to the device.
- * material_idx, density_gcc: nx*ny*nz entries (host), density > 0.  dims > 0, voxel_cm > 0.
+ * material_idx, density_gcc: nx*ny*nz entries (host), density > 0.  1 <= dims <= 1024 per axis (a track carries
+ * its voxel indices in one 32-bit word), voxel_cm > 0.
  * origin_cm: coordinates of the low corner of voxel (0,0,0).  *out receives the context. */
 mc_status mc_create(const uint8_t *material_idx, const float *density_gcc, const int32_t dims[3],
                     const float voxel_cm[3], const float origin_cm[3], mc_ctx **out);

@@ -55,7 +55,12 @@ enum StatId {
     S_HIST, S_COUNT
 };
 enum LedgerId { LG_SRC = 0, LG_ESC, LG_DEP, LG_COUNT };
-enum { TE_R = 0, TE_L, TE_SMAX, TE_SM, TE_SHARD, TE_K1, TE_COUNT };  // electron tables per material
+// electron tables per material, node-interleaved so that one 16-byte load serves a look-up (float2 units, N = nodes):
+//   [0, 2N)  float4 (R, dR, L, dL)            step start            (d = slope to the next node)
+//   [2N, 4N) float4 (R, 1/dR, K1, dK1)        inverse-range probes + K1 at the probed node
+//   [4N, 6N) float4 (S_hard, d, S_Moller, d)  hard-event thinning
+//   [6N, 7N) float2 (S_max, d)                d_event
+constexpr int kETabUnits = 7;  // float2 per node and material; the per-material stride is rounded up to 16 bytes
 enum { TP_TOT = 0, TP_C, TP_PP, TP_COUNT };                         // photon tables per material (after mu_maj)
 enum { CODE_ELECTRON = 0u, CODE_POSITRON = 1u, CODE_PHOTON = 2u };
 struct RunParams {
@@ -63,8 +68,9 @@ struct RunParams {
     BeamDev beam;
     const uint2* vox;    // per voxel: (density bits, material index)
     const float2* tabP;  // photon tables, (value, slope): [0] mu_maj, then per material mu_tot, mu_C, mu_pp
-    const float2* tabE;  // electron tables per material: R, L, S_max, S_M, S_hard, K1
+    const float2* tabE;  // electron tables per material (layout: kETabUnits above)
     int N, n_mat, k_cut;
+    int e_stride;        // float2 per material in tabE
     float lnE0, dln, inv_dln, e_cut, g_cut, d_maxs, f_maxe;
     float lnE0P, inv_dlnP;  // grid of the photon tables (may be user supplied, mc_set_photon_tables)
     float lscr[MAX_MAT];

@@ -67,6 +67,8 @@ mc_status fail(mc_ctx* c, mc_status s, const std::string& msg) {
                         std::string(#call) + ": " + cudaGetErrorString(e_));                       \
     } while (0)
 
+size_t e_stride(int N) { return ((size_t)kETabUnits * N + 1) & ~(size_t)1; }  // float2 per material, 16-byte multiple
+
 std::vector<float2> pairs(const float* t, int N) {  // (value, slope to the next node); fp32 subtraction (R20)
     std::vector<float2> o(N);
     for (int i = 0; i < N; ++i) { o[i].x = t[i]; o[i].y = i + 1 < N ? t[i + 1] - t[i] : 0.0f; }
@@ -107,7 +109,8 @@ mc_status upload_tables(mc_ctx* ctx) {
     if (!ctx->tables_dirty) return MC_OK;
     const Tables& t = ctx->tabs;
     const int N = t.N, nm = t.n_mat;
-    std::vector<float2> P((size_t)(1 + nm * TP_COUNT) * N), E((size_t)nm * TE_COUNT * N);
+    const size_t es = e_stride(N);
+    std::vector<float2> P((size_t)(1 + nm * TP_COUNT) * N), E((size_t)nm * es, float2{0.0f, 0.0f});
     auto put = [&](std::vector<float2>& dst, size_t slot, const float* src) {
         std::vector<float2> pr = pairs(src, N);
         std::copy(pr.begin(), pr.end(), dst.begin() + slot * N);
@@ -117,8 +120,16 @@ mc_status upload_tables(mc_ctx* ctx) {
         put(P, 1 + m * TP_COUNT + TP_TOT, ctx->p_tot.data() + (size_t)m * N);
         put(P, 1 + m * TP_COUNT + TP_C, ctx->p_C.data() + (size_t)m * N);
         put(P, 1 + m * TP_COUNT + TP_PP, ctx->p_pp.data() + (size_t)m * N);
-        const int src[TE_COUNT] = {T_RANGE, T_L, T_S_MAX, T_S_MOLLER, T_S_HARD, T_K1};
-        for (int k = 0; k < TE_COUNT; ++k) put(E, (size_t)m * TE_COUNT + k, t.t[src[k]][m].data());
+        // electron tables, node-interleaved (mc_device.cuh: kETabUnits)
+        const std::vector<float2> R = pairs(t.t[T_RANGE][m].data(), N), Lc = pairs(t.t[T_L][m].data(), N), K1 = pairs(t.t[T_K1][m].data(), N),
+                                  SH = pairs(t.t[T_S_HARD][m].data(), N), SM = pairs(t.t[T_S_MOLLER][m].data(), N), SX = pairs(t.t[T_S_MAX][m].data(), N);
+        float2* e = E.data() + (size_t)m * es;
+        for (int i = 0; i < N; ++i) {
+            e[2 * i] = R[i]; e[2 * i + 1] = Lc[i];
+            e[2 * N + 2 * i] = float2{R[i].x, R[i].y != 0.0f ? 1.0f / R[i].y : 0.0f}; e[2 * N + 2 * i + 1] = K1[i];
+            e[4 * N + 2 * i] = SH[i]; e[4 * N + 2 * i + 1] = SM[i];
+            e[6 * N + i] = SX[i];
+        }
     }
     if (P.size() > ctx->tabP_cap) { cudaFree(ctx->d_tabP); ctx->d_tabP = nullptr; CU(cudaMalloc(&ctx->d_tabP, P.size() * sizeof(float2))); ctx->tabP_cap = P.size(); }
     if (E.size() > ctx->tabE_cap) { cudaFree(ctx->d_tabE); ctx->d_tabE = nullptr; CU(cudaMalloc(&ctx->d_tabE, E.size() * sizeof(float2))); ctx->tabE_cap = E.size(); }
@@ -130,8 +141,8 @@ mc_status upload_tables(mc_ctx* ctx) {
 
 // shared memory of a transport CTA of T threads: tables + per-thread counters + per-thread energy ledger + track pool
 size_t smem_e(const mc_ctx* c, int T) {
-    return (size_t)c->tabs.n_mat * TE_COUNT * c->tabs.N * sizeof(float2) + (size_t)SE_COUNT * T * sizeof(uint32_t) +
-           2 * (size_t)T * sizeof(double) + (size_t)(kTrackWords * kSlots + kSlots + 1) * T * sizeof(uint32_t);
+    return (size_t)c->tabs.n_mat * e_stride(c->tabs.N) * sizeof(float2) + (size_t)SE_COUNT * T * sizeof(uint32_t) +
+           2 * (size_t)T * sizeof(double) + (size_t)kGroups * kSlots * T * sizeof(uint4) + 2 * (size_t)T * sizeof(uint32_t);
 }
 size_t smem_p(const mc_ctx* c, int T) {
     return (size_t)(1 + c->tabs.n_mat * TP_COUNT) * c->tabs.N * sizeof(float2) + (size_t)SP_COUNT * T * sizeof(uint32_t) +
@@ -207,7 +218,7 @@ void fill_params(const mc_ctx* ctx, RunParams& P) {
     const Tables& t = ctx->tabs;
     P.g = ctx->g;
     P.vox = ctx->d_vox; P.tabP = ctx->d_tabP; P.tabE = ctx->d_tabE;
-    P.N = t.N; P.n_mat = t.n_mat; P.k_cut = t.k_cut;
+    P.N = t.N; P.n_mat = t.n_mat; P.k_cut = t.k_cut; P.e_stride = (int)e_stride(t.N);
     P.lnE0 = (float)t.lnE0; P.dln = (float)t.dln; P.inv_dln = (float)(1.0 / t.dln);
     P.lnE0P = ctx->lnE0P; P.inv_dlnP = ctx->inv_dlnP;
     P.e_cut = ctx->params.e_cut_MeV; P.g_cut = ctx->params.g_cut_MeV;
@@ -446,7 +457,7 @@ mc_status mc_create(const uint8_t* material_idx, const float* density_gcc, const
     *out = nullptr;
     if (!material_idx || !density_gcc || !dims || !voxel_cm || !origin_cm) return MC_ERR_INVALID_ARG;
     for (int a = 0; a < 3; ++a)
-        if (dims[a] <= 0 || !(voxel_cm[a] > 0.0f) || !std::isfinite(voxel_cm[a]) || !std::isfinite(origin_cm[a])) return MC_ERR_INVALID_ARG;
+        if (dims[a] <= 0 || dims[a] > 1024 || !(voxel_cm[a] > 0.0f) || !std::isfinite(voxel_cm[a]) || !std::isfinite(origin_cm[a])) return MC_ERR_INVALID_ARG;
     const uint64_t nvox = (uint64_t)dims[0] * (uint64_t)dims[1] * (uint64_t)dims[2];
     if (nvox >= (1ull << 31)) return MC_ERR_INVALID_ARG;
     for (uint64_t i = 0; i < nvox; ++i)

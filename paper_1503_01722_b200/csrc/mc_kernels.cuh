@@ -59,25 +59,6 @@ __device__ __forceinline__ float face_dist(const Geometry& g, float x, float y, 
     return best;
 }
 
-// Table coordinate (node + fraction) of the energy whose residual range is Rt: exact inverse of the
-// piecewise-linear (in ln T) range interpolant (R5).  The bracket search starts at `guess` (callers pass
-// the constant-L estimate ex + ln(1 - rho d L/T)/dln, which is within a fraction of a node) and needs one shared
-// load per probe: node lo brackets Rt iff 0 <= (Rt - R[lo]) / (R[lo+1] - R[lo]) < 1.
-__device__ __forceinline__ float inv_range_coord(const float2* R, float Rt, float guess, int k_cut, int N) {
-    if (Rt <= 0.0f) return (float)k_cut;
-    int lo = min(max((int)guess, k_cut), N - 2);
-    float f;
-    int way = 0;  // the walk never turns round: a value in the rounding gap between two segments ends it
-    for (;;) {
-        float2 a = R[lo];
-        f = (Rt - a.x) * f_rcp(a.y);
-        if (f < 0.0f && lo > k_cut && way <= 0) { --lo; way = -1; }
-        else if (f >= 1.0f && lo < N - 2 && way >= 0) { ++lo; way = 1; }
-        else break;
-    }
-    return (float)lo + fminf(fmaxf(f, 0.0f), 1.0f);
-}
-
 __device__ __forceinline__ unsigned long long warp_sum(uint32_t v) {
     unsigned long long s = v;
 #pragma unroll
@@ -117,22 +98,24 @@ __device__ __forceinline__ void emit(const RunParams& P, const Queue& q, Score& 
 // =================================================================================================
 // electron / positron kernel
 //
-// One lane = one track.  A warp executes, per iteration, ONE of three blocks for the lanes that want it:
-//   STEP   one condensed-history step (S4-S6, S8)            — lanes in state L_STEP
-//   HARD   hard-event thinning + Moller / bremsstrahlung (S7) — lanes in state L_HARD (pending)
-//   REFILL queue pop / source generation (S0, S1)            — lanes in state L_IDLE
-// Divergent work is deferred until enough lanes of the warp want it (hard_lanes / refill_lanes) or nothing
+// A warp executes, per iteration, ONE of three blocks on up to 32 tracks of its pool that are in the state the block
+// serves:
+//   STEP   one condensed-history step (S4-S6, S8)            — tracks in state L_STEP
+//   HARD   hard-event thinning + Moller / bremsstrahlung (S7) — tracks in state L_HARD (pending)
+//   REFILL queue pop / source generation (S0, S1)            — slots in state L_IDLE
+// Divergent work is deferred until enough tracks of the pool want it (hard_lanes / refill_lanes) or nothing
 // else can run, so the rare blocks run with many lanes instead of one or two (profiles/README.md).
-// Every lane owns kSlots tracks, parked in shared memory (field-major, one bank per lane: conflict-free); a block
-// loads the lane's track that is in the state the block serves, works on it in registers and stores it back.
-// While one track of a lane waits for the HARD block, the lane keeps stepping its other track, so the STEP block
-// runs with nearly all lanes and the rare blocks can wait for nearly full warps.
+// A warp's pool = kSlots x 32 tracks in shared memory, each track kGroups 16-byte groups (one LDS.128 / STS.128 per
+// group: 5 loads and 3-4 stores per step); the fields are grouped by how often they change:
+//   G0 x y z T | G1 u v w msc | G2 acc d_vox block smax | G3 rho tagk vox idx | G4 hist trk_lo trk_hi -
+// (tagk = batch << 6 | material << 2 | charge code; idx = ix | iy << 10 | iz << 20; d_vox = distance to the nearest
+// face along the direction, the only geometric quantity carried from step to step.)
 // =================================================================================================
 // One CTA per SM (the tables are staged once per SM).  kThreadsE = CTA size: 768 (24 warps) when tables + pools fit in
 // the 227 KB of shared memory, else 512 or 256 (more materials / finer grids); instantiated in mc_engine.cu.
 constexpr int kSlots = 2;       // tracks per lane, parked in shared memory between the blocks that work on them
 enum LaneState { L_IDLE = 0, L_STEP = 1, L_HARD = 2, L_DONE = 3 };
-constexpr int kTrackWords = 24;
+constexpr int kGroups = 5;      // 16-byte groups per track
 enum { SE_STEP = 0, SE_MOLLER, SE_BREMS, SE_SEC_E, SE_SEC_G, SE_HIST, SE_RED, SE_COUNT };
 
 // distances along (u,v,w) to the three faces of voxel (ix,iy,iz) the direction points at
@@ -147,87 +130,112 @@ __device__ __forceinline__ void face_all(const Geometry& g, float x, float y, fl
     tz = fabsf(w) > 1e-20f ? c : kInf;
 }
 
+// Table coordinate (node + fraction) of the energy whose residual range is Rt: exact inverse of the piecewise-linear
+// (in ln T) range interpolant (R5).  B[lo] = (R[lo], 1 / (R[lo+1] - R[lo]), K1[lo], K1[lo+1] - K1[lo]): node lo
+// brackets Rt iff 0 <= (Rt - R[lo]) / (R[lo+1] - R[lo]) < 1.  The search starts at `guess` (callers pass the constant-L
+// estimate ex + ln(1 - rho d L/T)/dln, within a fraction of a node): two probes without a branch (the second at the
+// neighbour the first one points to, or at the same node), then — rarely — a walk in the same direction.  The walk
+// never turns round: a value in the rounding gap between two segments ends it.  `node` returns B[lo] of the result and
+// `frac` the fraction inside it (coordinate = lo + frac).
+__device__ __forceinline__ float inv_range_coord(const float4* B, float Rt, float guess, int k_cut, int N, float4& node, float& frac) {
+    int lo = min(max((int)guess, k_cut), N - 2);
+    float4 a = B[lo];
+    float f = (Rt - a.x) * a.y;
+    const int mv = (f < 0.0f && lo > k_cut) ? -1 : ((f >= 1.0f && lo < N - 2) ? 1 : 0);
+    lo += mv;
+    a = B[lo];
+    f = (Rt - a.x) * a.y;
+    while (mv < 0 ? (f < 0.0f && lo > k_cut) : (mv > 0 && f >= 1.0f && lo < N - 2)) {
+        lo += mv;
+        a = B[lo];
+        f = (Rt - a.x) * a.y;
+    }
+    node = a;
+    frac = fminf(fmaxf(f, 0.0f), 1.0f);
+    return (float)lo + frac;
+}
+
 struct ELane {
-    float x, y, z, u, v, w, T, ex, rho, tx, ty, tz, acc, smax;
+    float x, y, z, T, u, v, w;
     float msc;  // R8b: scattering power travelled but not yet sampled for (< 0: sampled ahead)
-    int ix, iy, iz, vox, mat;
-    uint32_t tag;
+    float acc, dvox, smax, rho, ex;
+    int vox;
+    uint32_t idx, tagk;
     Rng rng;
 };
 
 template <int kThreadsE>
 __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_constant__ RunParams P) {
-    extern __shared__ float2 s_tab[];
-    const int ntab = P.n_mat * TE_COUNT * P.N;
-    uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_tab + ntab);           // [SE_COUNT][kThreadsE]
+    extern __shared__ __align__(16) float2 s_tab[];
+    const int ntab = P.n_mat * P.e_stride;
+    uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_tab + ntab);              // [SE_COUNT][kThreadsE]
     double* s_led = reinterpret_cast<double*>(s_cnt + SE_COUNT * kThreadsE);  // [2][kThreadsE]: e_src, e_esc
-    uint32_t* s_trk = reinterpret_cast<uint32_t*>(s_led + 2 * kThreadsE);      // [kTrackWords][kSlots][kThreadsE]
-    uint32_t* s_st = s_trk + kTrackWords * kSlots * kThreadsE;                 // [kSlots][kThreadsE]: slot states
-    uint32_t* s_asg = s_st + kSlots * kThreadsE;                               // [kThreadsE]: per-warp assignment
+    uint4* s_trk = reinterpret_cast<uint4*>(s_led + 2 * kThreadsE);            // [kGroups][kSlots][kThreadsE]
+    uint32_t* s_st = reinterpret_cast<uint32_t*>(s_trk + kGroups * kSlots * kThreadsE);  // [kThreadsE]: byte k = state of slot k
+    uint32_t* s_asg = s_st + kThreadsE;                                        // [kThreadsE]: per-warp assignment
     for (int i = threadIdx.x; i < ntab; i += kThreadsE) s_tab[i] = P.tabE[i];
     const int tid = threadIdx.x;
 #pragma unroll
     for (int k = 0; k < SE_COUNT; ++k) s_cnt[k * kThreadsE + tid] = 0u;
     s_led[tid] = 0.0; s_led[kThreadsE + tid] = 0.0;
+    uint32_t st0 = 0u;  // slots beyond kSlots do not exist: L_DONE
+#pragma unroll
+    for (int k = kSlots; k < 4; ++k) st0 |= (uint32_t)L_DONE << (8 * k);
+    s_st[tid] = st0;
     __syncthreads();
     const int lane = tid & 31;
+    const unsigned lt_mask = (1u << lane) - 1u;
     const int N = P.N, k_cut = P.k_cut;
     const Geometry& g = P.g;
     const bool no_hard = P.flags & 1u, no_ms = P.flags & 2u, local_sec = P.flags & 4u;
-    const float2* const tR = s_tab + TE_R * N;  // + mat * TE_COUNT * N
-    const int mstride = TE_COUNT * N;
     const int KH = P.hard_lanes, KR = P.refill_lanes;
+    constexpr int GS = kSlots * kThreadsE;  // uint4 stride between the groups of a track
 
     int state = L_IDLE;            // state of the track being worked on (L)
-#pragma unroll
-    for (int k = 0; k < kSlots; ++k) s_st[k * kThreadsE + tid] = L_IDLE;
     const int wbase = tid & ~31;   // first thread of this warp: a warp's kSlots x 32 slots form its track pool
-    int slot = 0;                  // pool slot (k * kThreadsE + owner thread) of the track being worked on
+    int slot = 0;                  // pool slot of the track being worked on: owner thread * 4 + k
     uint32_t n_step_w = 0u;
     ELane L;
-    L.x = L.y = L.z = 0.f; L.u = L.v = 0.f; L.w = 1.f; L.T = 0.f; L.ex = 0.f; L.rho = 1.f; L.tx = L.ty = L.tz = 0.f;
-    L.acc = 0.f; L.smax = 0.f; L.msc = 0.f; L.ix = L.iy = L.iz = L.vox = L.mat = 0; L.tag = 0u; L.rng = {0, 0, 0, 0};
-    auto W = [&](int f, int sl) -> uint32_t& { return s_trk[f * (kSlots * kThreadsE) + sl]; };
-    // what = 0: a new track, every word; 1: after a step or a hard event that stayed in its voxel; 2: after a step
-    // that crossed into another voxel.  Identity words (tag, history, track id) never change after birth.
-    auto store_slot = [&](int k, int what) {
-        W(0, k) = __float_as_uint(L.x); W(1, k) = __float_as_uint(L.y); W(2, k) = __float_as_uint(L.z);
-        W(3, k) = __float_as_uint(L.u); W(4, k) = __float_as_uint(L.v); W(5, k) = __float_as_uint(L.w);
-        W(6, k) = __float_as_uint(L.T); W(7, k) = __float_as_uint(L.msc);
-        W(9, k) = __float_as_uint(L.tx); W(10, k) = __float_as_uint(L.ty); W(11, k) = __float_as_uint(L.tz);
-        W(12, k) = __float_as_uint(L.acc); W(23, k) = L.rng.block;
-        if (state == L_HARD) W(13, k) = __float_as_uint(L.smax);
-        if (what != 1) {
-            W(8, k) = __float_as_uint(L.rho);
-            W(14, k) = (uint32_t)L.ix; W(15, k) = (uint32_t)L.iy; W(16, k) = (uint32_t)L.iz; W(17, k) = (uint32_t)L.vox;
-            W(18, k) = (uint32_t)L.mat;
-        }
-        if (what == 0) { W(19, k) = L.tag; W(20, k) = L.rng.hist; W(21, k) = L.rng.trk_lo; W(22, k) = L.rng.trk_hi; }
+    L.x = L.y = L.z = 0.f; L.u = L.v = 0.f; L.w = 1.f; L.T = 0.f; L.ex = 0.f; L.rho = 1.f; L.dvox = 0.f;
+    L.acc = 0.f; L.smax = 0.f; L.msc = 0.f; L.vox = 0; L.idx = 0u; L.tagk = 0u; L.rng = {0, 0, 0, 0};
+    auto trk = [&](int s) -> uint4* { return s_trk + (s & 3) * kThreadsE + (s >> 2); };
+    auto mat_of = [&]() { return (int)((L.tagk >> 2) & 15u); };
+    auto tabA = [&]() { return reinterpret_cast<const float4*>(s_tab + mat_of() * P.e_stride); };
+    // what = 0: a new track, every group; 1: after a step or a hard event that stayed in its voxel; 2: after a step
+    // that crossed into another voxel.  Identity words (history, track id) never change after birth.
+    auto store_slot = [&](int s, int what) {
+        uint4* t = trk(s);
+        t[0] = make_uint4(__float_as_uint(L.x), __float_as_uint(L.y), __float_as_uint(L.z), __float_as_uint(L.T));
+        t[GS] = make_uint4(__float_as_uint(L.u), __float_as_uint(L.v), __float_as_uint(L.w), __float_as_uint(L.msc));
+        t[2 * GS] = make_uint4(__float_as_uint(L.acc), __float_as_uint(L.dvox), L.rng.block, __float_as_uint(L.smax));
+        if (what != 1) t[3 * GS] = make_uint4(__float_as_uint(L.rho), L.tagk, (uint32_t)L.vox, L.idx);
+        if (what == 0) t[4 * GS] = make_uint4(L.rng.hist, L.rng.trk_lo, L.rng.trk_hi, 0u);
     };
-    auto load_slot = [&](int k) {
-        L.x = __uint_as_float(W(0, k)); L.y = __uint_as_float(W(1, k)); L.z = __uint_as_float(W(2, k));
-        L.u = __uint_as_float(W(3, k)); L.v = __uint_as_float(W(4, k)); L.w = __uint_as_float(W(5, k));
-        L.T = __uint_as_float(W(6, k)); L.msc = __uint_as_float(W(7, k)); L.rho = __uint_as_float(W(8, k));
-        L.tx = __uint_as_float(W(9, k)); L.ty = __uint_as_float(W(10, k)); L.tz = __uint_as_float(W(11, k));
-        L.acc = __uint_as_float(W(12, k)); L.smax = __uint_as_float(W(13, k));
-        L.ix = (int)W(14, k); L.iy = (int)W(15, k); L.iz = (int)W(16, k); L.vox = (int)W(17, k);
-        L.mat = (int)W(18, k); L.tag = W(19, k);
+    auto load_slot = [&](int s) {
+        const uint4* t = trk(s);
+        const uint4 a = t[0], b = t[GS], c = t[2 * GS], d = t[3 * GS], e = t[4 * GS];
+        L.x = __uint_as_float(a.x); L.y = __uint_as_float(a.y); L.z = __uint_as_float(a.z); L.T = __uint_as_float(a.w);
+        L.u = __uint_as_float(b.x); L.v = __uint_as_float(b.y); L.w = __uint_as_float(b.z); L.msc = __uint_as_float(b.w);
+        L.acc = __uint_as_float(c.x); L.dvox = __uint_as_float(c.y); L.rng.block = c.z; L.smax = __uint_as_float(c.w);
+        L.rho = __uint_as_float(d.x); L.tagk = d.y; L.vox = (int)d.z; L.idx = d.w;
+        L.rng.hist = e.x; L.rng.trk_lo = e.y; L.rng.trk_hi = e.z;
         L.ex = fmaf(f_lg2(L.T), P.ex_a, -P.ex_b);  // table coordinate of T (not stored)
-        L.rng.hist = W(20, k); L.rng.trk_lo = W(21, k); L.rng.trk_hi = W(22, k); L.rng.block = W(23, k);
     };
     auto park = [&](int what) {  // put the working track back into its pool slot: only live tracks need their data
         if (state == L_STEP || state == L_HARD) store_slot(slot, what);
-        s_st[slot] = (uint32_t)state;
+        reinterpret_cast<volatile uint8_t*>(s_st)[slot] = (uint8_t)state;
     };
     auto bump = [&](int k) { s_cnt[k * kThreadsE + tid] += 1u; };
     auto flush = [&]() {  // one red.global.add.f32 per (track, voxel) visit (S6)
         if (L.acc > 0.0f) {
-            const uint32_t cell = (L.tag >> 2) * (uint32_t)g.nvox + (uint32_t)L.vox;  // n_batches * nvox < 2^32
+            const uint32_t cell = (L.tagk >> 6) * (uint32_t)g.nvox + (uint32_t)L.vox;  // n_batches * nvox < 2^32
             if (P.aggregate) { if (red_add_aggregated(P.edep, cell, L.acc)) bump(SE_RED); }
             else { atomicAdd(P.edep + cell, L.acc); bump(SE_RED); }
         }
         L.acc = 0.0f;
     };
+    auto qtag = [&](uint32_t code) { return ((L.tagk >> 6) << 2) | code; };  // queue-record tag of a secondary
+    auto is_positron = [&]() { return (L.tagk & 3u) == CODE_POSITRON; };
     auto emit_rec = [&](const Queue& q, const QRec& r, int stat) {
         if (local_sec) { L.acc += r.E + (((r.tag & 3u) == CODE_POSITRON) ? 2.0f * kMeF : 0.0f); return; }
         bump(stat);
@@ -236,11 +244,11 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
     // end of track (S8): absorb the remaining kinetic energy; a positron annihilates at rest (R9)
     auto terminate = [&]() {
         L.acc += L.T;
-        if ((L.tag & 3u) == CODE_POSITRON) {
+        if (is_positron()) {
             uint4 a4 = next_block(L.rng, P.seed_lo, P.seed_hi);
             float mu = 2.0f * u01f(a4.z) - 1.0f, sn = f_sqrt(fmaxf(1.0f - mu * mu, 0.0f)), ph = kTwoPiF * u01f(a4.w);
             QRec r; r.x = L.x; r.y = L.y; r.z = L.z; r.u = sn * f_cos(ph); r.v = sn * f_sin(ph); r.w = mu; r.E = kMeF;
-            r.hist = L.rng.hist; r.trk_lo = a4.x; r.trk_hi = a4.y; r.vox = L.vox; r.tag = (L.tag & ~3u) | CODE_PHOTON;
+            r.hist = L.rng.hist; r.trk_lo = a4.x; r.trk_hi = a4.y; r.vox = L.vox; r.tag = qtag(CODE_PHOTON);
             emit_rec(P.q_p_out, r, SE_SEC_G);
             uint4 b4 = next_block(L.rng, P.seed_lo, P.seed_hi);
             r.u = -r.u; r.v = -r.v; r.w = -r.w; r.trk_lo = b4.x; r.trk_hi = b4.y;
@@ -249,29 +257,35 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         flush();
         state = L_IDLE;
     };
+    // d_vox of the track where it stands (after a change of direction)
+    auto set_dvox = [&]() {
+        float tx, ty, tz;
+        face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, (int)(L.idx & 1023u), (int)((L.idx >> 10) & 1023u), (int)(L.idx >> 20), tx, ty, tz);
+        L.dvox = fminf(tx, fminf(ty, tz));
+    };
 
     for (;;) {
         // ---- scheduling: count the pool's tracks by state, choose ONE block, hand its tracks to the lanes ------
-        unsigned ms[kSlots], mh[kSlots], mi[kSlots];
-        int ns = 0, nh = 0, ni = 0;
+        // byte k of a lane's state word = state of its slot k; one-hot byte counters summed over the warp (REDUX)
+        const uint32_t sw = s_st[tid];
+        uint32_t cnt1 = 0u;
 #pragma unroll
-        for (int k = 0; k < kSlots; ++k) {
-            const uint32_t sk = s_st[k * kThreadsE + tid];
-            ms[k] = __ballot_sync(kFull, sk == L_STEP); mh[k] = __ballot_sync(kFull, sk == L_HARD);
-            mi[k] = __ballot_sync(kFull, sk == L_IDLE);
-            ns += __popc(ms[k]); nh += __popc(mh[k]); ni += __popc(mi[k]);
-        }
-        if ((ns | nh | ni) == 0) break;
+        for (int k = 0; k < kSlots; ++k) cnt1 += 1u << (8u * ((sw >> (8 * k)) & 3u));
+        const uint32_t tot = __reduce_add_sync(kFull, cnt1);
+        const int ni = (int)(tot & 0xffu), ns = (int)((tot >> 8) & 0xffu), nh = (int)((tot >> 16) & 0xffu);
+        if ((tot & 0xffffffu) == 0u) break;
         // a rare block runs when it can fill a warp (>= KH / KR tracks), or when it has more tracks than STEP
         const bool do_hard = nh >= KH || (nh > ns && nh >= ni);
         const bool do_refill = !do_hard && (ni >= KR || ni > ns);
+        const uint32_t cs = do_hard ? (uint32_t)L_HARD : (do_refill ? (uint32_t)L_IDLE : (uint32_t)L_STEP);
         // the r-th track of the chosen state (slot-major, then owner lane) goes to lane r: its owner posts the slot
         int rank = 0;
 #pragma unroll
         for (int k = 0; k < kSlots; ++k) {
-            const unsigned m = do_hard ? mh[k] : (do_refill ? mi[k] : ms[k]);
-            const int r = rank + __popc(m & ((1u << lane) - 1u));
-            if (((m >> lane) & 1u) && r < 32) s_asg[wbase + r] = (uint32_t)(k * kThreadsE + tid);
+            const bool mine = ((sw >> (8 * k)) & 0xffu) == cs;
+            const unsigned m = __ballot_sync(kFull, mine);
+            const int r = rank + __popc(m & lt_mask);
+            if (mine && r < 32) s_asg[wbase + r] = (uint32_t)(tid * 4 + k);
             rank += __popc(m);
         }
         __syncwarp();
@@ -283,14 +297,16 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
             // ---- REFILL: queue first, then new primaries (S0, S1) --------------------------------
             uint32_t item = claim(P.counters + C_HEAD, n_work >= 32 ? kFull : ((1u << n_work) - 1u), lane);
             if (have) {
-                state = L_IDLE; L.acc = 0.0f; L.msc = 0.0f;
+                state = L_IDLE; L.acc = 0.0f; L.msc = 0.0f; L.smax = 0.0f;
                 bool ok = false;
+                uint32_t qt = 0u;
+                int ix = 0, iy = 0, iz = 0;
                 if (item < P.n_in) {
                     QRec r = load_record(P.q_in, item);
                     L.x = r.x; L.y = r.y; L.z = r.z; L.u = r.u; L.v = r.v; L.w = r.w; L.T = r.E;
                     L.rng.hist = r.hist; L.rng.trk_lo = r.trk_lo; L.rng.trk_hi = r.trk_hi; L.rng.block = 0;
-                    L.vox = r.vox; L.tag = r.tag;
-                    L.ix = L.vox % g.nx; int t2 = L.vox / g.nx; L.iy = t2 % g.ny; L.iz = t2 / g.ny;
+                    L.vox = r.vox; qt = r.tag;
+                    ix = L.vox % g.nx; int t2 = L.vox / g.nx; iy = t2 % g.ny; iz = t2 / g.ny;
                     ok = true;
                 } else if (item < P.n_in + P.n_new) {
                     unsigned long long h = P.h_first + (item - P.n_in);
@@ -298,22 +314,21 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
                     uint4 w4 = next_block(L.rng, P.seed_lo, P.seed_hi);
                     Primary p = sample_primary<false>(P, w4);
                     uint32_t code = P.beam.particle > 0 ? CODE_POSITRON : CODE_ELECTRON;
-                    L.tag = (batch_of(h, P.n_batches, P.n_total, P.inv_n_total) << 2) | code;
+                    qt = (batch_of(h, P.n_batches, P.n_total, P.inv_n_total) << 2) | code;
                     float e0 = p.E + (code == CODE_POSITRON ? 2.0f * kMeF : 0.0f);
                     s_led[tid] += (double)e0; bump(SE_HIST);
                     L.x = p.x; L.y = p.y; L.z = p.z; L.u = p.u; L.v = p.v; L.w = p.w; L.T = p.E;
-                    L.ix = p.ix; L.iy = p.iy; L.iz = p.iz; L.vox = L.ix + g.nx * (L.iy + g.ny * L.iz);
+                    ix = p.ix; iy = p.iy; iz = p.iz; L.vox = ix + g.nx * (iy + g.ny * iz);
                     if (p.inside) ok = true; else s_led[kThreadsE + tid] += (double)e0;
                 } else state = L_DONE;
                 if (ok) {
                     uint2 vd = P.vox[L.vox];
-                    L.rho = __uint_as_float(vd.x); L.mat = (int)vd.y;
+                    L.rho = __uint_as_float(vd.x);
+                    L.tagk = ((qt >> 2) << 6) | (vd.y << 2) | (qt & 3u);
+                    L.idx = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20);
                     state = L_STEP;
                     if (L.T <= P.e_cut) terminate();  // born at or below the cut-off (pair electrons)
-                    else {
-                        L.ex = fmaf(f_lg2(L.T), P.ex_a, -P.ex_b);
-                        face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, L.ix, L.iy, L.iz, L.tx, L.ty, L.tz);
-                    }
+                    else set_dvox();
                 }
                 park(0);  // L_DONE (nothing left to claim) retires the slot
             }
@@ -328,12 +343,12 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
             if (have) {
                 load_slot(slot);
                 state = L_STEP;
-                const float2* tm = tR + L.mat * mstride;
                 uint4 h4 = next_block(L.rng, P.seed_lo, P.seed_hi);
                 const float r = u01f(h4.x) * L.smax;
                 int i1 = min(max((int)L.ex, 0), N - 2);
                 float f1 = L.ex - (float)i1;
-                const float SH = lerp(tm + (TE_SHARD - TE_R) * N, i1, f1), SM = lerp(tm + (TE_SM - TE_R) * N, i1, f1);
+                const float4 hd = (tabA() + 2 * N)[i1];  // (S_hard, slope, S_Moller, slope)
+                const float SH = fmaf(f1, hd.y, hd.x), SM = fmaf(f1, hd.w, hd.z);
                 if (r < SH) {
                     const bool mol = r < SM;
                     const float T0 = L.T;
@@ -348,7 +363,7 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
                         float ec = f_rcp(ca), o = f_rcp(1.0f - ec);
                         cm = fmaxf(1.0f - cb * ec * o + ec * ec * (cc + o * o), 1.0f - cb + 0.25f * (cc + 4.0f));  // max(g(e_c), g(1/2))
                     } else {
-                        cb = f_rcp(Et); cc = P.lscr[L.mat];
+                        cb = f_rcp(Et); cc = P.lscr[mat_of()];
                         ca = f_lg2(T0 * f_rcp(P.g_cut));
                         cm = (4.0f / 3.0f) * (fminf(f_ln(2.0f * Et * (Et - P.g_cut) * f_rcp(kMeF * P.g_cut)), cc) - 0.5f);
                     }
@@ -380,16 +395,16 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
                         const float W = val * T0, Tp = T0 - W, t2m = T0 + 2.0f * kMeF;
                         const float c1 = f_sqrt(Tp * t2m * f_rcp(T0 * (Tp + 2.0f * kMeF)));
                         omu_q = 1.0f - f_sqrt(W * t2m * f_rcp(T0 * (W + 2.0f * kMeF)));
-                        q.E = W; q.tag = (L.tag & ~3u) | CODE_ELECTRON;
+                        q.E = W; q.tag = qtag(CODE_ELECTRON);
                         rotate_fast(L.u, L.v, L.w, 1.0f - c1, sphi, cphi);
-                        face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, L.ix, L.iy, L.iz, L.tx, L.ty, L.tz);
+                        set_dvox();
                         sphi = -sphi; cphi = -cphi;  // the delta ray leaves at azimuth phi + pi
                         L.T = Tp;
                     } else {
                         bump(SE_BREMS);
                         const float sh = f_sin(0.5f * kMeF * cb);
                         omu_q = 2.0f * sh * sh;  // polar angle mc^2 / (T0 + mc^2)
-                        q.E = val; q.tag = (L.tag & ~3u) | CODE_PHOTON;
+                        q.E = val; q.tag = qtag(CODE_PHOTON);
                         L.T = T0 - val;
                     }
                     rotate_fast(q.u, q.v, q.w, omu_q, sphi, cphi);
@@ -399,7 +414,6 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
                         push_record2(P.q_e_out, P.q_p_out, mol, P.counters + C_OVERFLOW, q);
                     }
                     if (L.T <= P.e_cut) terminate();
-                    else L.ex = fmaf(f_lg2(L.T), P.ex_a, -P.ex_b);
                 }
                 park(1);
             }
@@ -412,13 +426,16 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         load_slot(slot);
         state = L_STEP;
         // ---- STEP set-up (S4): d = min[d_vox, d_maxs, d_maxe, d_range, d_event] ------------------------------
-        const float2* tm = tR + L.mat * mstride;
+        const float4* const tA = tabA();  // [N] (R, slope, L, slope) | [N] inverse-range pack | [N] hard pack | [N] float2 S_max
+        const float4* const tB = tA + N;
         int i0 = min(max((int)L.ex, 0), N - 2);
         float f0 = L.ex - (float)i0;
-        float R0 = lerp(tm, i0, f0), L0 = lerp(tm + (TE_L - TE_R) * N, i0, f0), Smax = lerp(tm + (TE_SMAX - TE_R) * N, i0, f0);
+        const float4 a0 = tA[i0];
+        const float2 s0 = reinterpret_cast<const float2*>(tA + 3 * N)[i0];
+        const float R0 = fmaf(f0, a0.y, a0.x), L0 = fmaf(f0, a0.w, a0.z), Smax = fmaf(f0, s0.y, s0.x);
         uint4 w4 = next_block(L.rng, P.seed_lo, P.seed_hi);
         const float rho = L.rho, irho = f_rcp(rho);
-        const float d_vox = fminf(L.tx, fminf(L.ty, L.tz));
+        const float d_vox = L.dvox;
         float d_lim = P.d_maxs;  // the non-geometric limits
         int lim = 1;
         const float d_maxe = P.f_maxe * L.T * irho * f_rcp(L0);
@@ -436,12 +453,12 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         L.x = fmaf(legA, L.u, L.x); L.y = fmaf(legA, L.v, L.y); L.z = fmaf(legA, L.w, L.z);
         const float xl = rho * L0 * f_rcp(L.T);  // fractional energy loss per unit path at constant L (search guess only)
         const float rd = rho * d;
-        bool turned = false;
         float k1rho = 0.0f;
+        float4 nd;
+        float fm;
         if (!no_ms) {
-            float em = inv_range_coord(tm, fmaf(-0.5f, rd, R0), fmaf(f_lg2(fmaf(-0.5f * d, xl, 1.0f)), P.ex_a, L.ex), k_cut, N);
-            int im = min(max((int)em, 0), N - 2);
-            k1rho = lerp(tm + (TE_K1 - TE_R) * N, im, em - (float)im) * rho;
+            inv_range_coord(tB, fmaf(-0.5f, rd, R0), fmaf(f_lg2(fmaf(-0.5f * d, xl, 1.0f)), P.ex_a, L.ex), k_cut, N, nd, fm);
+            k1rho = fmaf(fm, nd.w, nd.z) * rho;  // K1 at the mid-step energy: its node is the one the search ended on
             // R8b: sample for the planned path plus the path travelled but not yet sampled for; never a negative path
             const float tq = fmaf(k1rho, d, P.ms_carry ? L.msc : 0.0f), t = fmaxf(tq, 0.0f);
             L.msc = tq - t;
@@ -450,58 +467,60 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
                 float omu = -am * kLn2F * f_lg2(1.0f - u01f(w4.z) * (1.0f - f_exp(-2.0f * f_rcp(am))));
                 float phi = kTwoPiF * u01f(w4.w);
                 rotate_fast(L.u, L.v, L.w, fminf(omu, 2.0f), f_sin(phi), f_cos(phi));
-                turned = true;
             }
         }
-        if (turned) face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, L.ix, L.iy, L.iz, L.tx, L.ty, L.tz);
-        else { L.tx -= legA; L.ty -= legA; L.tz -= legA; }
+        int ix = (int)(L.idx & 1023u), iy = (int)((L.idx >> 10) & 1023u), iz = (int)(L.idx >> 20);
+        float tx, ty, tz;
+        face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, ix, iy, iz, tx, ty, tz);
         const float rest = d - legA;
         int ax = 0;
-        float tf = L.tx;
-        if (L.ty < tf) { tf = L.ty; ax = 1; }
-        if (L.tz < tf) { tf = L.tz; ax = 2; }
-        // R8: a voxel-limited step may run on to the face by up to kHingeOverrun of the planned second leg, never
+        float tf = tx;
+        if (ty < tf) { tf = ty; ax = 1; }
+        if (tz < tf) { tf = tz; ax = 2; }
+        // R8: a voxel-limited step may run on to the face by up to hinge_overrun of the planned second leg, never
         // beyond the non-geometric limits (removes the tiny catch-up steps after half of the voxel-limited steps)
         const bool cross = tf <= fmaxf(fminf((1.0f + P.hinge_overrun) * rest, d_lim - legA), rest);
         const float legB = cross ? tf : rest;
         L.x = fmaf(legB, L.u, L.x); L.y = fmaf(legB, L.v, L.y); L.z = fmaf(legB, L.w, L.z);
-        L.tx = fmaxf(L.tx - legB, 0.0f); L.ty = fmaxf(L.ty - legB, 0.0f); L.tz = fmaxf(L.tz - legB, 0.0f);
+        tx = fmaxf(tx - legB, 0.0f); ty = fmaxf(ty - legB, 0.0f); tz = fmaxf(tz - legB, 0.0f);
         const float d_act = legA + legB;
         L.msc = fmaf(k1rho, d_act - d, L.msc);
         // ---- CSDA loss through the range table (S6; R5) + scoring ------------------------------------------
-        float T1, ex1;
-        if (lim == 3 && !cross) { T1 = P.e_cut; ex1 = (float)k_cut; }
+        float T1;
+        if (lim == 3 && !cross) T1 = P.e_cut;
         else {
-            ex1 = inv_range_coord(tm, fmaf(-rho, d_act, R0), fmaf(f_lg2(fmaxf(fmaf(-d_act, xl, 1.0f), 1e-3f)), P.ex_a, L.ex), k_cut, N);
+            const float ex1 = inv_range_coord(tB, fmaf(-rho, d_act, R0), fmaf(f_lg2(fmaxf(fmaf(-d_act, xl, 1.0f), 1e-3f)), P.ex_a, L.ex), k_cut, N, nd, fm);
             T1 = fminf(f_ex2(fmaf(ex1, P.t_a, P.t_b)), L.T);
         }
         L.acc += L.T - T1;
-        L.T = T1; L.ex = ex1;
+        L.T = T1;
         if (cross) {
             // leave the voxel: flush its deposit, move to the neighbour, coordinate snapped to the face (R8).
             // Written with one predicate per axis so that it compiles to selects, not to a 3-way branch.
             flush();
-            const bool a0 = ax == 0, a1 = ax == 1, a2 = ax == 2;
-            const float dc = a0 ? L.u : (a1 ? L.v : L.w);
+            const bool a0x = ax == 0, a1x = ax == 1, a2x = ax == 2;
+            const float dc = a0x ? L.u : (a1x ? L.v : L.w);
             const int dir = dc > 0.0f ? 1 : -1, up = dc > 0.0f ? 1 : 0;
-            const float tnew = (a0 ? g.hx : (a1 ? g.hy : g.hz)) * f_rcp(fabsf(dc));
+            const float tnew = (a0x ? g.hx : (a1x ? g.hy : g.hz)) * f_rcp(fabsf(dc));
             // the face that was hit is the one the direction points at
-            const float fx = fmaf((float)(L.ix + up), g.hx, g.ox), fy = fmaf((float)(L.iy + up), g.hy, g.oy),
-                        fz = fmaf((float)(L.iz + up), g.hz, g.oz);
-            L.x = a0 ? fx : L.x; L.y = a1 ? fy : L.y; L.z = a2 ? fz : L.z;
-            L.tx = a0 ? tnew : L.tx; L.ty = a1 ? tnew : L.ty; L.tz = a2 ? tnew : L.tz;
-            L.ix += a0 ? dir : 0; L.iy += a1 ? dir : 0; L.iz += a2 ? dir : 0;
-            L.vox += dir * (a0 ? 1 : (a1 ? g.nx : g.nx * g.ny));
-            if ((unsigned)L.ix >= (unsigned)g.nx || (unsigned)L.iy >= (unsigned)g.ny || (unsigned)L.iz >= (unsigned)g.nz) {
-                s_led[kThreadsE + tid] += (double)(L.T + ((L.tag & 3u) == CODE_POSITRON ? 2.0f * kMeF : 0.0f));
+            const float fx = fmaf((float)(ix + up), g.hx, g.ox), fy = fmaf((float)(iy + up), g.hy, g.oy),
+                        fz = fmaf((float)(iz + up), g.hz, g.oz);
+            L.x = a0x ? fx : L.x; L.y = a1x ? fy : L.y; L.z = a2x ? fz : L.z;
+            tx = a0x ? tnew : tx; ty = a1x ? tnew : ty; tz = a2x ? tnew : tz;
+            ix += a0x ? dir : 0; iy += a1x ? dir : 0; iz += a2x ? dir : 0;
+            L.vox += dir * (a0x ? 1 : (a1x ? g.nx : g.nx * g.ny));
+            if ((unsigned)ix >= (unsigned)g.nx || (unsigned)iy >= (unsigned)g.ny || (unsigned)iz >= (unsigned)g.nz) {
+                s_led[kThreadsE + tid] += (double)(L.T + (is_positron() ? 2.0f * kMeF : 0.0f));
                 state = L_IDLE;
             } else {
+                L.idx = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20);
                 uint2 vd = P.vox[L.vox];
-                L.rho = __uint_as_float(vd.x); L.mat = (int)vd.y;
+                L.rho = __uint_as_float(vd.x); L.tagk = (L.tagk & ~60u) | (vd.y << 2);
                 if (L.T <= P.e_cut) terminate();
             }
         } else if (L.T <= P.e_cut) terminate();
         else if (lim == 4) { state = L_HARD; L.smax = Smax; }
+        L.dvox = fminf(tx, fminf(ty, tz));
         park(cross ? 2 : 1);
         __syncwarp();
     }
