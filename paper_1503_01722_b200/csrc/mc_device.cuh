@@ -89,6 +89,7 @@ struct RunParams {
     int hard_lanes;           // lanes of a warp that must hold a pending hard event before the warp runs that block
     // table coordinate <-> energy in base 2: ex = lg2(T) * ex_a - ex_b;  T = ex2(ex * t_a + t_b)
     float ex_a, ex_b, t_a, t_b;
+    uint32_t seed_rk[10];     // seed_lo + r * 0xBB67AE85: Philox round keys of the second key word
     float hinge_overrun;      // DESIGN.md R8
     int ms_carry;             // DESIGN.md R8b
 };
@@ -107,8 +108,25 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
     }
     return make_uint4(c0, c1, c2, c3);
 }
+// Same generator with the round keys of the second key word (seed_lo + r * 0xBB67AE85, launch constants) read from
+// `rk` instead of being recomputed per block.
+__device__ __forceinline__ uint4 philox4x32_10_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, const uint32_t (&rk)[10]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        c0 = h1 ^ c1 ^ k0; c1 = l1; c2 = h0 ^ c3 ^ rk[r]; c3 = l0;
+        k0 += 0x9E3779B9u;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
 __device__ __forceinline__ uint4 next_block(Rng& r, uint32_t seed_lo, uint32_t seed_hi) {
     uint4 w = philox4x32_10(r.block, r.trk_lo, r.trk_hi, seed_hi, r.hist, seed_lo);
+    ++r.block;
+    return w;
+}
+__device__ __forceinline__ uint4 next_block_rk(Rng& r, const RunParams& P) {
+    uint4 w = philox4x32_10_rk(r.block, r.trk_lo, r.trk_hi, P.seed_hi, r.hist, P.seed_rk);
     ++r.block;
     return w;
 }

@@ -141,8 +141,8 @@ mc_status upload_tables(mc_ctx* ctx) {
 
 // shared memory of a transport CTA of T threads: tables + per-thread counters + per-thread energy ledger + track pool
 size_t smem_e(const mc_ctx* c, int T) {
-    return (size_t)c->tabs.n_mat * e_stride(c->tabs.N) * sizeof(float2) + (size_t)SE_COUNT * T * sizeof(uint32_t) +
-           2 * (size_t)T * sizeof(double) + (size_t)kGroups * kSlots * T * sizeof(uint4) + 2 * (size_t)T * sizeof(uint32_t);
+    return (size_t)c->tabs.n_mat * e_stride(c->tabs.N) * sizeof(float2) + (size_t)kGroups * kSlots * T * sizeof(uint4) +
+           2 * (size_t)T * sizeof(uint32_t) + (size_t)(T / 32) * (2 * sizeof(double) + 8 * sizeof(uint32_t));
 }
 size_t smem_p(const mc_ctx* c, int T) {
     return (size_t)(1 + c->tabs.n_mat * TP_COUNT) * c->tabs.N * sizeof(float2) + (size_t)SP_COUNT * T * sizeof(uint32_t) +
@@ -153,9 +153,9 @@ using TransportKernel = void (*)(const RunParams);
 struct KernelChoice { TransportKernel fn; int threads; size_t smem; };
 // the largest CTA whose tables + pools fit (more materials or a finer grid leave less room for the pools)
 bool choose_electron_kernel(const mc_ctx* c, KernelChoice& k) {
-    const int T[3] = {768, 512, 256};
-    const TransportKernel fn[3] = {electron_kernel<768>, electron_kernel<512>, electron_kernel<256>};
-    for (int i = 0; i < 3; ++i)
+    const int T[4] = {1024, 768, 512, 256};
+    const TransportKernel fn[4] = {electron_kernel<1024>, electron_kernel<768>, electron_kernel<512>, electron_kernel<256>};
+    for (int i = 0; i < 4; ++i)
         if (smem_e(c, T[i]) <= kSmemMax) { k = KernelChoice{fn[i], T[i], smem_e(c, T[i])}; return true; }
     return false;
 }
@@ -303,6 +303,7 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
     P.edep = d_edep; P.n_total = n_total; P.n_batches = n_batches;
     P.inv_n_total = n_total > 1 ? (unsigned long long)((((unsigned __int128)1) << 64) / n_total) : ~0ull;
     P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) P.seed_rk[r] = P.seed_lo + (uint32_t)r * 0xBB67AE85u;
 
     const bool photon_beam = beam && beam->particle == MC_PHOTON;
     uint64_t remaining = n_run, h_next = h0;

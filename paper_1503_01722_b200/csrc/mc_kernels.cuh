@@ -65,6 +65,11 @@ __device__ __forceinline__ unsigned long long warp_sum(uint32_t v) {
     for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(kFull, s, o);
     return s;
 }
+__device__ __forceinline__ float warp_sum_f(float v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+    return v;
+}
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
     for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
@@ -108,8 +113,9 @@ __device__ __forceinline__ void emit(const RunParams& P, const Queue& q, Score& 
 // A warp's pool = kSlots x 32 tracks in shared memory, each track kGroups 16-byte groups (one LDS.128 / STS.128 per
 // group: 5 loads and 3-4 stores per step); the fields are grouped by how often they change:
 //   G0 x y z T | G1 u v w msc | G2 acc d_vox block smax | G3 rho tagk vox idx | G4 hist trk_lo trk_hi -
-// (tagk = batch << 6 | material << 2 | charge code; idx = ix | iy << 10 | iz << 20; d_vox = distance to the nearest
-// face along the direction, the only geometric quantity carried from step to step.)
+// (x, y, z = position relative to the low corner of the track's voxel; tagk = batch << 6 | material << 2 | charge code;
+// idx = ix | iy << 10 | iz << 20; d_vox = distance to the nearest face along the direction, the only geometric
+// quantity carried from step to step.)
 // =================================================================================================
 // One CTA per SM (the tables are staged once per SM).  kThreadsE = CTA size: 768 (24 warps) when tables + pools fit in
 // the 227 KB of shared memory, else 512 or 256 (more materials / finer grids); instantiated in mc_engine.cu.
@@ -118,12 +124,11 @@ enum LaneState { L_IDLE = 0, L_STEP = 1, L_HARD = 2, L_DONE = 3 };
 constexpr int kGroups = 5;      // 16-byte groups per track
 enum { SE_STEP = 0, SE_MOLLER, SE_BREMS, SE_SEC_E, SE_SEC_G, SE_HIST, SE_RED, SE_COUNT };
 
-// distances along (u,v,w) to the three faces of voxel (ix,iy,iz) the direction points at
-__device__ __forceinline__ void face_all(const Geometry& g, float x, float y, float z, float u, float v, float w, int ix, int iy,
-                                         int iz, float& tx, float& ty, float& tz) {
-    float px = fmaf((float)(ix + (u > 0.0f ? 1 : 0)), g.hx, g.ox);
-    float py = fmaf((float)(iy + (v > 0.0f ? 1 : 0)), g.hy, g.oy);
-    float pz = fmaf((float)(iz + (w > 0.0f ? 1 : 0)), g.hz, g.oz);
+// distances along (u,v,w) to the three faces of the voxel the direction points at; (x,y,z) = position relative to the
+// voxel's low corner
+__device__ __forceinline__ void face_all(const Geometry& g, float x, float y, float z, float u, float v, float w, float& tx, float& ty,
+                                         float& tz) {
+    float px = u > 0.0f ? g.hx : 0.0f, py = v > 0.0f ? g.hy : 0.0f, pz = w > 0.0f ? g.hz : 0.0f;
     float a = fmaxf((px - x) * f_rcp(u), 0.0f), b = fmaxf((py - y) * f_rcp(v), 0.0f), c = fmaxf((pz - z) * f_rcp(w), 0.0f);
     tx = fabsf(u) > 1e-20f ? a : kInf;
     ty = fabsf(v) > 1e-20f ? b : kInf;
@@ -145,10 +150,13 @@ __device__ __forceinline__ float inv_range_coord(const float4* B, float Rt, floa
     lo += mv;
     a = B[lo];
     f = (Rt - a.x) * a.y;
-    while (mv < 0 ? (f < 0.0f && lo > k_cut) : (mv > 0 && f >= 1.0f && lo < N - 2)) {
-        lo += mv;
-        a = B[lo];
-        f = (Rt - a.x) * a.y;
+    if (mv != 0) {  // rarely taken further than the neighbour
+        const int stop = mv < 0 ? k_cut : N - 2;
+        while ((mv < 0 ? f < 0.0f : f >= 1.0f) && lo != stop) {
+            lo += mv;
+            a = B[lo];
+            f = (Rt - a.x) * a.y;
+        }
     }
     node = a;
     frac = fminf(fmaxf(f, 0.0f), 1.0f);
@@ -168,16 +176,16 @@ template <int kThreadsE>
 __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_constant__ RunParams P) {
     extern __shared__ __align__(16) float2 s_tab[];
     const int ntab = P.n_mat * P.e_stride;
-    uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_tab + ntab);              // [SE_COUNT][kThreadsE]
-    double* s_led = reinterpret_cast<double*>(s_cnt + SE_COUNT * kThreadsE);  // [2][kThreadsE]: e_src, e_esc
-    uint4* s_trk = reinterpret_cast<uint4*>(s_led + 2 * kThreadsE);            // [kGroups][kSlots][kThreadsE]
+    constexpr int kWarps = kThreadsE / 32;
+    uint4* s_trk = reinterpret_cast<uint4*>(s_tab + ntab);                     // [kGroups][kSlots][kThreadsE]
     uint32_t* s_st = reinterpret_cast<uint32_t*>(s_trk + kGroups * kSlots * kThreadsE);  // [kThreadsE]: byte k = state of slot k
     uint32_t* s_asg = s_st + kThreadsE;                                        // [kThreadsE]: per-warp assignment
+    double* s_led = reinterpret_cast<double*>(s_asg + kThreadsE);              // [kWarps][2]: e_src, e_esc of the warp
+    uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_led + 2 * kWarps);         // [kWarps][8]: event counters of the warp
     for (int i = threadIdx.x; i < ntab; i += kThreadsE) s_tab[i] = P.tabE[i];
     const int tid = threadIdx.x;
-#pragma unroll
-    for (int k = 0; k < SE_COUNT; ++k) s_cnt[k * kThreadsE + tid] = 0u;
-    s_led[tid] = 0.0; s_led[kThreadsE + tid] = 0.0;
+    if (tid < 8 * kWarps) s_cnt[tid] = 0u;
+    if (tid < 2 * kWarps) s_led[tid] = 0.0;
     uint32_t st0 = 0u;  // slots beyond kSlots do not exist: L_DONE
 #pragma unroll
     for (int k = kSlots; k < 4; ++k) st0 |= (uint32_t)L_DONE << (8 * k);
@@ -225,7 +233,9 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         if (state == L_STEP || state == L_HARD) store_slot(slot, what);
         reinterpret_cast<volatile uint8_t*>(s_st)[slot] = (uint8_t)state;
     };
-    auto bump = [&](int k) { s_cnt[k * kThreadsE + tid] += 1u; };
+    uint32_t* const w_cnt = s_cnt + 8 * (tid >> 5);  // this warp's counters (shared-memory atomics: lanes bump them in divergent code)
+    double* const w_led = s_led + 2 * (tid >> 5);
+    auto bump = [&](int k) { atomicAdd(w_cnt + k, 1u); };
     auto flush = [&]() {  // one red.global.add.f32 per (track, voxel) visit (S6)
         if (L.acc > 0.0f) {
             const uint32_t cell = (L.tagk >> 6) * (uint32_t)g.nvox + (uint32_t)L.vox;  // n_batches * nvox < 2^32
@@ -236,6 +246,12 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
     };
     auto qtag = [&](uint32_t code) { return ((L.tagk >> 6) << 2) | code; };  // queue-record tag of a secondary
     auto is_positron = [&]() { return (L.tagk & 3u) == CODE_POSITRON; };
+    // a secondary is born where the track stands: world coordinates for the queue record
+    auto born_here = [&](QRec& r) {
+        r.x = fmaf((float)(L.idx & 1023u), g.hx, g.ox) + L.x; r.y = fmaf((float)((L.idx >> 10) & 1023u), g.hy, g.oy) + L.y;
+        r.z = fmaf((float)(L.idx >> 20), g.hz, g.oz) + L.z;
+        r.hist = L.rng.hist; r.vox = L.vox;
+    };
     auto emit_rec = [&](const Queue& q, const QRec& r, int stat) {
         if (local_sec) { L.acc += r.E + (((r.tag & 3u) == CODE_POSITRON) ? 2.0f * kMeF : 0.0f); return; }
         bump(stat);
@@ -245,12 +261,12 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
     auto terminate = [&]() {
         L.acc += L.T;
         if (is_positron()) {
-            uint4 a4 = next_block(L.rng, P.seed_lo, P.seed_hi);
+            uint4 a4 = next_block_rk(L.rng, P);
             float mu = 2.0f * u01f(a4.z) - 1.0f, sn = f_sqrt(fmaxf(1.0f - mu * mu, 0.0f)), ph = kTwoPiF * u01f(a4.w);
-            QRec r; r.x = L.x; r.y = L.y; r.z = L.z; r.u = sn * f_cos(ph); r.v = sn * f_sin(ph); r.w = mu; r.E = kMeF;
-            r.hist = L.rng.hist; r.trk_lo = a4.x; r.trk_hi = a4.y; r.vox = L.vox; r.tag = qtag(CODE_PHOTON);
+            QRec r; born_here(r); r.u = sn * f_cos(ph); r.v = sn * f_sin(ph); r.w = mu; r.E = kMeF;
+            r.trk_lo = a4.x; r.trk_hi = a4.y; r.tag = qtag(CODE_PHOTON);
             emit_rec(P.q_p_out, r, SE_SEC_G);
-            uint4 b4 = next_block(L.rng, P.seed_lo, P.seed_hi);
+            uint4 b4 = next_block_rk(L.rng, P);
             r.u = -r.u; r.v = -r.v; r.w = -r.w; r.trk_lo = b4.x; r.trk_hi = b4.y;
             emit_rec(P.q_p_out, r, SE_SEC_G);
         }
@@ -260,7 +276,7 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
     // d_vox of the track where it stands (after a change of direction)
     auto set_dvox = [&]() {
         float tx, ty, tz;
-        face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, (int)(L.idx & 1023u), (int)((L.idx >> 10) & 1023u), (int)(L.idx >> 20), tx, ty, tz);
+        face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, tx, ty, tz);
         L.dvox = fminf(tx, fminf(ty, tz));
     };
 
@@ -296,6 +312,7 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         if (do_refill) {
             // ---- REFILL: queue first, then new primaries (S0, S1) --------------------------------
             uint32_t item = claim(P.counters + C_HEAD, n_work >= 32 ? kFull : ((1u << n_work) - 1u), lane);
+            float e_new = 0.0f, e_out = 0.0f;  // source energy of the new primaries / of those that miss the phantom
             if (have) {
                 state = L_IDLE; L.acc = 0.0f; L.msc = 0.0f; L.smax = 0.0f;
                 bool ok = false;
@@ -311,21 +328,25 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
                 } else if (item < P.n_in + P.n_new) {
                     unsigned long long h = P.h_first + (item - P.n_in);
                     L.rng.hist = (uint32_t)h; L.rng.trk_lo = 0; L.rng.trk_hi = 0; L.rng.block = 0;
-                    uint4 w4 = next_block(L.rng, P.seed_lo, P.seed_hi);
+                    uint4 w4 = next_block_rk(L.rng, P);
                     Primary p = sample_primary<false>(P, w4);
                     uint32_t code = P.beam.particle > 0 ? CODE_POSITRON : CODE_ELECTRON;
                     qt = (batch_of(h, P.n_batches, P.n_total, P.inv_n_total) << 2) | code;
                     float e0 = p.E + (code == CODE_POSITRON ? 2.0f * kMeF : 0.0f);
-                    s_led[tid] += (double)e0; bump(SE_HIST);
+                    e_new = e0;
                     L.x = p.x; L.y = p.y; L.z = p.z; L.u = p.u; L.v = p.v; L.w = p.w; L.T = p.E;
                     ix = p.ix; iy = p.iy; iz = p.iz; L.vox = ix + g.nx * (iy + g.ny * iz);
-                    if (p.inside) ok = true; else s_led[kThreadsE + tid] += (double)e0;
+                    if (p.inside) ok = true; else e_out = e0;
                 } else state = L_DONE;
                 if (ok) {
                     uint2 vd = P.vox[L.vox];
                     L.rho = __uint_as_float(vd.x);
                     L.tagk = ((qt >> 2) << 6) | (vd.y << 2) | (qt & 3u);
                     L.idx = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20);
+                    // position relative to the voxel's low corner (a particle born on a face may be a rounding error outside)
+                    L.x = fminf(fmaxf(L.x - fmaf((float)ix, g.hx, g.ox), 0.0f), g.hx);
+                    L.y = fminf(fmaxf(L.y - fmaf((float)iy, g.hy, g.oy), 0.0f), g.hy);
+                    L.z = fminf(fmaxf(L.z - fmaf((float)iz, g.hz, g.oz), 0.0f), g.hz);
                     state = L_STEP;
                     if (L.T <= P.e_cut) terminate();  // born at or below the cut-off (pair electrons)
                     else set_dvox();
@@ -333,6 +354,13 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
                 park(0);  // L_DONE (nothing left to claim) retires the slot
             }
             __syncwarp();
+            // ledger and history count of this refill: one warp-level sum (at most 32 primaries: exact to ~1e-7 in fp32)
+            const unsigned m_new = __ballot_sync(kFull, e_new > 0.0f);
+            if (m_new) {
+                const float s_new = warp_sum_f(e_new), s_out = warp_sum_f(e_out);
+                if (lane == 0) { w_led[0] += (double)s_new; w_led[1] += (double)s_out; w_cnt[SE_HIST] += (uint32_t)__popc(m_new); }
+                __syncwarp();
+            }
             continue;
         }
 
@@ -343,7 +371,7 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
             if (have) {
                 load_slot(slot);
                 state = L_STEP;
-                uint4 h4 = next_block(L.rng, P.seed_lo, P.seed_hi);
+                uint4 h4 = next_block_rk(L.rng, P);
                 const float r = u01f(h4.x) * L.smax;
                 int i1 = min(max((int)L.ex, 0), N - 2);
                 float f1 = L.ex - (float)i1;
@@ -381,14 +409,14 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
                     };
                     float val;
                     for (;;) {
-                        uint4 m4 = next_block(L.rng, P.seed_lo, P.seed_hi);
+                        uint4 m4 = next_block_rk(L.rng, P);
                         if (trial(m4.x, m4.y, val)) break;
                         if (trial(m4.z, m4.w, val)) break;
                     }
                     const float phi = kTwoPiF * u01f(h4.w);
                     float sphi = f_sin(phi), cphi = f_cos(phi);
-                    QRec q; q.x = L.x; q.y = L.y; q.z = L.z; q.u = L.u; q.v = L.v; q.w = L.w; q.hist = L.rng.hist;
-                    q.trk_lo = h4.y; q.trk_hi = h4.z; q.vox = L.vox;
+                    QRec q; born_here(q); q.u = L.u; q.v = L.v; q.w = L.w;
+                    q.trk_lo = h4.y; q.trk_hi = h4.z;
                     float omu_q;  // 1 - cos(polar angle) of the secondary
                     if (mol) {
                         bump(SE_MOLLER);
@@ -433,7 +461,7 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         const float4 a0 = tA[i0];
         const float2 s0 = reinterpret_cast<const float2*>(tA + 3 * N)[i0];
         const float R0 = fmaf(f0, a0.y, a0.x), L0 = fmaf(f0, a0.w, a0.z), Smax = fmaf(f0, s0.y, s0.x);
-        uint4 w4 = next_block(L.rng, P.seed_lo, P.seed_hi);
+        uint4 w4 = next_block_rk(L.rng, P);
         const float rho = L.rho, irho = f_rcp(rho);
         const float d_vox = L.dvox;
         float d_lim = P.d_maxs;  // the non-geometric limits
@@ -469,9 +497,8 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
                 rotate_fast(L.u, L.v, L.w, fminf(omu, 2.0f), f_sin(phi), f_cos(phi));
             }
         }
-        int ix = (int)(L.idx & 1023u), iy = (int)((L.idx >> 10) & 1023u), iz = (int)(L.idx >> 20);
         float tx, ty, tz;
-        face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, ix, iy, iz, tx, ty, tz);
+        face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, tx, ty, tz);
         const float rest = d - legA;
         int ax = 0;
         float tf = tx;
@@ -495,46 +522,44 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         L.acc += L.T - T1;
         L.T = T1;
         if (cross) {
-            // leave the voxel: flush its deposit, move to the neighbour, coordinate snapped to the face (R8).
-            // Written with one predicate per axis so that it compiles to selects, not to a 3-way branch.
+            // leave the voxel: flush its deposit, enter the neighbour through the face that was hit (the one the
+            // direction points at; R8).  One predicate per axis: selects, not a 3-way branch.
             flush();
             const bool a0x = ax == 0, a1x = ax == 1, a2x = ax == 2;
             const float dc = a0x ? L.u : (a1x ? L.v : L.w);
-            const int dir = dc > 0.0f ? 1 : -1, up = dc > 0.0f ? 1 : 0;
-            const float tnew = (a0x ? g.hx : (a1x ? g.hy : g.hz)) * f_rcp(fabsf(dc));
-            // the face that was hit is the one the direction points at
-            const float fx = fmaf((float)(ix + up), g.hx, g.ox), fy = fmaf((float)(iy + up), g.hy, g.oy),
-                        fz = fmaf((float)(iz + up), g.hz, g.oz);
-            L.x = a0x ? fx : L.x; L.y = a1x ? fy : L.y; L.z = a2x ? fz : L.z;
+            const bool up = dc > 0.0f;
+            const float ha = a0x ? g.hx : (a1x ? g.hy : g.hz);
+            const float tnew = ha * f_rcp(fabsf(dc)), xin = up ? 0.0f : ha;  // local coordinate on the face it enters through
+            L.x = a0x ? xin : L.x; L.y = a1x ? xin : L.y; L.z = a2x ? xin : L.z;
             tx = a0x ? tnew : tx; ty = a1x ? tnew : ty; tz = a2x ? tnew : tz;
-            ix += a0x ? dir : 0; iy += a1x ? dir : 0; iz += a2x ? dir : 0;
-            L.vox += dir * (a0x ? 1 : (a1x ? g.nx : g.nx * g.ny));
-            if ((unsigned)ix >= (unsigned)g.nx || (unsigned)iy >= (unsigned)g.ny || (unsigned)iz >= (unsigned)g.nz) {
-                s_led[kThreadsE + tid] += (double)(L.T + (is_positron() ? 2.0f * kMeF : 0.0f));
+            const int sh = 10 * ax;
+            const int ia = (int)((L.idx >> sh) & 1023u) + (up ? 1 : -1);
+            const int na = a0x ? g.nx : (a1x ? g.ny : g.nz), stride = a0x ? 1 : (a1x ? g.nx : g.nx * g.ny);
+            if ((unsigned)ia >= (unsigned)na) {
+                atomicAdd(w_led + 1, (double)(L.T + (is_positron() ? 2.0f * kMeF : 0.0f)));
                 state = L_IDLE;
             } else {
-                L.idx = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20);
+                L.idx = (L.idx & ~(1023u << sh)) | ((uint32_t)ia << sh);
+                L.vox += up ? stride : -stride;
                 uint2 vd = P.vox[L.vox];
                 L.rho = __uint_as_float(vd.x); L.tagk = (L.tagk & ~60u) | (vd.y << 2);
-                if (L.T <= P.e_cut) terminate();
             }
-        } else if (L.T <= P.e_cut) terminate();
-        else if (lim == 4) { state = L_HARD; L.smax = Smax; }
+        }
+        if (state == L_STEP) {
+            if (L.T <= P.e_cut) terminate();
+            else if (lim == 4 && !cross) { state = L_HARD; L.smax = Smax; }
+        }
         L.dvox = fminf(tx, fminf(ty, tz));
         park(cross ? 2 : 1);
         __syncwarp();
     }
-    // ---- exit: reduce the per-thread counters ------------------------------------------------------------------
+    // ---- exit: the warp's counters and ledger go to the global ones -------------------------------------------------
+    __syncwarp();
     const int sid[SE_COUNT] = {S_ESTEP, S_MOLLER, S_BREMS, S_SEC_E, S_SEC_G, S_HIST, S_ATOMICS};
-#pragma unroll
-    for (int k = 0; k < SE_COUNT; ++k) {
-        unsigned long long s = k == SE_STEP ? (unsigned long long)n_step_w : warp_sum(s_cnt[k * kThreadsE + tid]);
-        if (lane == 0) stat_add(P.stats, sid[k], s);
-    }
-    double s_src = warp_sum(s_led[tid]), s_esc = warp_sum(s_led[kThreadsE + tid]);
+    if (lane < SE_COUNT) stat_add(P.stats, sid[lane], lane == SE_STEP ? (unsigned long long)n_step_w : (unsigned long long)w_cnt[lane]);
     if (lane == 0) {
-        if (s_src != 0.0) atomicAdd(P.ledger + LG_SRC, s_src);
-        if (s_esc != 0.0) atomicAdd(P.ledger + LG_ESC, s_esc);
+        if (w_led[0] != 0.0) atomicAdd(P.ledger + LG_SRC, w_led[0]);
+        if (w_led[1] != 0.0) atomicAdd(P.ledger + LG_ESC, w_led[1]);
     }
 }
 
@@ -657,7 +682,7 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
                 } else if (item < P.n_in + P.n_new) {
                     unsigned long long h = P.h_first + (item - P.n_in);
                     rng.hist = (uint32_t)h; rng.trk_lo = 0; rng.trk_hi = 0; rng.block = 0;
-                    uint4 w4 = next_block(rng, P.seed_lo, P.seed_hi);
+                    uint4 w4 = next_block_rk(rng, P);
                     Primary p = sample_primary<false>(P, w4);
                     tag = (batch_of(h, P.n_batches, P.n_total, P.inv_n_total) << 2) | CODE_PHOTON;
                     s_led[tid] += (double)p.E; bump(SP_HIST, 1u);
@@ -693,11 +718,11 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
                     return u01f(wb) <= 1.0f - eps * sin2 * f_rcp(1.0f + eps * eps);
                 };
                 for (;;) {
-                    uint4 c4 = next_block(rng, P.seed_lo, P.seed_hi);
+                    uint4 c4 = next_block_rk(rng, P);
                     if (trial(c4.x, c4.y)) break;
                     if (trial(c4.z, c4.w)) break;
                 }
-                uint4 d4 = next_block(rng, P.seed_lo, P.seed_hi);
+                uint4 d4 = next_block_rk(rng, P);
                 const float E1 = eps * E, Te = E - E1;
                 const float u0 = u, v0 = v, w0 = w;
                 const float phi = kTwoPiF * u01f(d4.z);
@@ -726,7 +751,7 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
         state = L_STEP;
         set_energy();
         // ---- FLY: up to two Woodcock flights from one Philox block (S2) --------------------------------------------
-        uint4 w4 = next_block(rng, P.seed_lo, P.seed_hi);
+        uint4 w4 = next_block_rk(rng, P);
         int chan = -1;
         uint32_t n_fl = 0, n_fi = 0;
         const float2* tm = s_tab;
@@ -761,12 +786,12 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
         } else if (chan == 1) {  // pair: both along the photon direction, uniform split
             bump(SP_PAIR, 1u);
             QRec q; q.x = x; q.y = y; q.z = z; q.hist = rng.hist; q.vox = vox;
-            uint4 a4 = next_block(rng, P.seed_lo, P.seed_hi);
+            uint4 a4 = next_block_rk(rng, P);
             float Tk = E - 2.0f * kMeF, us = u01f(a4.z);
             q.u = u; q.v = v; q.w = w;
             q.E = us * Tk; q.trk_lo = a4.x; q.trk_hi = a4.y; q.tag = (tag & ~3u) | CODE_ELECTRON;
             emit_e(q);
-            uint4 b4 = next_block(rng, P.seed_lo, P.seed_hi);
+            uint4 b4 = next_block_rk(rng, P);
             q.E = Tk - q.E; q.trk_lo = b4.x; q.trk_hi = b4.y; q.tag = (tag & ~3u) | CODE_POSITRON;
             emit_e(q);
             state = L_IDLE;
