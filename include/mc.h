@@ -111,6 +111,7 @@ typedef struct {
     double e_source_MeV, e_deposited_MeV, e_escaped_MeV; /* energy ledger                      */
     double transport_ms;         /* CUDA-event time of the transport launches                  */
     double electron_kernel_ms, photon_kernel_ms; /* split of transport_ms by kernel            */
+    uint64_t n_host_syncs;       /* counter read-backs (stream synchronisations) inside the transport loop */
 } mc_stats;
 
 /* mc_create — copy the phantom to the device.
@@ -224,6 +225,10 @@ mc_status mc_set_stream(mc_ctx *ctx, void *cuda_stream);
  *   "hard_lanes"    tracks of a warp's pool that must wait for the hard-event / Compton block before the warp runs it
  *                   (default 32 = a full warp; the block also runs when it has more tracks than the step block)
  *   "refill_lanes"  empty slots of a warp's pool that trigger a refill from the queue / the source (default 32)
+ *   "plan_ahead"    1 (default): once the secondaries-per-primary ratios of the beam are known (a probe launch, or the
+ *                   previous run with the same kind of beam) the launches of a run are enqueued ahead — every kernel
+ *                   reads the size of its input queue on the device and leaves it empty — and the host reads the
+ *                   counters back only once per round of the final cascade; 0: one read-back per launch
  *   "blocks_per_sm" cap on the CTAs per SM (0 = as many as fit; the transport kernels use one)
  *   "aggregate"     1: lanes of a warp that score into the same cell at the same moment combine into one
  *                   red.global.add.f32; 0: one per lane; -1 (default): 1 for beams entering through fewer than 16

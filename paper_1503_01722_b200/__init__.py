@@ -64,7 +64,7 @@ class _Stats(C.Structure):
         "n_photoelectric", "n_moller", "n_brems", "n_secondary_electrons", "n_secondary_photons",
         "n_dose_atomics", "n_kernel_launches")] + [(n, C.c_double) for n in (
             "e_source_MeV", "e_deposited_MeV", "e_escaped_MeV", "transport_ms", "electron_kernel_ms",
-            "photon_kernel_ms")]
+            "photon_kernel_ms")] + [("n_host_syncs", C.c_uint64)]
 
 
 def lib():

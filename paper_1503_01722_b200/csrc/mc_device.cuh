@@ -49,7 +49,7 @@ struct Queue {
     uint32_t* count;  // device counter (tail)
     uint32_t cap;
 };
-enum Counter { C_HEAD = 0, C_E_A, C_E_B, C_P, C_OVERFLOW, C_COUNT };
+enum Counter { C_HEAD = 0, C_E_A, C_E_B, C_P, C_OVERFLOW, C_DONE, C_COUNT };  // C_DONE: CTAs of the running launch that have finished
 enum StatId {
     S_ESTEP = 0, S_FLIGHT, S_FICT, S_COMPTON, S_PAIR, S_PE, S_MOLLER, S_BREMS, S_SEC_E, S_SEC_G, S_ATOMICS,
     S_HIST, S_COUNT
@@ -80,7 +80,7 @@ struct RunParams {
     unsigned long long inv_n_total;       // floor(2^64 / n_total), see batch_of
     int n_batches;
     uint32_t seed_lo, seed_hi;
-    uint32_t n_in, n_new;     // queued particles to consume, new primaries to generate
+    uint32_t n_new;           // new primaries to generate (the queued particles to consume = *q_in.count, read on the device)
     Queue q_in, q_e_out, q_p_out;
     uint32_t* counters;       // Counter
     unsigned long long* stats;  // StatId

@@ -42,8 +42,11 @@ struct mc_ctx {
     float *d_dose = nullptr, *d_sigma = nullptr;
     float* d_beam = nullptr;  // E nodes, pdf nodes, cdf: 3 x kMaxNodes
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    std::vector<cudaEvent_t> lev;  // event pairs around the transport launches of a run (read after the run's last sync)
+    std::vector<char> lev_p;       // launch i was a photon kernel
     // options (M "manually adjusted")
     int64_t wave_size = 1 << 24, queue_factor = 4, blocks_per_sm = 0, refill_lanes = 32, aggregate = -1, hard_lanes = 32, adaptive = 1;
+    int64_t plan_ahead = 1;  // enqueue launches ahead of the counters once the secondaries-per-primary ratios are known
     int64_t hinge_overrun_pct = 25, ms_carry = 1;  // readings R8 / R8b; the oracle has the same switches
     mc_stats stats{};
     // secondaries-per-primary ratios measured by the last run, reused when the next run has the same kind of beam
@@ -165,6 +168,12 @@ bool choose_photon_kernel(const mc_ctx* c, KernelChoice& k) {
     for (int i = 0; i < 3; ++i)
         if (smem_p(c, T[i]) <= kSmemMax) { k = KernelChoice{fn[i], T[i], smem_p(c, T[i])}; return true; }
     return false;
+}
+
+// what the remembered secondaries-per-primary ratios belong to (mc_build_tables, mc_set_photon_tables and mc_set_option
+// forget them: cut-offs, tables and scheduling options change the ratios)
+double beam_key_of(const mc_ctx*, const mc_beam* b) {
+    return (double)b->particle * 1e3 + (double)b->E_nodes_MeV[b->n_nodes - 1] + 1e-3 * b->n_nodes;
 }
 
 mc_status check_beam(mc_ctx* ctx, const mc_beam* b) {
@@ -314,23 +323,81 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
     double ms_e = 0, ms_p = 0;
     // secondaries queued per new primary (electron queue, photon queue): measured while running; the first launch of a
     // context is a probe (16 assumed), later runs with the same kind of beam start from the last measurement
-    const double key = beam ? (double)beam->particle * 1e3 + (double)beam->E_nodes_MeV[beam->n_nodes - 1] : -2.0;
-    double m_new_e = key == ctx->beam_key ? ctx->last_m_e : 16.0, m_new_p = key == ctx->beam_key ? ctx->last_m_p : 16.0;
+    const double key = beam ? beam_key_of(ctx, beam) : -2.0;
+    bool have_ratio = key == ctx->beam_key;
+    double m_new_e = have_ratio ? ctx->last_m_e : 16.0, m_new_p = have_ratio ? ctx->last_m_p : 16.0;
+    // Every transport launch: the kernel reads the size of its input queue on the device, and its last CTA empties that
+    // queue and the work counter, so a launch needs nothing from the host but the number of new primaries.
+    size_t n_timed = 0;  // event pairs ctx->lev[2i], [2i+1] bracket the launches of this run; lev_p[i] = photon kernel
+    auto issue = [&](bool run_p, uint32_t n_new, uint64_t items_hint) -> mc_status {
+        P.n_new = n_new; P.h_first = h_next;
+        Queue qe_cur{ctx->d_q[cur], ctx->d_counters + C_E_A + cur, ctx->q_cap};
+        Queue qe_oth{ctx->d_q[1 - cur], ctx->d_counters + C_E_A + (1 - cur), ctx->q_cap};
+        Queue qp{ctx->d_q[2], ctx->d_counters + C_P, ctx->q_cap};
+        const int occ = run_p ? occ_p : occ_e, thr = run_p ? kp.threads : ke.threads;
+        int grid = (int)std::min<uint64_t>((uint64_t)ctx->sm_count * occ, (items_hint + thr - 1) / thr);
+        grid = std::max(grid, 1);
+        if (ctx->lev.size() < 2 * (n_timed + 1)) {
+            cudaEvent_t a, b;
+            CU(cudaEventCreate(&a)); ctx->lev.push_back(a);
+            CU(cudaEventCreate(&b)); ctx->lev.push_back(b);
+        }
+        if (ctx->lev_p.size() < n_timed + 1) ctx->lev_p.resize(n_timed + 1);
+        ctx->lev_p[n_timed] = run_p;
+        CU(cudaEventRecord(ctx->lev[2 * n_timed], s));
+        if (run_p) {
+            P.q_in = qp; P.q_e_out = qe_cur; P.q_p_out = qp;
+            kp.fn<<<grid, kp.threads, sp, s>>>(P);
+        } else {
+            P.q_in = qe_cur; P.q_e_out = qe_oth; P.q_p_out = qp;
+            ke.fn<<<grid, ke.threads, se, s>>>(P);
+            cur = 1 - cur;  // what this launch produced is the next electron launch's input
+        }
+        CU(cudaGetLastError());
+        CU(cudaEventRecord(ctx->lev[2 * n_timed + 1], s));
+        ++n_timed;
+        ++S.n_kernel_launches;
+        remaining -= n_new; h_next += n_new;
+        return MC_OK;
+    };
+    auto read_counters = [&]() -> mc_status {  // the one host <-> device crossing: 24 bytes and a stream synchronisation
+        CU(cudaMemcpyAsync(ctx->h_counters, ctx->d_counters, C_COUNT * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+        CU(cudaStreamSynchronize(s));
+        ++S.n_host_syncs;
+        if (ctx->h_counters[C_OVERFLOW]) {
+            ctx->beam_key = -1.0;  // the remembered ratios admitted too much: probe again next time
+            return fail(ctx, MC_ERR_QUEUE_OVERFLOW, "particle queue overflow: lower option wave_size or raise queue_factor");
+        }
+        cnt_e[0] = ctx->h_counters[C_E_A]; cnt_e[1] = ctx->h_counters[C_E_B]; cnt_p = ctx->h_counters[C_P];
+        return MC_OK;
+    };
+    // new primaries a launch of the source's type may admit: up to a wave, and no more than the output queues can take
+    // at the secondaries-per-primary ratios (R21: a queue must not overflow by admission; overflow is still detected)
+    auto admit = [&](bool run_p, double in_e, double in_p) -> uint32_t {
+        const double n_in = run_p ? in_p : in_e;
+        if (n_in >= W) return 0u;
+        const double room_e = (double)ctx->q_cap - (run_p ? in_e : 0.0) - n_in;
+        const double room_p = run_p ? 1e30 : (double)ctx->q_cap - in_p - n_in;
+        const double fit = ctx->adaptive ? std::max(0.0, std::min(room_e / m_new_e, room_p / m_new_p)) : 1e30;
+        uint32_t n_new = (uint32_t)std::min<double>((double)std::min<uint64_t>(remaining, (uint64_t)(W - n_in)), fit);
+        if (n_new == 0 && n_in == 0) n_new = (uint32_t)std::min<uint64_t>(remaining, 1024);  // always progress
+        return n_new;
+    };
     CU(cudaEventRecord(ctx->ev[0], s));
-    while (remaining > 0 || cnt_e[cur] > 0 || cnt_p > 0) {
+    const bool plan_ahead = beam && ctx->plan_ahead && ctx->adaptive;
+    // ---- launches decided one at a time from the counters (Table 1): particle lists, the probe launches of
+    // a beam whose secondaries-per-primary ratios are not known yet, and everything when option plan_ahead is 0 --------
+    while ((remaining > 0 || cnt_e[cur] > 0 || cnt_p > 0) && !(plan_ahead && have_ratio)) {
         if (d_list && remaining > 0 && cnt_e[cur] < W && cnt_p < W) {
             // particle-list source: the next wave of listed particles goes straight into the input queues
             const uint32_t n_load = (uint32_t)std::min<uint64_t>(remaining, W);
-            P.h_first = h_next; P.n_in = 0; P.n_new = 0;
+            P.h_first = h_next; P.n_new = 0;
             P.q_e_out = Queue{ctx->d_q[cur], ctx->d_counters + C_E_A + cur, ctx->q_cap};
             P.q_p_out = Queue{ctx->d_q[2], ctx->d_counters + C_P, ctx->q_cap};
             load_particles_kernel<<<std::min<uint32_t>((n_load + kThreads - 1) / kThreads, (uint32_t)ctx->sm_count * 8), kThreads, 0, s>>>(P, d_list, n_load);
             CU(cudaGetLastError());
-            CU(cudaMemcpyAsync(ctx->h_counters, ctx->d_counters, C_COUNT * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
-            CU(cudaStreamSynchronize(s));
             ++S.n_kernel_launches;
-            if (ctx->h_counters[C_OVERFLOW]) return fail(ctx, MC_ERR_QUEUE_OVERFLOW, "particle queue overflow while loading the particle list");
-            cnt_e[cur] = ctx->h_counters[C_E_A + cur]; cnt_p = ctx->h_counters[C_P];
+            if ((st = read_counters()) != MC_OK) return st;
             remaining -= n_load; h_next += n_load;
             continue;
         }
@@ -342,56 +409,63 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
             uint64_t avail_e = cnt_e[cur] + (photon_beam ? 0 : src), avail_p = cnt_p + (photon_beam ? src : 0);
             run_p = avail_p > avail_e;
         }
-        uint32_t n_in = run_p ? cnt_p : cnt_e[cur], n_new = 0;
-        if (beam && run_p == photon_beam && n_in < W) {
-            // new primaries admitted by this launch: up to a wave, and no more than the output queues can take at
-            // the secondaries-per-primary ratio measured so far (first launch: a probe of cap / 16 histories)
-            const double room_e = (double)ctx->q_cap - (run_p ? cnt_e[cur] : 0u) - (double)n_in;
-            const double room_p = run_p ? 1e30 : (double)ctx->q_cap - cnt_p - (double)n_in;
-            const double fit = ctx->adaptive ? std::max(0.0, std::min(room_e / m_new_e, room_p / m_new_p)) : 1e30;
-            n_new = (uint32_t)std::min<double>((double)std::min<uint64_t>(remaining, W - n_in), fit);
-            if (n_new == 0 && n_in == 0) n_new = (uint32_t)std::min<uint64_t>(remaining, 1024);  // always progress
-        }
-        P.n_in = n_in; P.n_new = n_new; P.h_first = h_next;
-        Queue qe_cur{ctx->d_q[cur], ctx->d_counters + C_E_A + cur, ctx->q_cap};
-        Queue qe_oth{ctx->d_q[1 - cur], ctx->d_counters + C_E_A + (1 - cur), ctx->q_cap};
-        Queue qp{ctx->d_q[2], ctx->d_counters + C_P, ctx->q_cap};
-        const uint64_t items = (uint64_t)n_in + n_new;
-        const int occ = run_p ? occ_p : occ_e, thr = run_p ? kp.threads : ke.threads;
-        int grid = (int)std::min<uint64_t>((uint64_t)ctx->sm_count * occ, (items + thr - 1) / thr);
-        grid = std::max(grid, 1);
-        CU(cudaEventRecord(ctx->ev[2], s));
-        if (run_p) {
-            P.q_in = qp; P.q_e_out = qe_cur; P.q_p_out = qp;
-            kp.fn<<<grid, kp.threads, sp, s>>>(P);
-        } else {
-            P.q_in = qe_cur; P.q_e_out = qe_oth; P.q_p_out = qp;
-            ke.fn<<<grid, ke.threads, se, s>>>(P);
-        }
-        CU(cudaGetLastError());
-        CU(cudaEventRecord(ctx->ev[3], s));
-        // the consumed queue and the work counter start the next launch empty
-        CU(cudaMemsetAsync(ctx->d_counters + C_HEAD, 0, sizeof(uint32_t), s));
-        CU(cudaMemsetAsync(run_p ? qp.count : qe_cur.count, 0, sizeof(uint32_t), s));
-        CU(cudaMemcpyAsync(ctx->h_counters, ctx->d_counters, C_COUNT * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
-        CU(cudaStreamSynchronize(s));
-        float ms = 0;
-        CU(cudaEventElapsedTime(&ms, ctx->ev[2], ctx->ev[3]));
-        (run_p ? ms_p : ms_e) += ms;
-        ++S.n_kernel_launches;
-        if (ctx->h_counters[C_OVERFLOW])
-            return fail(ctx, MC_ERR_QUEUE_OVERFLOW, "particle queue overflow: lower option wave_size or raise queue_factor");
-        remaining -= n_new; h_next += n_new;
+        const uint32_t n_in = run_p ? cnt_p : cnt_e[cur];
+        const uint32_t n_new = beam && run_p == photon_beam ? admit(run_p, cnt_e[cur], cnt_p) : 0u;
+        const uint32_t before_e = cnt_e[cur], before_p = cnt_p;
+        const int cur0 = cur;
+        if ((st = issue(run_p, n_new, (uint64_t)n_in + n_new)) != MC_OK) return st;
+        if ((st = read_counters()) != MC_OK) return st;
         if (n_new >= n_in && n_new >= 1024) {  // a launch dominated by primaries: update the measured ratios
-            const double out_e = run_p ? (double)ctx->h_counters[C_E_A + cur] - cnt_e[cur] : (double)ctx->h_counters[C_E_A + (1 - cur)];
-            const double out_p = run_p ? 0.0 : (double)ctx->h_counters[C_P] - cnt_p;
+            const double out_e = run_p ? (double)cnt_e[cur0] - before_e : (double)cnt_e[1 - cur0];
+            const double out_p = run_p ? 0.0 : (double)cnt_p - before_p;
             const double n_items = (double)n_in + n_new;
             m_new_e = std::max(0.05, 1.5 * out_e / n_items);
             m_new_p = std::max(0.05, 1.5 * out_p / n_items);
             ctx->beam_key = key; ctx->last_m_e = m_new_e; ctx->last_m_p = m_new_p;
+            have_ratio = true;
         }
-        if (run_p) { cnt_p = 0; cnt_e[cur] = ctx->h_counters[C_E_A + cur]; }
-        else { cnt_e[cur] = 0; cur = 1 - cur; cnt_e[cur] = ctx->h_counters[C_E_A + cur]; cnt_p = ctx->h_counters[C_P]; }
+    }
+    // ---- launches enqueued ahead (ratios known): the host does not wait between launches.  Per wave: the source's kernel
+    // (it also consumes whatever its queue holds), then the other type where its queue fills fastest; after the last wave
+    // the cascade is drained by rounds of [photon, electron, electron] launches — a launch whose queue turns out to be
+    // empty returns at once — with one read-back per round to see whether anything is left. ---------------------------
+    if (remaining > 0 || cnt_e[cur] > 0 || cnt_p > 0) {
+        const uint64_t full = ~0ull >> 1;  // size unknown on the host: full grid
+        double est_e = cnt_e[cur], est_p = cnt_p;  // upper estimates of what the queues hold
+        int wave = 0;
+        while (remaining > 0) {
+            const uint32_t n_new = admit(photon_beam, est_e, est_p);
+            if (n_new == 0) {  // the estimates say the queues are too full: drain one generation and look
+                if ((st = issue(!photon_beam, 0, full)) != MC_OK) return st;
+                if ((st = issue(photon_beam, 0, full)) != MC_OK) return st;
+                if ((st = read_counters()) != MC_OK) return st;
+                est_e = cnt_e[cur]; est_p = cnt_p;
+                continue;
+            }
+            if ((st = issue(photon_beam, n_new, full)) != MC_OK) return st;
+            if (photon_beam) {
+                // a photon wave fills the electron queue: run it now; its own output (delta rays, bremsstrahlung) rides
+                // along with the next wave
+                est_e += m_new_e * n_new;
+                if ((st = issue(false, 0, full)) != MC_OK) return st;
+                est_e = 0.15 * est_e; est_p = 0.15 * m_new_e * n_new;
+            } else {
+                // an electron wave: delta rays go to the next electron launch, photons wait for every second wave
+                est_e = m_new_e * n_new; est_p += m_new_p * n_new;
+                if ((++wave & 1) == 0 || est_p > 0.5 * ctx->q_cap) {
+                    if ((st = issue(true, 0, full)) != MC_OK) return st;
+                    est_e += 0.5 * est_p; est_p = 0.0;
+                }
+            }
+        }
+        do {
+            for (int k = 0; k < 4; ++k) {
+                if ((st = issue(true, 0, full)) != MC_OK) return st;
+                if ((st = issue(false, 0, full)) != MC_OK) return st;
+                if ((st = issue(false, 0, full)) != MC_OK) return st;
+            }
+            if ((st = read_counters()) != MC_OK) return st;
+        } while (cnt_e[0] > 0 || cnt_e[1] > 0 || cnt_p > 0);
     }
     CU(cudaEventRecord(ctx->ev[1], s));
     // ledger: deposited energy is the total of the batch grids
@@ -405,6 +479,11 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
     CU(cudaStreamSynchronize(s));
     float ms = 0;
     CU(cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]));
+    for (size_t i = 0; i < n_timed; ++i) {
+        float t = 0;
+        CU(cudaEventElapsedTime(&t, ctx->lev[2 * i], ctx->lev[2 * i + 1]));
+        (ctx->lev_p[i] ? ms_p : ms_e) += t;
+    }
     S.n_histories = hs[S_HIST]; S.n_electron_steps = hs[S_ESTEP]; S.n_photon_flights = hs[S_FLIGHT];
     S.n_fictitious = hs[S_FICT]; S.n_compton = hs[S_COMPTON]; S.n_pair = hs[S_PAIR]; S.n_photoelectric = hs[S_PE];
     S.n_moller = hs[S_MOLLER]; S.n_brems = hs[S_BREMS]; S.n_secondary_electrons = hs[S_SEC_E];
@@ -486,6 +565,7 @@ void mc_destroy(mc_ctx* ctx) {
         cudaFree(ctx->d_counters); cudaFreeHost(ctx->h_counters); cudaFree(ctx->d_stats); cudaFree(ctx->d_ledger);
         cudaFree(ctx->d_edep); cudaFree(ctx->d_dose); cudaFree(ctx->d_sigma); cudaFree(ctx->d_beam);
         for (auto e : ctx->ev) if (e) cudaEventDestroy(e);
+        for (auto e : ctx->lev) cudaEventDestroy(e);
     }
     delete ctx;
 }
@@ -521,7 +601,7 @@ mc_status mc_build_tables(mc_ctx* ctx, const mc_material* mats, int32_t n_mats, 
         std::copy(ctx->tabs.t[T_MU_C][m].begin(), ctx->tabs.t[T_MU_C][m].end(), ctx->p_C.begin() + (size_t)m * N);
         std::copy(ctx->tabs.t[T_MU_PP][m].begin(), ctx->tabs.t[T_MU_PP][m].end(), ctx->p_pp.begin() + (size_t)m * N);
     }
-    ctx->have_tables = true; ctx->tables_dirty = true;
+    ctx->have_tables = true; ctx->tables_dirty = true; ctx->beam_key = -1.0;
     return MC_OK;
 }
 
@@ -558,7 +638,7 @@ mc_status mc_set_photon_tables(mc_ctx* ctx, float lnE0, float inv_dln, const flo
     ctx->lnE0P = lnE0; ctx->inv_dlnP = inv_dln;
     ctx->p_maj.assign(mu_maj, mu_maj + N);
     ctx->p_tot.assign(mu_tot, mu_tot + nm * N); ctx->p_C.assign(mu_C, mu_C + nm * N); ctx->p_pp.assign(mu_pp, mu_pp + nm * N);
-    ctx->tables_dirty = true;
+    ctx->tables_dirty = true; ctx->beam_key = -1.0;
     return MC_OK;
 }
 
@@ -813,8 +893,10 @@ mc_status mc_set_option(mc_ctx* ctx, const char* name, int64_t value) {
     else if (n == "adaptive") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "adaptive in {0, 1}"); ctx->adaptive = value; }
     else if (n == "aggregate") { if (value < -1 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "aggregate in {-1, 0, 1}"); ctx->aggregate = value; }
     else if (n == "hinge_overrun_pct") { if (value < 0 || value > 100) return fail(ctx, MC_ERR_INVALID_ARG, "hinge_overrun_pct in [0, 100]"); ctx->hinge_overrun_pct = value; }
+    else if (n == "plan_ahead") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "plan_ahead in {0, 1}"); ctx->plan_ahead = value; }
     else if (n == "ms_carry") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "ms_carry in {0, 1}"); ctx->ms_carry = value; }
     else return fail(ctx, MC_ERR_INVALID_ARG, "unknown option: " + n);
+    ctx->beam_key = -1.0;  // scheduling options and readings change the secondaries-per-primary ratios: probe again
     return MC_OK;
 }
 

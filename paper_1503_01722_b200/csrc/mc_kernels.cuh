@@ -88,6 +88,19 @@ __device__ __forceinline__ uint32_t claim(uint32_t* head, unsigned want_mask, in
     return base + __popc(want_mask & ((1u << lane) - 1u));
 }
 
+// End of a transport launch: the last CTA to finish empties the consumed input queue and the work counter, so that the
+// next launch can be enqueued without the host touching the counters (no launch pushes into its own input queue).
+__device__ __forceinline__ void launch_epilogue(const RunParams& P) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(P.counters + C_DONE, 1u) == gridDim.x - 1u) {
+            P.counters[C_HEAD] = 0u; *P.q_in.count = 0u; P.counters[C_DONE] = 0u;
+            __threadfence();
+        }
+    }
+}
+
 // Make a secondary: queue it, or (MC_FLAG_LOCAL_SECONDARIES) score its energy where it is born.
 __device__ __forceinline__ void emit(const RunParams& P, const Queue& q, Score& sc, uint32_t cell, const QRec& r,
                                      uint32_t& n_pushed) {
@@ -175,6 +188,9 @@ struct ELane {
 template <int kThreadsE>
 __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_constant__ RunParams P) {
     extern __shared__ __align__(16) float2 s_tab[];
+    // the launch consumes the whole input queue as it stands (no host round trip)
+    const uint32_t n_in = *static_cast<const volatile uint32_t*>(P.q_in.count);
+    if (n_in + P.n_new == 0u) return;  // nothing to do: an enqueued-ahead launch of a generation that does not exist
     const int ntab = P.n_mat * P.e_stride;
     constexpr int kWarps = kThreadsE / 32;
     uint4* s_trk = reinterpret_cast<uint4*>(s_tab + ntab);                     // [kGroups][kSlots][kThreadsE]
@@ -318,15 +334,15 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
                 bool ok = false;
                 uint32_t qt = 0u;
                 int ix = 0, iy = 0, iz = 0;
-                if (item < P.n_in) {
+                if (item < n_in) {
                     QRec r = load_record(P.q_in, item);
                     L.x = r.x; L.y = r.y; L.z = r.z; L.u = r.u; L.v = r.v; L.w = r.w; L.T = r.E;
                     L.rng.hist = r.hist; L.rng.trk_lo = r.trk_lo; L.rng.trk_hi = r.trk_hi; L.rng.block = 0;
                     L.vox = r.vox; qt = r.tag;
                     ix = L.vox % g.nx; int t2 = L.vox / g.nx; iy = t2 % g.ny; iz = t2 / g.ny;
                     ok = true;
-                } else if (item < P.n_in + P.n_new) {
-                    unsigned long long h = P.h_first + (item - P.n_in);
+                } else if (item < n_in + P.n_new) {
+                    unsigned long long h = P.h_first + (item - n_in);
                     L.rng.hist = (uint32_t)h; L.rng.trk_lo = 0; L.rng.trk_hi = 0; L.rng.block = 0;
                     uint4 w4 = next_block_rk(L.rng, P);
                     Primary p = sample_primary<false>(P, w4);
@@ -561,6 +577,7 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         if (w_led[0] != 0.0) atomicAdd(P.ledger + LG_SRC, w_led[0]);
         if (w_led[1] != 0.0) atomicAdd(P.ledger + LG_ESC, w_led[1]);
     }
+    launch_epilogue(P);
 }
 
 // =================================================================================================
@@ -577,6 +594,8 @@ enum { SP_FLIGHT = 0, SP_FICT, SP_COMPTON, SP_PAIR, SP_PE, SP_SEC_E, SP_HIST, SP
 template <int kThreadsP>
 __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_constant__ RunParams P) {
     extern __shared__ float2 s_tab[];
+    const uint32_t n_in = *static_cast<const volatile uint32_t*>(P.q_in.count);  // as in electron_kernel
+    if (n_in + P.n_new == 0u) return;
     const int ntab = (1 + P.n_mat * TP_COUNT) * P.N;
     uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_tab + ntab);              // [SP_COUNT][kThreadsP]
     double* s_led = reinterpret_cast<double*>(s_cnt + SP_COUNT * kThreadsP);  // [2][kThreadsP]: e_src, e_esc
@@ -673,14 +692,14 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
             if (have) {
                 state = L_IDLE;
                 bool ok = false;
-                if (item < P.n_in) {
+                if (item < n_in) {
                     QRec r = load_record(P.q_in, item);
                     x = r.x; y = r.y; z = r.z; u = r.u; v = r.v; w = r.w; E = r.E;
                     rng.hist = r.hist; rng.trk_lo = r.trk_lo; rng.trk_hi = r.trk_hi; rng.block = 0;
                     vox = r.vox; tag = r.tag;
                     ok = true;
-                } else if (item < P.n_in + P.n_new) {
-                    unsigned long long h = P.h_first + (item - P.n_in);
+                } else if (item < n_in + P.n_new) {
+                    unsigned long long h = P.h_first + (item - n_in);
                     rng.hist = (uint32_t)h; rng.trk_lo = 0; rng.trk_hi = 0; rng.block = 0;
                     uint4 w4 = next_block_rk(rng, P);
                     Primary p = sample_primary<false>(P, w4);
@@ -810,6 +829,7 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
         if (s_src != 0.0) atomicAdd(P.ledger + LG_SRC, s_src);
         if (s_esc != 0.0) atomicAdd(P.ledger + LG_ESC, s_esc);
     }
+    launch_epilogue(P);
 }
 
 // =================================================================================================

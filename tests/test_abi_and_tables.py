@@ -42,7 +42,7 @@ def test_struct_layouts_match_the_header():
     assert C.sizeof(mc._Params) == 28
     assert C.sizeof(mc._Material) == 40
     assert C.sizeof(mc._Beam) == 64
-    assert C.sizeof(mc._Stats) == 13 * 8 + 6 * 8
+    assert C.sizeof(mc._Stats) == 13 * 8 + 6 * 8 + 8
     assert mc.PARTICLE_DTYPE.itemsize == 32 and W.PARTICLE_DTYPE == mc.PARTICLE_DTYPE  # mc_particle
 
 
