@@ -32,8 +32,11 @@ sys.path.insert(0, ROOT)
 
 from paper_1503_01722_b200 import workloads as W  # noqa: E402  (input generators only)
 
-# Algorithmic thread-instructions per unit of work.
-INSTR_PER = {"e_step": 240.0, "hard_event": 150.0, "photon_flight": 60.0, "photon_interaction": 150.0}
+# Algorithmic thread-instructions per unit of work (SURVEY.md 8(d) "Algorithmic work per unit").
+# Headline: the figures the survey's own ceiling uses (225 per e- step; mid-range for the rest); beside it the top-of-range
+# variant round 1 reported.
+INSTR_PER = {"e_step": 225.0, "hard_event": 115.0, "photon_flight": 75.0, "photon_interaction": 150.0}
+INSTR_PER_TOP = {"e_step": 240.0, "hard_event": 150.0, "photon_flight": 60.0, "photon_interaction": 150.0}
 SM_COUNT, SCHEDULERS_PER_SM, LANES = 148, 4, 32
 
 
@@ -51,6 +54,20 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--option", action="append", default=[], help="engine option name=value (mc_set_option)")
     return ap.parse_args()
+
+
+def profile_traffic(kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full summary of the
+    current round (profiles/r2_<kernel>_ncu_full.txt, line 'dram_bytes_per_launch: <bytes> ...'), else null: the
+    bench does not run under ncu, so the figure can only come from the capture."""
+    p = os.path.join(ROOT, "profiles", f"r2_{kernel}_ncu_full.txt")
+    try:
+        for ln in open(p):
+            if ln.startswith("dram_bytes_per_launch:"):
+                return float(ln.split()[1]), f"profiles/r2_{kernel}_ncu_full.txt (ncu --set full, first wave of primaries of its config)"
+    except OSError:
+        pass
+    return None, "no ncu capture of this kernel committed for this round"
 
 
 def peaks():
@@ -333,28 +350,49 @@ def run_engine(args):
     issue_peak = SM_COUNT * SCHEDULERS_PER_SM * LANES * pk["sm_max_mhz"] * 1e6  # thread-instructions / s
     issue_measured = max(mc.mc_bench_issue(eng.ctx, 4096) for _ in range(3))  # FFMA micro-benchmark on this GPU
     e_ms, p_ms = acc["electron_kernel_ms"], acc["photon_kernel_ms"]
-    alg_e = acc["n_electron_steps"] * INSTR_PER["e_step"] + (acc["n_moller"] + acc["n_brems"]) * INSTR_PER["hard_event"]
-    alg_p = acc["n_photon_flights"] * INSTR_PER["photon_flight"] + \
-        (acc["n_compton"] + acc["n_pair"] + acc["n_photoelectric"]) * INSTR_PER["photon_interaction"]
     dom = "electron_kernel" if e_ms >= p_ms else "photon_kernel"
-    alg, kms = (alg_e, e_ms) if dom == "electron_kernel" else (alg_p, p_ms)
-    achieved = alg / (kms * 1e-3) if kms > 0 else 0.0
+    kms = e_ms if dom == "electron_kernel" else p_ms
+
+    def algorithmic(per):
+        if dom == "electron_kernel":
+            return acc["n_electron_steps"] * per["e_step"] + (acc["n_moller"] + acc["n_brems"]) * per["hard_event"]
+        return acc["n_photon_flights"] * per["photon_flight"] + \
+            (acc["n_compton"] + acc["n_pair"] + acc["n_photoelectric"]) * per["photon_interaction"]
+
+    achieved = algorithmic(INSTR_PER) / (kms * 1e-3) if kms > 0 else 0.0
+    achieved_top = algorithmic(INSTR_PER_TOP) / (kms * 1e-3) if kms > 0 else 0.0
+    traffic, traffic_src = profile_traffic(dom)
     roofline = {"bound": "alu", "kernel": dom, "achieved": achieved / 1e12, "peak": issue_peak / 1e12,
                 "unit": "Tinstr/s (thread-instructions)", "frac": achieved / issue_peak,
-                # dram__bytes_read.sum + dram__bytes_write.sum of one launch of that kernel (a wave of primaries) from the
-                # committed ncu --set full capture, profiles/r1b_*_kernel_ncu_full.txt: queue records, not a bound
-                "traffic": {"electron_kernel": 435.8e6, "photon_kernel": 160.7e6}[dom], "traffic_unit": "bytes per launch (ncu capture, profiles/)",
+                "instr_per_unit": INSTR_PER, "frac_top_of_range": achieved_top / issue_peak, "instr_per_unit_top_of_range": INSTR_PER_TOP,
+                "headline": "frac (SURVEY 8(d) ceiling figures: 225 thread-instructions per e- step)",
+                "traffic": traffic, "traffic_unit": "bytes per launch", "traffic_source": traffic_src,
                 "peak_source": f"148 SM x 4 schedulers x 32 lanes x sm_max_mhz ({pk_kind} MEASURED_PEAKS.json clock)",
                 "peak_measured": issue_measured / 1e12, "frac_of_measured": achieved / issue_measured,
                 "peak_measured_source": "mc_bench_issue: 2 x 1024-thread CTAs per SM, 8 independent FFMA chains per thread, best of 3",
                 "kernel_ms_per_step": kms / K, "kernel_share_of_step": kms / total_ms if world == 1 else None}
-    # scoring roofline: measured red.global.add.f32 peak into a window the size of one batch grid
-    red_ms = min(mc.mc_bench_red(eng.ctx, nvox, 64, 0, SM_COUNT * 8) for _ in range(3))
-    red_peak = SM_COUNT * 8 * 256 * 64 / (red_ms * 1e-3)
+    # scoring roofline: red.global.add.f32 peak, best over occupancy (1, 2, 4, 8 CTAs of 256 threads per SM) on windows
+    # the size of one batch grid of configs 2-4 (0.9 MB) and of config 5 (7.1 MB), random cells (no intra-warp
+    # collisions on average), >= 2 ms per launch; mode 1 (one cell per warp) beside it
+    red_table, red_peak = [], 0.0
+    for cells in (223260, 1786080):
+        for per_sm in (1, 2, 4, 8):
+            blocks = SM_COUNT * per_sm
+            per_thread = int(min(60000, max(64, 4e8 / (blocks * 256))))
+            ms = mc.mc_bench_red(eng.ctx, cells, per_thread, 0, blocks)
+            rate = blocks * 256 * per_thread / (ms * 1e-3)
+            red_table.append({"window_MB": round(cells * 4 / 1e6, 1), "ctas_per_sm": per_sm, "mode": "random cells", "ms": round(ms, 3), "Gred_s": round(rate / 1e9, 1)})
+            red_peak = max(red_peak, rate)
+    for cells in (223260,):
+        blocks = SM_COUNT * 8
+        per_thread = 2000
+        ms = mc.mc_bench_red(eng.ctx, cells, per_thread, 1, blocks)
+        red_table.append({"window_MB": round(cells * 4 / 1e6, 1), "ctas_per_sm": 8, "mode": "one cell per warp", "ms": round(ms, 3),
+                          "Gred_s": round(blocks * 256 * per_thread / (ms * 1e-3) / 1e9, 1)})
     red_rate = acc["n_dose_atomics"] / ((e_ms + p_ms) * 1e-3)
     roofline_scoring = {"bound": "l2_atomic", "achieved": red_rate / 1e9, "peak": red_peak / 1e9, "unit": "Gred/s",
-                        "frac": red_rate / red_peak,
-                        "peak_source": "mc_bench_red: random cells of one batch grid, 148x8 CTAs x 256 thr x 64 reds, best of 3"}
+                        "frac": red_rate / red_peak, "peak_table": red_table,
+                        "peak_source": "mc_bench_red: best of the random-cell rows of peak_table (occupancy x window sweep)"}
 
     if rank == 0:
         out = {"metric": "histories/s", "value": n_job * K / (total_ms * 1e-3), "unit": "histories/s",

@@ -159,8 +159,9 @@ typedef struct {
 
 /* mc_run_particles — as mc_run, but the source is a list: history h is particles[h], transported with track id (0,0)
  * from Philox block 0 (R13b).  A particle outside the phantom counts as escaped (no re-entry, R3).
- * particles: n records, HOST or DEVICE memory (a host list is validated and staged; a device list is read in place and
- * must already satisfy the constraints above).  Other arguments and errors as mc_run. */
+ * particles: n records, HOST or DEVICE memory (a host list is validated on the host and staged; a device list is
+ * validated by one kernel pass and read in place).  Errors: an energy outside (0, e_max_MeV] -> MC_ERR_ENERGY_RANGE, a
+ * direction that is not a unit vector or an unknown particle type -> MC_ERR_INVALID_ARG; otherwise as mc_run. */
 mc_status mc_run_particles(mc_ctx *ctx, const mc_particle *particles, uint64_t n, uint64_t seed, int32_t n_batches,
                            float *dose_out, float *sigma_out);
 
@@ -199,6 +200,8 @@ mc_status mc_ipc_close_handle(void *dev_ptr);
 mc_status mc_run_atten(mc_ctx *ctx, const mc_beam *beam, uint64_t n, uint64_t seed, int32_t *voxel_out,
                        uint8_t *channel_out);
 
+/* ---- Diagnostics: test and measurement hooks, not part of the hot path -------------------------------------------
+ * (mc_philox_selftest, mc_bench_red, mc_bench_issue: used by tests/ and bench.py only.) */
 /* Philox4x32-10 on the device: n blocks, ctr[4n], key[2n] -> out[4n] (host pointers). */
 mc_status mc_philox_selftest(const uint32_t *ctr, const uint32_t *key, int32_t n, uint32_t *out);
 
@@ -212,6 +215,8 @@ mc_status mc_bench_red(mc_ctx *ctx, uint32_t n_cells, int32_t per_thread, int32_
 /* mc_bench_issue — measures the transport roofline's denominator: 2 x 1024-thread CTAs per SM each run iters x 64
  * independent FFMAs per thread; *thread_instr_per_s (host) = FFMA thread-instructions per second achieved. */
 mc_status mc_bench_issue(mc_ctx *ctx, int32_t iters, double *thread_instr_per_s);
+
+/* ---- end of diagnostics ------------------------------------------------------------------------------------------- */
 
 mc_status mc_get_stats(const mc_ctx *ctx, mc_stats *out);
 /* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); 0 = default stream. */

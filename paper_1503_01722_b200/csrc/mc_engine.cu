@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -142,6 +143,30 @@ mc_status upload_tables(mc_ctx* ctx) {
     return MC_OK;
 }
 
+// The library's own memory pool for the particle queues, one per device, created on first use (thread-safe: function-local
+// statics), never destroyed: freed queues stay in it for the next context.
+cudaMemPool_t queue_pool() {
+    static std::mutex mu;
+    static std::vector<cudaMemPool_t> pools;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    std::lock_guard<std::mutex> lock(mu);
+    if ((int)pools.size() <= dev) pools.resize(dev + 1, nullptr);
+    if (!pools[dev]) {
+        cudaMemPoolProps props{};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t p = nullptr;
+        if (cudaMemPoolCreate(&p, &props) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        unsigned long long keep = ~0ull;
+        cudaMemPoolSetAttribute(p, cudaMemPoolAttrReleaseThreshold, &keep);
+        pools[dev] = p;
+    }
+    return pools[dev];
+}
+
 // shared memory of a transport CTA of T threads: tables + per-thread counters + per-thread energy ledger + track pool
 size_t smem_e(const mc_ctx* c, int T) {
     return (size_t)c->tabs.n_mat * e_stride(c->tabs.N) * sizeof(float2) + (size_t)kGroups * kSlots * T * sizeof(uint4) +
@@ -273,22 +298,16 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
     const uint32_t W = (uint32_t)std::min<uint64_t>((uint64_t)ctx->wave_size, std::max<uint64_t>(n_run, 1024));
     const uint32_t cap = (uint32_t)std::min<uint64_t>((uint64_t)W * (uint64_t)ctx->queue_factor, 0x7fffffffull / 3);
     if (cap > ctx->q_cap) {
-        // The queues are gigabytes: they come from the device's stream-ordered memory pool, which is told to keep freed
-        // memory (release threshold), so that a new context of the same process reuses them instead of paying
-        // cudaMalloc / cudaFree of several GB again (measured: 30 - 300 ms per context).
-        static bool pool_set = false;
-        if (!pool_set) {
-            int dev = 0; cudaMemPool_t pool;
-            if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-                unsigned long long keep = ~0ull;
-                cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-            }
-            cudaGetLastError();
-            pool_set = true;
-        }
+        // The queues are gigabytes: they come from a stream-ordered memory pool of the library's own (the device's default
+        // pool and its policy are left alone) that keeps freed memory, so that a later context of the same process
+        // reuses them instead of paying cudaMalloc / cudaFree of several GB again (measured: 30 - 300 ms per context).
+        cudaMemPool_t pool = queue_pool();
         for (auto& q : ctx->d_q) { if (q) cudaFreeAsync(q, ctx->stream); q = nullptr; }
         ctx->q_cap = 0;
-        for (auto& q : ctx->d_q) CU(cudaMallocAsync(&q, (size_t)cap * 3 * sizeof(uint4), ctx->stream));
+        for (auto& q : ctx->d_q) {
+            if (pool) CU(cudaMallocFromPoolAsync(&q, (size_t)cap * 3 * sizeof(uint4), pool, ctx->stream));
+            else CU(cudaMallocAsync(&q, (size_t)cap * 3 * sizeof(uint4), ctx->stream));
+        }
         ctx->q_cap = cap;
     }
     cudaStream_t s = ctx->stream;
@@ -772,7 +791,24 @@ mc_status mc_run_particles(mc_ctx* ctx, const mc_particle* particles, uint64_t n
         d_list = staged;
     }
     const size_t nvox = ctx->g.nvox;
-    st = ensure_edep(ctx, (size_t)n_batches * nvox);
+    st = MC_OK;
+    if (on_device) {
+        // a device-resident list is checked where it is: one pass, one flag word back (bit 0: energy not in (0, e_max],
+        // bit 1: direction not a unit vector, bit 2: unknown particle type)
+        cudaError_t e = cudaMemsetAsync(ctx->d_counters + C_DONE, 0, sizeof(uint32_t), ctx->stream);
+        if (e == cudaSuccess) {
+            check_particles_kernel<<<std::min<uint64_t>((n + kThreads - 1) / kThreads, (uint64_t)ctx->sm_count * 8), kThreads, 0, ctx->stream>>>(
+                d_list, (uint32_t)n, ctx->params.e_max_MeV, ctx->d_counters + C_DONE);
+            e = cudaGetLastError();
+        }
+        uint32_t bad = 0;
+        if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, ctx->d_counters + C_DONE, sizeof bad, cudaMemcpyDeviceToHost, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) st = fail(ctx, MC_ERR_CUDA, cudaGetErrorString(e));
+        else if (bad & 1u) st = fail(ctx, MC_ERR_ENERGY_RANGE, "particle energy not in (0, e_max_MeV]");
+        else if (bad & 6u) st = fail(ctx, MC_ERR_INVALID_ARG, "particle directions must be unit vectors and particle types -1, 0 or 1");
+    }
+    if (st == MC_OK) st = ensure_edep(ctx, (size_t)n_batches * nvox);
     if (st == MC_OK) st = transport(ctx, nullptr, d_list, n, 0, n, seed, n_batches, ctx->d_edep);
     if (st == MC_OK) st = finalize_device(ctx, ctx->d_edep, n, n_batches);
     if (st == MC_OK) {

@@ -888,6 +888,22 @@ __global__ void __launch_bounds__(kThreads) atten_kernel(const __grid_constant__
 // rule, R25), book the source / escaped energy, push a queue record (track id (0,0)) to the queue of its type.
 // =================================================================================================
 struct ListParticle { float x, y, z, u, v, w, E; int32_t particle; };  // = mc_particle (include/mc.h)
+// validation of a device-resident list (a host list is checked on the host): flags |= 1 energy not in (0, e_max],
+// 2 direction not a unit vector, 4 unknown particle type
+__global__ void __launch_bounds__(kThreads) check_particles_kernel(const ListParticle* __restrict__ list, uint32_t n, float e_max,
+                                                                   uint32_t* flags) {
+    uint32_t bad = 0u;
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const ListParticle p = list[i];
+        if (!(p.E > 0.0f) || !(p.E <= e_max)) bad |= 1u;
+        const float nn = p.u * p.u + p.v * p.v + p.w * p.w;
+        if (!(fabsf(nn - 1.0f) < 1e-3f)) bad |= 2u;
+        if (p.particle < -1 || p.particle > 1) bad |= 4u;
+    }
+    bad = __reduce_or_sync(kFull, bad);
+    if ((threadIdx.x & 31) == 0 && bad) atomicOr(flags, bad);
+}
+
 __global__ void __launch_bounds__(kThreads) load_particles_kernel(const __grid_constant__ RunParams P, const ListParticle* __restrict__ list,
                                                                   uint32_t n) {
     const Geometry& g = P.g;

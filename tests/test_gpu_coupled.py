@@ -126,11 +126,9 @@ def _check(out):
         for k in EVENTS:  # physics events per history: 1 %, or 5 standard errors of the count where that is larger
             tol = max(0.01 * ref[k], 5.0 * np.sqrt(2.0 * max(ref[k], 1e-9) / min(out["n_gpu"], out["n_orc"])), 1e-4)
             assert abs(r["per_history"][k] - ref[k]) <= tol, (seed, k, r["per_history"][k], ref[k], tol)
-        # Condensed-history steps: a voxel-limited step whose second leg ends a hair short of the face is
-        # followed by a tiny catch-up step; whether "short" or "on the face" is decided in fp32 here and in
-        # fp64 in the oracle (tolerance note), so the count differs by a few per cent while
-        # path, energy loss and dose do not.
-        assert r["per_history"]["e_steps"] == pytest.approx(ref["e_steps"], rel=0.08), (seed, r["per_history"], ref)
+        # Condensed-history steps per history: with reading R8 (no catch-up steps behind voxel-limited steps) the
+        # count no longer depends on fp32-vs-fp64 face decisions: 2 %.
+        assert r["per_history"]["e_steps"] == pytest.approx(ref["e_steps"], rel=0.02), (seed, r["per_history"], ref)
         assert r["n"] > 0
     same, indep = out[1], out[2]
     assert same["mean_diff"] <= 0.01, same
@@ -139,6 +137,8 @@ def _check(out):
         return
     assert indep["frac3"] >= 0.99, indep
     assert indep["mean_diff"] <= 0.01 + indep["noise"], indep
+    if indep["noise"] <= 0.8 * 0.003:  # mean combined sigma <= 0.3 % of Dmax: north_star's 1 % bar with no allowance
+        assert indep["mean_diff"] <= 0.01, indep
     # the independent run's difference must be explained by its noise (no hidden bias)
     assert indep["mean_diff"] <= 1.25 * indep["noise"] + 0.002, indep
 
@@ -358,25 +358,78 @@ def test_more_materials_pick_a_smaller_cta_and_give_the_same_histories():
     eng.close()
 
 
-def test_depth_dose_and_total_energy_agree_at_high_statistics():
-    """Laterally integrated depth-dose curve of config 2: the engine with 1e8 histories against the oracle with 1e7
-    (independent streams).  The integration removes most of the noise, so a systematic difference of a few 0.1 % in
-    range, energy loss or scattering would show (measured: 0.03 % of the maximum, energy ratio 1.00001)."""
-    cfg = W.config(2)
-    eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])
-    orc = oracle.Oracle(cfg["phantom"], cfg["materials"], cfg["params"])
-    do, _, sto = orc.run(cfg["beam"], 10 ** 7, 1, 40, workers=WORKERS)
-    dg, _ = eng.run(cfg["beam"], 10 ** 8, 7, 40)
+HIGH_STAT = [  # (config, beam, engine histories, oracle histories, block size for the oracle's statistics)
+    pytest.param(2, None, 10 ** 8, 10 ** 7, id="config2_15MeV_e_water"),
+    pytest.param(3, None, 4 * 10 ** 8, 4 * 10 ** 7, id="config3_6MV_photons_water"),
+    pytest.param(4, "e", 10 ** 8, 10 ** 7, id="config4_slab_electrons"),
+    pytest.param(4, "g", 4 * 10 ** 8, 4 * 10 ** 7, id="config4_slab_photons"),
+    pytest.param(5, "e", 10 ** 8, 4 * 10 ** 6, id="config5_halfslab_electrons"),
+]
+
+
+def _curves(edep, rho, dims, voxel_cm, n_total):
+    """Per-batch integrated curves from per-batch energy grids [B, nvox] (MeV): the depth curve (energy per history
+    and slab) and two lateral profiles (mean dose over y and a 3 cm slab, depths 1-4 cm and 4-7 cm).  Returns
+    {name: (mean over batches, standard error of that mean)}."""
+    B = edep.shape[0]
+    nx, ny, nz = dims
+    h = float(voxel_cm[2])
+    nb = np.array([-(-(b + 1) * n_total // B) - -(-b * n_total // B) for b in range(B)], np.float64)  # batch sizes (R18)
+    inv_mass = 1.0 / (rho.reshape(nz, ny, nx).astype(np.float64) * float(np.prod(voxel_cm)))
+    per = {"depth": [], "profile_1_4cm": [], "profile_4_7cm": []}
+    for b in range(B):
+        e = edep[b].reshape(nz, ny, nx).astype(np.float64) / nb[b]
+        per["depth"].append(e.sum(axis=(1, 2)))
+        for name, (z0, z1) in (("profile_1_4cm", (1.0, 4.0)), ("profile_4_7cm", (4.0, 7.0))):
+            k0, k1 = int(round(z0 / h)), int(round(z1 / h))
+            per[name].append((e[k0:k1] * inv_mass[k0:k1]).mean(axis=(0, 1)))
+    out = {}
+    for k, v in per.items():
+        a = np.stack(v)
+        out[k] = (a.mean(axis=0), a.std(axis=0, ddof=1) / np.sqrt(B))
+    return out
+
+
+@pytest.mark.parametrize("c,beam,n_gpu,n_orc", HIGH_STAT)
+def test_depth_dose_profiles_and_total_energy_agree_at_high_statistics(c, beam, n_gpu, n_orc):
+    """Integrated curves at high statistics, independent streams (engine seed 7, oracle seed 1): the laterally
+    integrated depth-dose curve, two lateral profiles (PAPER.md:92 compares profiles at fixed depths) and the deposited
+    fraction of the source energy.  Integration removes most of the noise, so a systematic difference of a few 0.1 % in
+    range, energy loss, scattering or interface handling would show.
+    Bars: depth curve within 0.3 % of its maximum, no noise allowance; profiles within 0.3 % of their maximum plus 4
+    standard errors of the difference at that point (from the 20 batches of each side; the oracle's statistics are
+    what 30 s of the host cores buy); deposited energy fraction within 5e-4."""
+    cfg = W.config(c, beam) if beam else W.config(c)
+    ph = cfg["phantom"]
+    B = 20
+    eng = mc.Engine(ph, cfg["materials"], cfg["params"])
+    orc = oracle.Oracle(ph, cfg["materials"], cfg["params"])
+    eo, sto = orc.run_edep_parallel(cfg["beam"], n_orc, 1, B, WORKERS)
+    co = _curves(eo, ph["density"], eng.dims, ph["voxel_cm"], n_orc)
+    del eo
+    eg = np.zeros((B, eng.nvox), np.float32)
+    mc.mc_run_range(eng.ctx, cfg["beam"], n_gpu, 0, n_gpu, 7, B, eg)
     st = eng.stats()
+    cg = _curves(eg, ph["density"], eng.dims, ph["voxel_cm"], n_gpu)
+    del eg
     eng.close()
-    nx, ny, nz = (int(x) for x in cfg["phantom"]["dims"])
-    rho = cfg["phantom"]["density"].reshape(nz, ny, nx).astype(np.float64)
-    zo = (do.reshape(nz, ny, nx) * rho).sum(axis=(1, 2))
-    zg = (dg.astype(np.float64).reshape(nz, ny, nx) * rho).sum(axis=(1, 2))
-    assert np.max(np.abs(zg - zo)) / zo.max() < 2e-3
-    assert zg.sum() / zo.sum() == pytest.approx(1.0, abs=5e-4)
-    # deposited fraction of the source energy, per history
-    assert st["e_deposited_MeV"] / st["e_source_MeV"] == pytest.approx(sto["e_dep"] / sto["e_src"], abs=5e-4)
-    # 15 MeV electrons stop: the dose beyond ~the CSDA range (8.7 cm restricted, PAPER.md:94 "fell quickly to zero")
-    # is bremsstrahlung tail only
-    assert zg[int(10.0 / 0.5):].max() < 0.02 * zg.max()
+    res = {}
+    for k in co:
+        (mo, so), (mg, sg) = co[k], cg[k]
+        diff, sd = np.abs(mg - mo), np.sqrt(so ** 2 + sg ** 2)
+        res[k] = {"max_diff": float(diff.max() / mo.max()), "max_sigma": float(sd.max() / mo.max()),
+                  "worst_excess": float(np.max(diff - 4.0 * sd) / mo.max())}
+    res["energy"] = float(cg["depth"][0].sum() / co["depth"][0].sum())
+    res["e_frac"] = (st["e_deposited_MeV"] / st["e_source_MeV"], sto["e_dep"] / sto["e_src"])
+    print(c, beam, res)
+    assert res["depth"]["max_diff"] < 3e-3, res
+    for k in ("profile_1_4cm", "profile_4_7cm"):
+        assert res[k]["worst_excess"] < 3e-3, (k, res)
+        assert res[k]["max_diff"] < 1e-2, (k, res)  # north_star's bar, point by point, no allowance
+    assert res["energy"] == pytest.approx(1.0, abs=5e-4), res
+    assert res["e_frac"][0] == pytest.approx(res["e_frac"][1], abs=5e-4), res
+    if c == 2:
+        # 15 MeV electrons stop: the dose beyond ~the CSDA range (8.7 cm restricted, PAPER.md:94 "fell quickly to
+        # zero") is bremsstrahlung tail only
+        zg = cg["depth"][0]
+        assert zg[int(10.0 / 0.5):].max() < 0.02 * zg.max()

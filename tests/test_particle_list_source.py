@@ -111,4 +111,17 @@ def test_mc_run_particles_matches_the_oracle():
     bad = p[:10].copy(); bad["u"][2] = 0.9
     with pytest.raises(mc.McError):
         mc.mc_run_particles(eng.ctx, bad, 1, 2, d, s)
+    # ... and of a device-resident list (checked by one kernel pass, same error codes)
+    bad = p[:1000].copy(); bad["E"][777] = 25.0
+    tb = torch.from_numpy(bad.view(np.uint8).reshape(-1)).cuda()
+    with pytest.raises(mc.McError) as e:
+        mc.mc_run_particles(eng.ctx, tb, 1, 2, d2, s2, n=len(bad))
+    assert e.value.status == mc.MC_ERR_ENERGY_RANGE
+    bad = p[:1000].copy(); bad["u"][5] = 0.9
+    tb = torch.from_numpy(bad.view(np.uint8).reshape(-1)).cuda()
+    with pytest.raises(mc.McError) as e:
+        mc.mc_run_particles(eng.ctx, tb, 1, 2, d2, s2, n=len(bad))
+    assert e.value.status == mc.MC_ERR_INVALID_ARG
+    mc.mc_run_particles(eng.ctx, t, 2, B, d2, s2, n=n)  # the context still works after a rejected list
+    assert np.allclose(d2.cpu().numpy(), d, rtol=1e-4, atol=1e-6 * d.max())
     eng.close()
