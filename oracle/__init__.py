@@ -17,7 +17,7 @@ from . import build as _build
 _lib = None
 
 TABLE_IDS = {"mu_tot": 0, "mu_C": 1, "mu_pp": 2, "R": 3, "L": 4, "S_hard": 5, "S_M": 6, "S_max": 7, "K1": 8,
-             "mu_maj": 9}
+             "mu_maj": 9, "lnA": 10}
 STAT_NAMES = ["e_src", "e_dep", "e_esc", "e_cutdep", "n_hist", "n_flight", "n_fict", "n_compton", "n_pair",
               "n_pe", "n_estep", "n_moller", "n_brems", "n_sec_e", "n_sec_g", "path_e", "lim_vox", "lim_maxs",
               "lim_maxe", "lim_range", "lim_event", "max_ledger_rel"]
@@ -168,7 +168,7 @@ class Oracle:
 
     def eval(self, which, E, arg=0.0, m=0):
         ids = {"sigma_kn": 0, "mu_C": 1, "mu_pe": 2, "mu_pp": 3, "L_col": 4, "L_rad": 5, "S_M": 6, "S_br": 7,
-               "K1": 8, "delta": 9, "brems_kdsdk": 10, "moller_dsde": 11}
+               "K1": 8, "delta": 9, "brems_kdsdk": 10, "moller_dsde": 11, "S_el": 12}
         return lib().orc_eval(self._h, int(m), ids[which], float(E), float(arg))
 
     def lerp(self, name, E, m=0):
@@ -361,6 +361,53 @@ def rotate(d, mu, phi):
     o = (C.c_double * 3)()
     lib().orc_rotate(di, float(mu), float(phi), o)
     return np.array(o[:])
+
+
+# -- Goudsmit-Saunderson multiple scattering (orc_gs.h; R27) -----------------------------------------
+def gs_dims():
+    o = (C.c_int * 3)()
+    lib().orc_gs_dims(o)
+    return tuple(o)
+
+
+def gs_nodes():
+    nt, na, nq = gs_dims()
+    t, A, r = np.zeros(nt), np.zeros(na), np.zeros(nq)
+    lib().orc_gs_nodes(_dp(t), _dp(A), _dp(r))
+    return t, A, r
+
+
+def gs_table():
+    """ln of the quantiles of 1 - cos(theta): [NT, NA, NQ]."""
+    nt, na, nq = gs_dims()
+    o = np.zeros((nt, na, nq))
+    lib().orc_gs_table(_dp(o))
+    return o
+
+
+def gs_moments(A, lmax):
+    o = np.zeros(lmax + 1)
+    lib().orc_gs_moments(C.c_double(A), int(lmax), _dp(o))
+    return o
+
+
+def gs_G1(A):
+    lib().orc_gs_G1.restype = C.c_double
+    return lib().orc_gs_G1(C.c_double(A))
+
+
+def gs_cdf(lam, A, x):
+    x = np.ascontiguousarray(x, np.float64)
+    o = np.zeros(len(x))
+    lib().orc_gs_cdf(C.c_double(lam), C.c_double(A), _dp(x), int(len(x)), _dp(o))
+    return o
+
+
+def gs_sample(t, A, n, seed=1):
+    """n samples of cos(theta) from the table sampler transport uses."""
+    o = np.zeros(n)
+    lib().orc_gs_sample(C.c_double(t), C.c_double(A), C.c_uint64(n), C.c_uint64(seed), _dp(o))
+    return o
 
 
 def sample_ms(a, n, seed=1):

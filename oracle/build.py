@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB = os.path.join(HERE, "liborc.so")
 SRC = [os.path.join(HERE, "orc_main.cpp")]
-DEPS = SRC + [os.path.join(HERE, "orc_physics.h")]
+DEPS = SRC + [os.path.join(HERE, "orc_physics.h"), os.path.join(HERE, "orc_gs.h")]
 
 
 def build(force=False):

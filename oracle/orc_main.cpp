@@ -15,6 +15,7 @@
 // Coupled dose: "parity unpinned" by any external number (no dose value in the paper is
 // reproducible here: gDPM, XCOM data and the 6 MV spectrum are missing) — DESIGN.md says so.
 #include "orc_physics.h"
+#include "orc_gs.h"
 #include <cstdint>
 #include <cstring>
 #include <cstdio>
@@ -52,10 +53,12 @@ struct Stream {
 
 // ------------------------------------------------------------------------------------------------
 struct Params { double e_cut, g_cut, e_max; int n_grid; double d_maxs, f_maxe; uint32_t flags; };
-enum { F_NO_HARD = 1, F_NO_MS = 2, F_LOCAL_SEC = 4 };
+enum { F_NO_HARD = 1, F_NO_MS = 2, F_LOCAL_SEC = 4, F_MS_GS = 8 };
+static GsTable g_gs;  // the Goudsmit-Saunderson sampling table (material independent, orc_gs.h), built on first use
 
 struct MatTables {  // all per unit density (cm^2/g, MeV cm^2/g, g/cm^2), one value per grid node
     std::vector<double> mu_tot, mu_C, mu_pp, R, L, S_hard, S_M, S_max, K1;
+    std::vector<double> lnA;  // ln of the effective screening parameter (R27): K1 = S_el G_1(A)
 };
 
 struct Ctx {
@@ -122,7 +125,7 @@ static void build_tables(Ctx& c) {
     for (size_t m = 0; m < nm; ++m) {
         const Material& M = c.mats[m];
         MatTables& t = c.tab[m];
-        for (auto* v : {&t.mu_tot, &t.mu_C, &t.mu_pp, &t.R, &t.L, &t.S_hard, &t.S_M, &t.S_max, &t.K1}) v->assign(N, 0.0);
+        for (auto* v : {&t.mu_tot, &t.mu_C, &t.mu_pp, &t.R, &t.L, &t.S_hard, &t.S_M, &t.S_max, &t.K1, &t.lnA}) v->assign(N, 0.0);
         for (int j = 0; j < N; ++j) {
             t.mu_C[j] = mu_compton(M, E[j]);
             t.mu_pp[j] = mu_pp(M, E[j]);
@@ -132,6 +135,7 @@ static void build_tables(Ctx& c) {
             t.S_hard[j] = t.S_M[j] + brems_sigma(M, E[j], c.p.g_cut);
             t.S_max[j] = std::max(t.S_hard[j], j ? t.S_max[j - 1] : 0.0);
             t.K1[j] = K1(M, E[j]);
+            t.lnA[j] = std::log(gs_effective_A(t.K1[j], S_el(M, E[j])));
         }
         // range: R(e_cut) = 0, R(T) = int_{e_cut}^{T} dT'/L(T'), Simpson in ln T between nodes
         auto seg = [&](int j) {  // integral from node j to node j+1
@@ -149,6 +153,7 @@ static void build_tables(Ctx& c) {
     for (int j = 0; j < N; ++j)
         for (size_t m = 0; m < nm; ++m) c.mu_maj[j] = std::max(c.mu_maj[j], rmax[m] * c.tab[m].mu_tot[j]);
     c.have_tables = true;
+    if (c.p.flags & F_MS_GS) g_gs.build();
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -460,8 +465,20 @@ struct Run {
                 double tu = std::max(tq, 0.0);
                 ms_carry = tq - tu;
                 q_used += tu;
-                double am = 1.0 - std::exp(-tu);
-                if (am > 0.0) rotate_dir(p.d, 1.0 - sample_ms_omu(am, s.u(2)), 2.0 * PI * s.u(3));
+                if (P.flags & F_MS_GS) {
+                    // Goudsmit-Saunderson angle (R27): scattering power below the table is not sampled
+                    // now but carried (R8b)
+                    if (tu < GS_T_MIN) {
+                        if (c.ms_carry) ms_carry += tu;
+                        q_used -= tu;
+                    } else {
+                        double A = std::exp(lerp_tab(c, t.lnA, Tmid));
+                        rotate_dir(p.d, 1.0 - gs_sample_omu(g_gs, tu, A, s.w[2], s.w[3]), 2.0 * PI * s.u(3));
+                    }
+                } else {
+                    double am = 1.0 - std::exp(-tu);
+                    if (am > 0.0) rotate_dir(p.d, 1.0 - sample_ms_omu(am, s.u(2)), 2.0 * PI * s.u(3));
+                }
             }
             double rest = (1.0 - xi) * d;
             double tf = face_dist(p.x, p.d, p.v, ax);
@@ -644,7 +661,7 @@ int orc_build_tables(Ctx* c, const orc_material* mats, int n_mats, const orc_par
     build_tables(*c);
     return 0;
 }
-void orc_set_flags(Ctx* c, uint32_t flags) { c->p.flags = flags; }
+void orc_set_flags(Ctx* c, uint32_t flags) { c->p.flags = flags; if (flags & F_MS_GS) g_gs.build(); }
 
 // grid description: out[0]=lnE0, out[1]=dln, out[2]=N, out[3]=k_cut
 void orc_grid(const Ctx* c, double* out) { out[0] = c->lnE0; out[1] = c->dln; out[2] = c->N; out[3] = c->k_cut; }
@@ -656,8 +673,8 @@ int orc_table(const Ctx* c, int m, int which, double* out) {
     else {
         if (m < 0 || m >= (int)c->tab.size()) return 1;
         const MatTables& t = c->tab[m];
-        const std::vector<double>* all[9] = {&t.mu_tot, &t.mu_C, &t.mu_pp, &t.R, &t.L, &t.S_hard, &t.S_M, &t.S_max, &t.K1};
-        if (which < 0 || which > 8) return 1;
+        const std::vector<double>* all[11] = {&t.mu_tot, &t.mu_C, &t.mu_pp, &t.R, &t.L, &t.S_hard, &t.S_M, &t.S_max, &t.K1, nullptr, &t.lnA};
+        if (which < 0 || which > 10 || which == 9) return 1;
         v = all[which];
     }
     std::memcpy(out, v->data(), sizeof(double) * v->size());
@@ -682,6 +699,7 @@ double orc_eval(const Ctx* c, int m, int which, double E, double arg) {
         case 6: return M.ne * moller_sigma(E, arg);
         case 7: return brems_sigma(M, E, arg);
         case 8: return K1(M, E);
+        case 12: return S_el(M, E);
         case 9: return density_effect(M, E);
         case 10: return brems_kdsdk(M, E, arg);
         case 11: return moller_dsde(E, arg);
@@ -801,6 +819,30 @@ void orc_sample_brems(const Ctx* c, int m, double T0, uint64_t n, uint64_t seed,
     }
 }
 // MS polar cosine for a given a = 1 - exp(-K1 rho d) (word 2 of the step block, as in transport)
+// ---- Goudsmit-Saunderson entries for the pins (the functions transport calls) ----------------------------------------
+void orc_gs_dims(int* out) { out[0] = GS_NT; out[1] = GS_NA; out[2] = GS_NQ; }
+void orc_gs_nodes(double* t, double* A, double* r) {
+    for (int i = 0; i < GS_NT; ++i) t[i] = gs_t_node(i);
+    for (int j = 0; j < GS_NA; ++j) A[j] = gs_A_node(j);
+    for (int k = 0; k < GS_NQ; ++k) r[k] = gs_r_node(k);
+}
+void orc_gs_table(double* out) { g_gs.build(); std::memcpy(out, g_gs.y.data(), sizeof(double) * g_gs.y.size()); }
+void orc_gs_moments(double A, int lmax, double* out) { std::vector<double> g = gs_moments(A, lmax); std::memcpy(out, g.data(), sizeof(double) * (lmax + 1)); }
+double orc_gs_G1(double A) { return gs_G1(A); }
+void orc_gs_cdf(double lambda, double A, const double* x, int n, double* out) {
+    std::vector<double> S = gs_cdf(lambda, A, std::vector<double>(x, x + n));
+    std::memcpy(out, S.data(), sizeof(double) * n);
+}
+// n samples of mu = cos(theta) for scattering power t and screening A, words 2 and 3 of block 0 of stream (seed, history i)
+void orc_gs_sample(double t, double A, uint64_t n, uint64_t seed, double* out) {
+    g_gs.build();
+    for (uint64_t i = 0; i < n; ++i) {
+        Stream s = pin_stream(i, seed);
+        s.next();
+        out[i] = 1.0 - gs_sample_omu(g_gs, t, A, s.w[2], s.w[3]);
+    }
+}
+
 void orc_sample_ms(double am, uint64_t n, uint64_t seed, double* out) {
     for (uint64_t i = 0; i < n; ++i) {
         Stream s = pin_stream(i, seed);

@@ -162,4 +162,18 @@ inline double K1(const Material& m, double T) {
     return NA * s;
 }
 
+// Total elastic cross section of the same screened-Rutherford law (cm^2/g): per element
+// sigma_el = pi r_e^2 Z(Z+1) (1 - beta^2)/beta^4 / (A_i (1 + A_i))  (integral of the law K1 is the first moment of).
+inline double S_el(const Material& m, double T) {
+    double tau = T / MEC2, g = tau + 1.0, b2 = 1.0 - 1.0 / (g * g), bg2 = g * g - 1.0;
+    double s = 0;
+    for (size_t i = 0; i < m.Z.size(); ++i) {
+        double Z = m.Z[i];
+        double az = ALPHA * Z;
+        double Ai = ALPHA * ALPHA * std::pow(Z, 2.0 / 3.0) / (4.0 * 0.885 * 0.885 * bg2) * (1.13 + 3.76 * az * az / b2);
+        s += m.w[i] / m.A[i] * PI * RE * RE * Z * (Z + 1.0) * (1.0 - b2) / (b2 * b2) / (Ai * (1.0 + Ai));
+    }
+    return NA * s;
+}
+
 }  // namespace orc

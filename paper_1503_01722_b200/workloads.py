@@ -61,6 +61,7 @@ def params(e_cut=0.2, g_cut=0.01, e_max=20.0, n_grid=256, d_maxs=0.5, f_maxe=0.2
 FLAG_NO_HARD = 1        # no Moller / bremsstrahlung events
 FLAG_NO_MS = 2          # no multiple-scattering deflection
 FLAG_LOCAL_SECONDARIES = 4  # secondaries are deposited where they are born
+FLAG_MS_GS = 8          # Goudsmit-Saunderson multiple-scattering angle instead of the Gaussian model (R27)
 
 
 # --- phantoms ------------------------------------------------------------------------------------
