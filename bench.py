@@ -50,6 +50,7 @@ def parse():
                     "own five cases (128^3 x 0.25 cm, 2x2 cm^2 field: context beside its Tables 2-3)")
     ap.add_argument("--beam", default=None, choices=[None, "e", "g"], help="configs 4, 5: electron or photon beam")
     ap.add_argument("--histories", type=int, default=0, help="override n_histories (the line then says so)")
+    ap.add_argument("--ms-model", default="gaussian", choices=["gaussian", "gs"], help="multiple-scattering angle model (north_star: Gaussian or Goudsmit-Saunderson)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--option", action="append", default=[], help="engine option name=value (mc_set_option)")
@@ -116,6 +117,8 @@ def workload(args):
     cfg = W.config(args.config, args.beam)
     if args.histories:
         cfg["n_histories"] = args.histories
+    if args.ms_model == "gs":  # Goudsmit-Saunderson angle instead of the Gaussian model (R27); the line says so
+        cfg["params"] = dict(cfg["params"], flags=cfg["params"]["flags"] | W.FLAG_MS_GS)
     return cfg
 
 
@@ -124,7 +127,7 @@ def config_dict(cfg, args, extra=None):
          "n_batches": cfg["n_batches"], "dims": [int(x) for x in cfg["phantom"]["dims"]],
          "voxel_cm": float(cfg["phantom"]["voxel_cm"][0]), "e_cut_MeV": cfg["params"]["e_cut_MeV"],
          "g_cut_MeV": cfg["params"]["g_cut_MeV"], "seed": cfg["seed"],
-         "histories_overridden": bool(args.histories)}
+         "histories_overridden": bool(args.histories), "ms_model": args.ms_model}
     d.update(extra or {})
     return d
 

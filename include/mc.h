@@ -63,6 +63,9 @@ typedef struct {
 #define MC_FLAG_NO_HARD_EVENTS 1u     /* no Moller / bremsstrahlung events (d_event = inf)        */
 #define MC_FLAG_NO_MS 2u              /* no multiple-scattering deflection                        */
 #define MC_FLAG_LOCAL_SECONDARIES 4u  /* secondaries deposit their energy where they are born     */
+#define MC_FLAG_MS_GS 8u              /* multiple-scattering angle from the Goudsmit-Saunderson distribution of the
+                                         screened-Rutherford law ("the method developed by Kawrakow";
+                                         DESIGN.md R27) instead of the Gaussian model (R7)                        */
 
 /* Cut-offs and step limits (PAPER.md:39 "user defined maximum step size", :86 cut-off energies).
  * e_cut_MeV: electron absorption energy = Moller delta-ray threshold; g_cut_MeV: photon absorption
@@ -132,6 +135,11 @@ mc_status mc_build_tables(mc_ctx *ctx, const mc_material *mats, int32_t n_mats, 
  * 4 L (MeV cm^2/g) 5 Sigma_hard 6 Sigma_Moller 7 Sigma_max 8 K1 (cm^2/g); material = -1, which = 9:
  * photon majorant mu_maj (1/cm).  out: n_grid floats (host). */
 mc_status mc_export_table(const mc_ctx *ctx, int32_t material, int32_t which, float *out);
+/* which = 10: ln of the effective screening parameter of the Goudsmit-Saunderson model (R27).
+ * mc_export_gs_table — the material-independent Goudsmit-Saunderson sampling table (R27): dims = {NT, NA, NQ};
+ * t_nodes[NT] (may be NULL) the scattering-power nodes; y[NT*NA*NQ] (may be NULL) ln of the quantiles of
+ * 1 - cos(theta).  Host pointers; needs no context and no device (the table is built on the host). */
+mc_status mc_export_gs_table(int32_t dims[3], float *t_nodes, float *y);
 /* grid[0] = ln E_0, grid[1] = delta ln E, grid[2] = n_grid, grid[3] = node index of e_cut. */
 mc_status mc_export_grid(const mc_ctx *ctx, double grid[4]);
 /* Replace the PHOTON tables by user-supplied data ("physics data ... stored in a database",

@@ -25,10 +25,10 @@ STATUS_NAMES = ["MC_OK", "MC_ERR_INVALID_ARG", "MC_ERR_STATE", "MC_ERR_ENERGY_RA
                 "MC_ERR_OOM", "MC_ERR_CUDA"]
 MC_FLAG_NO_HARD_EVENTS, MC_FLAG_NO_MS, MC_FLAG_LOCAL_SECONDARIES = 1, 2, 4
 TABLE_IDS = {"mu_tot": 0, "mu_C": 1, "mu_pp": 2, "R": 3, "L": 4, "S_hard": 5, "S_M": 6, "S_max": 7, "K1": 8,
-             "mu_maj": 9}
+             "mu_maj": 9, "lnA": 10}
 
 # every symbol include/mc.h declares (tests check that the library exports each of them)
-SYMBOLS = ["mc_create", "mc_destroy", "mc_build_tables", "mc_export_table", "mc_export_grid",
+SYMBOLS = ["mc_create", "mc_destroy", "mc_build_tables", "mc_export_table", "mc_export_grid", "mc_export_gs_table",
            "mc_set_photon_tables", "mc_run", "mc_run_particles", "mc_run_range", "mc_finalize", "mc_edep_buffer",
            "mc_finalize_multi", "mc_ipc_get_handle", "mc_ipc_open_handle", "mc_ipc_close_handle", "mc_run_atten",
            "mc_philox_selftest", "mc_bench_red", "mc_bench_issue", "mc_get_stats", "mc_set_stream", "mc_set_option",
@@ -180,6 +180,16 @@ def mc_export_grid(ctx):
     g = np.zeros(4)
     _check(ctx, lib().mc_export_grid(ctx, g.ctypes.data))
     return {"lnE0": g[0], "dln": g[1], "N": int(g[2]), "k_cut": int(g[3])}
+
+
+def mc_export_gs_table():
+    """The Goudsmit-Saunderson sampling table (R27): (t_nodes[NT], y[NT, NA, NQ] = ln of the quantiles of 1 - cos theta)."""
+    dims = (C.c_int32 * 3)()
+    _check(None, lib().mc_export_gs_table(dims, None, None))
+    t = np.zeros(dims[0], np.float32)
+    y = np.zeros((dims[0], dims[1], dims[2]), np.float32)
+    _check(None, lib().mc_export_gs_table(dims, t.ctypes.data_as(C.c_void_p), y.ctypes.data_as(C.c_void_p)))
+    return t, y
 
 
 def mc_export_table(ctx, name, material=0):

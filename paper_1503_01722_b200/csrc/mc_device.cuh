@@ -90,6 +90,12 @@ struct RunParams {
     // table coordinate <-> energy in base 2: ex = lg2(T) * ex_a - ex_b;  T = ex2(ex * t_a + t_b)
     float ex_a, ex_b, t_a, t_b;
     uint32_t seed_rk[10];     // seed_lo + r * 0xBB67AE85: Philox round keys of the second key word
+    // Goudsmit-Saunderson angle (flags & 8; R27): quantile table (log2 of 1 - cos theta) followed by the per-material
+    // coarse (every 8th node) ln A table as (value, slope) pairs; 1 - exp(-t) at the t-nodes; grid constants
+    const float* gs;
+    int gs_words, gs_n8;      // floats to stage; coarse ln A entries per material
+    float gs_an[16];
+    float gs_c0, gs_inv_dc, gs_lnA0, gs_inv_dA;
     float hinge_overrun;      // DESIGN.md R8
     int ms_carry;             // DESIGN.md R8b
 };

@@ -32,6 +32,9 @@ struct mc_ctx {
     uint2* d_vox = nullptr;
     float2 *d_tabP = nullptr, *d_tabE = nullptr;
     size_t tabP_cap = 0, tabE_cap = 0;
+    float* d_gs = nullptr;  // Goudsmit-Saunderson quantile table + per-material coarse ln A table (flags & MC_FLAG_MS_GS)
+    size_t gs_cap = 0, gs_words = 0;
+    int gs_n8 = 0;
     uint4* d_q[3] = {nullptr, nullptr, nullptr};  // electron A, electron B, photon
     uint32_t q_cap = 0;
     uint32_t* d_counters = nullptr;
@@ -71,6 +74,7 @@ mc_status fail(mc_ctx* c, mc_status s, const std::string& msg) {
                         std::string(#call) + ": " + cudaGetErrorString(e_));                       \
     } while (0)
 
+int gs_coarse_nodes(int N) { return (N - 1 + 7) / 8 + 1; }  // ln A is kept on every 8th node of the energy grid
 size_t e_stride(int N) { return ((size_t)kETabUnits * N + 1) & ~(size_t)1; }  // float2 per material, 16-byte multiple
 
 std::vector<float2> pairs(const float* t, int N) {  // (value, slope to the next node); fp32 subtraction (R20)
@@ -139,6 +143,23 @@ mc_status upload_tables(mc_ctx* ctx) {
     if (E.size() > ctx->tabE_cap) { cudaFree(ctx->d_tabE); ctx->d_tabE = nullptr; CU(cudaMalloc(&ctx->d_tabE, E.size() * sizeof(float2))); ctx->tabE_cap = E.size(); }
     CU(cudaMemcpy(ctx->d_tabP, P.data(), P.size() * sizeof(float2), cudaMemcpyHostToDevice));
     CU(cudaMemcpy(ctx->d_tabE, E.data(), E.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    if (ctx->params.flags & MC_FLAG_MS_GS) {
+        // quantile table as log2 x (one EX2 per sample), then per material ln A on every 8th energy node as (value, slope)
+        const GsTable& G = gs_table();
+        const int n8 = gs_coarse_nodes(N);
+        std::vector<float> buf(G.y.size() + (size_t)nm * n8 * 2);
+        for (size_t k = 0; k < G.y.size(); ++k) buf[k] = (float)((double)G.y[k] * 1.4426950408889634);
+        for (int m = 0; m < nm; ++m)
+            for (int k = 0; k < n8; ++k) {
+                const std::vector<float>& la = t.t[T_LNA][m];
+                const float v0 = la[std::min(8 * k, N - 1)], v1 = la[std::min(8 * k + 8, N - 1)];
+                buf[G.y.size() + 2 * ((size_t)m * n8 + k)] = v0;
+                buf[G.y.size() + 2 * ((size_t)m * n8 + k) + 1] = v1 - v0;
+            }
+        if (buf.size() > ctx->gs_cap) { cudaFree(ctx->d_gs); ctx->d_gs = nullptr; CU(cudaMalloc(&ctx->d_gs, buf.size() * sizeof(float))); ctx->gs_cap = buf.size(); }
+        CU(cudaMemcpy(ctx->d_gs, buf.data(), buf.size() * sizeof(float), cudaMemcpyHostToDevice));
+        ctx->gs_words = buf.size(); ctx->gs_n8 = n8;
+    }
     ctx->tables_dirty = false;
     return MC_OK;
 }
@@ -169,8 +190,10 @@ cudaMemPool_t queue_pool() {
 
 // shared memory of a transport CTA of T threads: tables + per-thread counters + per-thread energy ledger + track pool
 size_t smem_e(const mc_ctx* c, int T) {
+    const size_t gs = (c->params.flags & MC_FLAG_MS_GS)
+                          ? ((size_t)kGsNT * kGsNA * kGsNQ + 2 * (size_t)c->tabs.n_mat * gs_coarse_nodes(c->tabs.N)) * sizeof(float) : 0;
     return (size_t)c->tabs.n_mat * e_stride(c->tabs.N) * sizeof(float2) + (size_t)kGroups * kSlots * T * sizeof(uint4) +
-           2 * (size_t)T * sizeof(uint32_t) + (size_t)(T / 32) * (2 * sizeof(double) + 8 * sizeof(uint32_t));
+           2 * (size_t)T * sizeof(uint32_t) + (size_t)(T / 32) * (2 * sizeof(double) + 8 * sizeof(uint32_t)) + gs;
 }
 size_t smem_p(const mc_ctx* c, int T) {
     return (size_t)(1 + c->tabs.n_mat * TP_COUNT) * c->tabs.N * sizeof(float2) + (size_t)SP_COUNT * T * sizeof(uint32_t) +
@@ -265,6 +288,14 @@ void fill_params(const mc_ctx* ctx, RunParams& P) {
     P.ex_a = (float)(ln2 / t.dln); P.ex_b = (float)(t.lnE0 / t.dln);
     P.t_a = (float)(t.dln * log2e); P.t_b = (float)(t.lnE0 * log2e);
     P.hinge_overrun = 0.01f * (float)ctx->hinge_overrun_pct; P.ms_carry = (int)ctx->ms_carry;
+    if (ctx->params.flags & MC_FLAG_MS_GS) {
+        const GsTable& G = gs_table();
+        P.gs = ctx->d_gs; P.gs_words = (int)ctx->gs_words; P.gs_n8 = ctx->gs_n8;
+        for (int i = 0; i < kGsNT; ++i) P.gs_an[i] = G.an[i];
+        const double c0 = gs_grid_coordinate(kGsTMin), c1 = gs_grid_coordinate(kGsTMax);
+        P.gs_c0 = (float)c0; P.gs_inv_dc = (float)((kGsNT - 1) / (c1 - c0));
+        P.gs_lnA0 = (float)std::log(kGsAMin); P.gs_inv_dA = (float)((kGsNA - 1) / std::log(kGsAMax / kGsAMin));
+    }
 }
 
 }  // namespace
@@ -579,7 +610,7 @@ mc_status mc_create(const uint8_t* material_idx, const float* density_gcc, const
 void mc_destroy(mc_ctx* ctx) {
     if (!ctx) return;
     if (ctx->dev_ready) {
-        cudaFree(ctx->d_vox); cudaFree(ctx->d_tabP); cudaFree(ctx->d_tabE);
+        cudaFree(ctx->d_vox); cudaFree(ctx->d_tabP); cudaFree(ctx->d_tabE); cudaFree(ctx->d_gs);
         for (auto q : ctx->d_q) if (q) cudaFreeAsync(q, nullptr);  // back to the pool (see transport())
         cudaFree(ctx->d_counters); cudaFreeHost(ctx->h_counters); cudaFree(ctx->d_stats); cudaFree(ctx->d_ledger);
         cudaFree(ctx->d_edep); cudaFree(ctx->d_dose); cudaFree(ctx->d_sigma); cudaFree(ctx->d_beam);
@@ -630,13 +661,22 @@ mc_status mc_export_table(const mc_ctx* cctx, int32_t material, int32_t which, f
     if (!ctx->have_tables) return fail(ctx, MC_ERR_STATE, "mc_build_tables has not been called");
     const int N = ctx->tabs.N;
     if (which == 9) { std::copy(ctx->p_maj.begin(), ctx->p_maj.end(), out); return MC_OK; }
-    if (which < 0 || which > 8 || material < 0 || material >= ctx->tabs.n_mat) return fail(ctx, MC_ERR_INVALID_ARG, "table id / material");
+    if (which < 0 || which > 10 || material < 0 || material >= ctx->tabs.n_mat) return fail(ctx, MC_ERR_INVALID_ARG, "table id / material");
     const float* src;
     if (which == 0) src = ctx->p_tot.data() + (size_t)material * N;
     else if (which == 1) src = ctx->p_C.data() + (size_t)material * N;
     else if (which == 2) src = ctx->p_pp.data() + (size_t)material * N;
-    else src = ctx->tabs.t[which][material].data();  // TableId order matches mc.h for 3..8
+    else src = ctx->tabs.t[which == 10 ? (int)T_LNA : which][material].data();  // TableId order matches mc.h for 3..8
     std::copy(src, src + N, out);
+    return MC_OK;
+}
+
+mc_status mc_export_gs_table(int32_t dims[3], float* t_nodes, float* y) {
+    if (!dims) return MC_ERR_INVALID_ARG;
+    const GsTable& G = gs_table();
+    dims[0] = kGsNT; dims[1] = kGsNA; dims[2] = kGsNQ;
+    if (t_nodes) std::copy(G.t, G.t + kGsNT, t_nodes);
+    if (y) std::copy(G.y.begin(), G.y.end(), y);
     return MC_OK;
 }
 

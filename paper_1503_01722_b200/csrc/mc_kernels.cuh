@@ -8,6 +8,7 @@
 //   finalize_kernel : batch means and standard errors (R17, R18)
 #pragma once
 #include "mc_device.cuh"
+#include "mc_gs.h"
 
 namespace mcb {
 
@@ -135,6 +136,7 @@ __device__ __forceinline__ void emit(const RunParams& P, const Queue& q, Score& 
 constexpr int kSlots = 2;       // tracks per lane, parked in shared memory between the blocks that work on them
 enum LaneState { L_IDLE = 0, L_STEP = 1, L_HARD = 2, L_DONE = 3 };
 constexpr int kGroups = 5;      // 16-byte groups per track
+constexpr float kGsTMinF = (float)kGsTMin, kGsTMaxF = (float)kGsTMax;  // Goudsmit-Saunderson table range (mc_gs.h; R27)
 enum { SE_STEP = 0, SE_MOLLER, SE_BREMS, SE_SEC_E, SE_SEC_G, SE_HIST, SE_RED, SE_COUNT };
 
 // distances along (u,v,w) to the three faces of the voxel the direction points at; (x,y,z) = position relative to the
@@ -198,7 +200,10 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
     uint32_t* s_asg = s_st + kThreadsE;                                        // [kThreadsE]: per-warp assignment
     double* s_led = reinterpret_cast<double*>(s_asg + kThreadsE);              // [kWarps][2]: e_src, e_esc of the warp
     uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_led + 2 * kWarps);         // [kWarps][8]: event counters of the warp
+    float* s_gs = reinterpret_cast<float*>(s_cnt + 8 * kWarps);                // Goudsmit-Saunderson tables (flags & 8 only)
+    const bool gs_ms = P.flags & 8u;
     for (int i = threadIdx.x; i < ntab; i += kThreadsE) s_tab[i] = P.tabE[i];
+    if (gs_ms) for (int i = threadIdx.x; i < P.gs_words; i += kThreadsE) s_gs[i] = P.gs[i];
     const int tid = threadIdx.x;
     if (tid < 8 * kWarps) s_cnt[tid] = 0u;
     if (tid < 2 * kWarps) s_led[tid] = 0.0;
@@ -501,16 +506,52 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         float4 nd;
         float fm;
         if (!no_ms) {
-            inv_range_coord(tB, fmaf(-0.5f, rd, R0), fmaf(f_lg2(fmaf(-0.5f * d, xl, 1.0f)), P.ex_a, L.ex), k_cut, N, nd, fm);
+            const float em = inv_range_coord(tB, fmaf(-0.5f, rd, R0), fmaf(f_lg2(fmaf(-0.5f * d, xl, 1.0f)), P.ex_a, L.ex), k_cut, N, nd, fm);
             k1rho = fmaf(fm, nd.w, nd.z) * rho;  // K1 at the mid-step energy: its node is the one the search ended on
             // R8b: sample for the planned path plus the path travelled but not yet sampled for; never a negative path
             const float tq = fmaf(k1rho, d, P.ms_carry ? L.msc : 0.0f), t = fmaxf(tq, 0.0f);
             L.msc = tq - t;
-            float am = t < 1e-3f ? t * (1.0f - 0.5f * t) : 1.0f - f_exp(-t);
-            if (am > 0.0f) {
-                float omu = -am * kLn2F * f_lg2(1.0f - u01f(w4.z) * (1.0f - f_exp(-2.0f * f_rcp(am))));
-                float phi = kTwoPiF * u01f(w4.w);
-                rotate_fast(L.u, L.v, L.w, fminf(omu, 2.0f), f_sin(phi), f_cos(phi));
+            const float am = t < 1e-3f ? t * (1.0f - 0.5f * t) : 1.0f - f_exp(-t);
+            if (!gs_ms) {
+                if (am > 0.0f) {  // Gaussian on the sphere (R7)
+                    float omu = -am * kLn2F * f_lg2(1.0f - u01f(w4.z) * (1.0f - f_exp(-2.0f * f_rcp(am))));
+                    float phi = kTwoPiF * u01f(w4.w);
+                    rotate_fast(L.u, L.v, L.w, fminf(omu, 2.0f), f_sin(phi), f_cos(phi));
+                }
+            } else if (t < kGsTMinF) {
+                if (P.ms_carry) L.msc += t;  // below the table: not sampled now, carried (R27)
+            } else {
+                // Goudsmit-Saunderson angle (R27): row by stochastic interpolation (9 low bits of the two
+                // words), inverse CDF linear in log2 x inside a quantile interval
+                const float2* tl = reinterpret_cast<const float2*>(s_gs + kGsNT * kGsNA * kGsNQ) + mat_of() * P.gs_n8;
+                const float e8 = em * 0.125f;
+                const int i8 = (int)e8;
+                const float2 la = tl[i8];
+                const float lnA = fmaf(e8 - (float)i8, la.y, la.x);
+                const float tc = fminf(t, kGsTMaxF);
+                const float cc = fmaf(f_lg2(tc), kLn2F, 4.0f * f_sqrt(tc));
+                int ir = min(max((int)((cc - P.gs_c0) * P.gs_inv_dc), 0), kGsNT - 2);
+                const float a0n = P.gs_an[ir], a1n = P.gs_an[ir + 1];
+                const float ft = (fminf(am, P.gs_an[kGsNT - 1]) - a0n) * f_rcp(a1n - a0n);
+                ir += ((float)(w4.z & 511u) + 0.5f < ft * 512.0f) ? 1 : 0;
+                const float al = fminf(fmaxf((lnA - P.gs_lnA0) * P.gs_inv_dA, 0.0f), (float)(kGsNA - 1));
+                int jr = min((int)al, kGsNA - 2);
+                jr += ((float)(w4.w & 511u) + 0.5f < (al - (float)jr) * 512.0f) ? 1 : 0;
+                const float* row = s_gs + (ir * kGsNA + jr) * kGsNQ;
+                const float r = u01f(w4.z), s32 = (1.0f - r) * 32.0f;
+                int kq;
+                float fq;
+                if (s32 > 1.0f) { const float r32 = 32.0f * r; kq = (int)r32; fq = r32 - (float)kq; }
+                else {
+                    const int jj = min(126 - (int)(__float_as_uint(s32) >> 23), kGsNQ - 33);
+                    const float sj = s32 * __uint_as_float((uint32_t)(127 + jj) << 23);  // s 2^jj in (1/2, 1]
+                    kq = 31 + jj;
+                    fq = jj < kGsNQ - 33 ? 2.0f - 2.0f * sj : 1.0f - sj;
+                }
+                const float y0 = row[kq], y1 = row[kq + 1];
+                const float xq = kq == 0 ? f_ex2(y1) * fq : f_ex2(fmaf(fq, y1 - y0, y0));
+                const float phi = kTwoPiF * u01f(w4.w);
+                rotate_fast(L.u, L.v, L.w, fminf(xq, 2.0f), f_sin(phi), f_cos(phi));
             }
         }
         float tx, ty, tz;

@@ -4,6 +4,7 @@
 // Bethe-Heitler-style bremsstrahlung, screened-Rutherford first transport cross section.
 // Quadratures are Gauss-Legendre panels split at the bremsstrahlung screening kink.
 #include "mc_tables.h"
+#include "mc_gs.h"
 
 #include <algorithm>
 #include <cmath>
@@ -163,6 +164,19 @@ double l_rad(const Mat& m, double T, double kc) {
     auto f = [&](double k) { return brems_k_dsdk(m, T, k); };
     return integrate(f, 0, ks, 2) + integrate(f, ks, top, 2);
 }
+// ln of the effective screening parameter A of the mixture (R27): G_1(A) = K1 / Sigma_el with both sums over the elements
+// of the same screened-Rutherford law (total cross section of an element ~ Z(Z+1) / (A_i (1 + A_i)))
+double ln_screening(const Mat& m, double T) {
+    double tau = T / kMe, gam = tau + 1, bg2 = tau * (tau + 2), beta2 = bg2 / (gam * gam), first = 0, total = 0;
+    for (const auto& e : m.el) {
+        double az = kAlpha * e.Z / std::sqrt(beta2);
+        double scr = kAlpha * kAlpha * std::cbrt((double)e.Z * e.Z) / (4 * 0.885 * 0.885 * bg2) * (1.13 + 3.76 * az * az);
+        double c = e.w / e.A * e.Z * (e.Z + 1.0);
+        first += 2 * c * (std::log1p(1 / scr) - 1 / (1 + scr));
+        total += c / (scr * (1 + scr));
+    }
+    return std::log(gs_screening_from_ratio(first / total));
+}
 double k1_transport(const Mat& m, double T) {
     double tau = T / kMe, gam = tau + 1, bg2 = tau * (tau + 2), beta2 = bg2 / (gam * gam), s = 0;
     for (const auto& e : m.el) {
@@ -235,6 +249,7 @@ std::string build_tables(const std::vector<MaterialSpec>& specs, const TablePara
             out.t[T_S_MOLLER][mi][j] = (float)sM;
             out.t[T_S_HARD][mi][j] = (float)s_hard[j];
             out.t[T_K1][mi][j] = (float)k1_transport(m, E[j]);
+            out.t[T_LNA][mi][j] = (float)ln_screening(m, E[j]);
             // range integral over the segment [node j, node j + 1]
             if (j + 1 < N) segv[j] = integrate([&](double lt) { double T = std::exp(lt); return T / L(T); }, std::log(E[j]), std::log(E[j + 1]), 1);
         });

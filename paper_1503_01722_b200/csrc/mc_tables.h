@@ -18,7 +18,9 @@ struct TableParams {
     int n_grid;
 };
 
-enum TableId { T_MU_TOT = 0, T_MU_C, T_MU_PP, T_RANGE, T_L, T_S_HARD, T_S_MOLLER, T_S_MAX, T_K1, T_COUNT };
+enum TableId { T_MU_TOT = 0, T_MU_C, T_MU_PP, T_RANGE, T_L, T_S_HARD, T_S_MOLLER, T_S_MAX, T_K1,
+               T_LNA,  // ln of the effective screening parameter of the Goudsmit-Saunderson model (R27)
+               T_COUNT };
 
 struct Tables {
     int N = 0, k_cut = 0, n_mat = 0;

@@ -216,3 +216,22 @@ def test_run_particles_argument_validation_before_any_device_work():
         mc.mc_run_particles(eng.ctx, p, 1, 1, d, s)
     assert e.value.status == mc.MC_ERR_INVALID_ARG
     eng.close()
+
+
+def test_engine_goudsmit_saunderson_tables_match_the_oracles():
+    """Two independent builders of the same definition (R27): the material-independent quantile table
+    (ln of the quantiles of 1 - cos theta over scattering power x screening parameter) and the per-material effective
+    screening parameter.  Host code only: no device needed."""
+    import oracle
+    t, y = mc.mc_export_gs_table()
+    To = oracle.gs_table()
+    tn, An, rn = oracle.gs_nodes()
+    assert y.shape == To.shape == oracle.gs_dims()
+    assert np.allclose(t, tn, rtol=1e-6)
+    assert np.max(np.abs(y - To)) < 3e-3 and np.mean(np.abs(y - To)) < 3e-4  # quantiles of x agree to 0.3 %
+    ph = W.homogeneous_phantom((2, 2, 2), 1.0)
+    eng = mc.Engine(ph, W.materials(3), W.params())
+    orc = oracle.Oracle(ph, W.materials(3), W.params())
+    for m in range(3):
+        assert np.allclose(mc.mc_export_table(eng.ctx, "lnA", m), orc.table("lnA", m), atol=5e-6)
+    eng.close()

@@ -183,6 +183,36 @@ def test_config5_halfslab_photons_full_size_engine_coarse_blocks():
     _check(_run_case(cfg, cfg["n_histories"], 4 * 10 ** 7, coarse=4))
 
 
+# ---- Goudsmit-Saunderson multiple-scattering angle (R27) -------------------
+@pytest.mark.parametrize("c,beam", [(1, None), (2, None), (4, "e")])
+def test_goudsmit_saunderson_angle_matches_the_oracle_with_the_same_model(c, beam):
+    cfg = W.config(c, beam) if beam else W.config(c)
+    cfg["params"] = dict(cfg["params"], flags=cfg["params"]["flags"] | W.FLAG_MS_GS)
+    out = _run_case(cfg, cfg["n_histories"], cfg["n_histories"])
+    print("GS", c, beam, out)
+    _check(out)
+
+
+def test_goudsmit_saunderson_angle_changes_the_dose_where_it_should():
+    """The model is not a no-op: against the Gaussian model the lateral spread of a 6 MeV pencil beam changes (single-
+    scattering tail), while the deposited energy and the energy ledger do not."""
+    cfg = W.config(1)
+    n, B = 400000, 10
+    res = []
+    for fl in (0, W.FLAG_MS_GS):
+        eng = mc.Engine(cfg["phantom"], cfg["materials"], dict(cfg["params"], flags=fl))
+        d, _ = eng.run(cfg["beam"], n, 3, B)
+        st = eng.stats()
+        assert _ledger(st) < 1e-4
+        res.append((d.reshape(20, 20, 20).astype(np.float64), st["e_deposited_MeV"] / st["e_source_MeV"]))
+        eng.close()
+    (dg, fg), (ds, fs) = res
+    assert fg == pytest.approx(fs, abs=5e-3)
+    x = (np.arange(20) - 9.5) * 0.5
+    r2 = lambda d: float((d.sum(axis=0) * (x[None, :] ** 2 + x[:, None] ** 2)).sum() / d.sum())
+    assert abs(r2(ds) / r2(dg) - 1.0) > 0.01, (r2(ds), r2(dg))
+
+
 # ---- physics switches, particle types, edge cases ---------------------------------------------------------
 def _small_case(flags=0, particle=W.ELECTRON, energy=6.0, n=200000, shape=W.PENCIL, phantom=None):
     ph = phantom or W.homogeneous_phantom((12, 12, 16), 0.5)
