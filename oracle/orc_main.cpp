@@ -53,7 +53,7 @@ struct Stream {
 
 // ------------------------------------------------------------------------------------------------
 struct Params { double e_cut, g_cut, e_max; int n_grid; double d_maxs, f_maxe; uint32_t flags; };
-enum { F_NO_HARD = 1, F_NO_MS = 2, F_LOCAL_SEC = 4, F_MS_GS = 8 };
+enum { F_NO_HARD = 1, F_NO_MS = 2, F_LOCAL_SEC = 4, F_MS_GS = 8, F_MULTI_VOXEL = 16 };
 static GsTable g_gs;  // the Goudsmit-Saunderson sampling table (material independent, orc_gs.h), built on first use
 
 struct MatTables {  // all per unit density (cm^2/g, MeV cm^2/g, g/cm^2), one value per grid node
@@ -408,7 +408,118 @@ struct Run {
     }
 
     // ---- electron / positron (R2, R5..R11) --------------------------------------
+    // ---- electron / positron, multi-voxel steps (gDPM "employed a fixed step algorithm, where an electron
+    // can cross multiple voxel boundaries before a hard event occurs"; reading R28) -------------------------
+    // The step length d = min[d_maxs, d_maxe, d_range, d_event] is planned from the voxel the step starts in and is NOT
+    // limited by the voxel.  The two legs of the random hinge are walked voxel by voxel; every segment loses energy
+    // through the range table of its own material (deposited in its own voxel), uses up the sampled number of mean free
+    // paths -ln u at rho_i Sigma_max,i(T_start) (Sigma_max is a running maximum, so the value at the step's start energy
+    // is a majorant for the whole step in every material: the thinning stays exact without gDPM's cross-section scaling)
+    // and adds K1_i(T_mid) rho_i l_i to the scattering power travelled (R8b carries the difference to what the hinge
+    // sampled for).  A segment ends the step early where the mean free paths run out (hard-event candidate) or the range
+    // does (end of track).
+    void electron_multi_voxel(Particle p) {
+        Stream s = stream(p);
+        const Params& P = c.p;
+        const bool primary = probe && p.trk_lo == 0 && p.trk_hi == 0;
+        double path = 0, nstep = 0, q_used = 0, q_act = 0, ms_carry = 0;
+        auto finish = [&](int reason) {
+            if (!primary) return;
+            for (int a = 0; a < 3; ++a) { probe[2 + a] = p.x[a]; probe[5 + a] = p.d[a]; }
+            probe[8] = path; probe[9] = nstep; probe[10] = p.E; probe[11] = reason; probe[14] = q_used; probe[15] = q_act;
+        };
+        for (;;) {
+            if (p.E <= P.e_cut) {
+                finish(0);
+                deposit(p.v, p.E, true);
+                if (p.q > 0) {  // annihilation at rest (R9)
+                    s.next();
+                    Particle g = p; g.q = 0; g.blk0 = 0; g.E = MEC2; g.trk_lo = s.w[0]; g.trk_hi = s.w[1];
+                    iso_direction(s.u(2), s.u(3), g.d);
+                    s.next();
+                    Particle g2 = g; g2.trk_lo = s.w[0]; g2.trk_hi = s.w[1];
+                    for (int a = 0; a < 3; ++a) g2.d[a] = -g.d[a];
+                    push(g); push(g2);
+                }
+                return;
+            }
+            const int v0 = vidx(p.v);
+            const MatTables& t0 = c.tab[c.mat[v0]];
+            const double rho0 = c.rho[v0], T0 = p.E;
+            const double R0 = lerp_tab(c, t0.R, T0), L0 = lerp_tab(c, t0.L, T0), Smax0 = lerp_tab(c, t0.S_max, T0);
+            s.next();
+            double tau = (P.flags & F_NO_HARD) ? 1e300 : -std::log(s.u(0));  // mean free paths to the next hard-event candidate
+            double d = std::min(std::min(P.d_maxs, P.f_maxe * T0 / (rho0 * L0)), std::min(std::max(R0, 0.0) / rho0, tau / (rho0 * Smax0)));
+            if (!(d > 0.0)) {  // no residual range left above the cut-off (rounding): the track ends here
+                deposit(p.v, p.E - P.e_cut, false);
+                p.E = P.e_cut;
+                continue;
+            }
+            st.n_estep += 1; nstep += 1;
+            const double Tmid = inv_range(c, t0.R, R0 - 0.5 * rho0 * d);
+            const double k1rho0 = (P.flags & F_NO_MS) ? 0.0 : lerp_tab(c, t0.K1, Tmid) * rho0;
+            double q_step = 0;  // scattering power travelled in this step
+            enum { NONE = 0, HARD = 1, STOP = 2, OUT = 3 };
+            double Smax_ev = Smax0;
+            // walk `len` cm along the direction, voxel by voxel
+            auto walk = [&](double len) -> int {
+                while (len > 0.0) {
+                    const int vi = vidx(p.v);
+                    const MatTables& ti = c.tab[c.mat[vi]];
+                    const double rho = c.rho[vi];
+                    int ax;
+                    const double tf = face_dist(p.x, p.d, p.v, ax);
+                    const double Smax_i = lerp_tab(c, ti.S_max, T0), Ri = lerp_tab(c, ti.R, p.E);
+                    double seg = std::min(len, tf);
+                    int ev = NONE;
+                    const double l_tau = tau / (rho * Smax_i), l_range = std::max(Ri, 0.0) / rho;
+                    // "<=" to rounding: a step planned up to the event (or the end of the range) ends exactly there
+                    if (l_tau <= seg * (1.0 + 1e-9)) { seg = std::min(seg, l_tau); ev = HARD; Smax_ev = Smax_i; }
+                    if (l_range <= seg * (1.0 + 1e-9)) { seg = std::min(seg, l_range); ev = STOP; }
+                    for (int a = 0; a < 3; ++a) p.x[a] += seg * p.d[a];
+                    const double T1 = ev == STOP ? P.e_cut : inv_range(c, ti.R, Ri - rho * seg);
+                    deposit(p.v, p.E - T1, false);
+                    p.E = T1;
+                    tau -= rho * Smax_i * seg;
+                    if (!(P.flags & F_NO_MS)) q_step += lerp_tab(c, ti.K1, Tmid) * rho * seg;
+                    st.path_e += seg; path += seg;
+                    len -= seg;
+                    if (ev != NONE) return ev;
+                    if (seg >= tf) {  // on the face: enter the neighbour
+                        const int dir = p.d[ax] > 0 ? 1 : -1;
+                        p.v[ax] += dir;
+                        p.x[ax] = c.org[ax] + (p.v[ax] + (dir > 0 ? 0 : 1)) * c.h[ax];
+                        if (!inside(p.v)) return OUT;
+                    }
+                }
+                return NONE;
+            };
+            const double xi = s.u(1);
+            int ev = walk(xi * d);
+            if (ev == NONE && (P.flags & F_NO_MS)) ev = walk((1.0 - xi) * d);
+            else if (ev == NONE) {
+                // the hinge (R7 / R27) with the bookkeeping of R8b
+                double tq = k1rho0 * d + (c.ms_carry ? ms_carry : 0.0), tu = std::max(tq, 0.0);
+                ms_carry = tq - tu;
+                q_used += tu;
+                if (P.flags & F_MS_GS) {
+                    if (tu < GS_T_MIN) { if (c.ms_carry) ms_carry += tu; q_used -= tu; }
+                    else rotate_dir(p.d, 1.0 - gs_sample_omu(g_gs, tu, std::exp(lerp_tab(c, t0.lnA, Tmid)), s.w[2], s.w[3]), 2.0 * PI * s.u(3));
+                } else {
+                    double am = 1.0 - std::exp(-tu);
+                    if (am > 0.0) rotate_dir(p.d, 1.0 - sample_ms_omu(am, s.u(2)), 2.0 * PI * s.u(3));
+                }
+                ms_carry -= k1rho0 * d;  // what was sampled for beyond the carry; the path travelled is added below
+                ev = walk((1.0 - xi) * d);
+            }
+            ms_carry += q_step; q_act += q_step;
+            if (ev == OUT) { finish(1); escape(p.E + (p.q > 0 ? 2.0 * MEC2 : 0.0)); return; }
+            if (ev == HARD && p.E > P.e_cut) hard_candidate(p, s, Smax_ev, primary, path);
+        }
+    }
+
     void electron(Particle p) {
+        if (c.p.flags & F_MULTI_VOXEL) { electron_multi_voxel(p); return; }
         Stream s = stream(p);
         const Params& P = c.p;
         const bool primary = probe && p.trk_lo == 0 && p.trk_hi == 0;  // per-history probe of the primary track (pins)
@@ -506,32 +617,40 @@ struct Run {
                 continue;
             }
             if (lim != 4 || p.E <= P.e_cut) continue;
-            // hard event candidate: thinning against the running-max majorant (R6)
-            s.next();
-            double r = s.u(0) * Smax;
-            double SM = lerp_tab(c, t.S_M, p.E), SH = lerp_tab(c, t.S_hard, p.E);
-            if (r >= SH) { if (primary && probe[0] == 0) probe[13] += 1; continue; }  // fictitious
-            uint32_t id_lo = s.w[1], id_hi = s.w[2];
-            double phi = 2.0 * PI * s.u(3);
-            double T0 = p.E;
-            if (primary && probe[0] == 0) { probe[0] = r < SM ? 1 : 2; probe[1] = T0; probe[12] = path; }
-            if (r < SM) {  // Moller (R10)
-                st.n_moller += 1;
-                double W = sample_moller(s, T0, P.e_cut) * T0, c1, c2;
-                moller_angles(T0, W, c1, c2);
-                Particle e = p; e.q = -1; e.blk0 = 0; e.E = W; e.trk_lo = id_lo; e.trk_hi = id_hi;
-                rotate_dir(e.d, c2, phi + PI);
-                rotate_dir(p.d, c1, phi);
-                p.E = T0 - W;
-                push(e);
-            } else {  // bremsstrahlung (R11)
-                st.n_brems += 1;
-                double kk = sample_brems(s, c.mats[c.mat[vi]], T0, P.g_cut);
-                Particle g = p; g.q = 0; g.blk0 = 0; g.E = kk; g.trk_lo = id_lo; g.trk_hi = id_hi;
-                rotate_dir(g.d, std::cos(MEC2 / (T0 + MEC2)), phi);
-                p.E = T0 - kk;
-                push(g);
-            }
+            hard_candidate(p, s, Smax, primary, path);
+        }
+    }
+
+    // Hard event candidate at the end of a step ("Woodcock again"; R6): thinning against the majorant the
+    // distance was sampled with, then Moller (R10) or bremsstrahlung (R11) in the material where the particle stands.
+    void hard_candidate(Particle& p, Stream& s, double Smax, bool primary, double path) {
+        const Params& P = c.p;
+        int vi = vidx(p.v);
+        const MatTables& t = c.tab[c.mat[vi]];
+        s.next();
+        double r = s.u(0) * Smax;
+        double SM = lerp_tab(c, t.S_M, p.E), SH = lerp_tab(c, t.S_hard, p.E);
+        if (r >= SH) { if (primary && probe[0] == 0) probe[13] += 1; return; }  // fictitious
+        uint32_t id_lo = s.w[1], id_hi = s.w[2];
+        double phi = 2.0 * PI * s.u(3);
+        double T0 = p.E;
+        if (primary && probe[0] == 0) { probe[0] = r < SM ? 1 : 2; probe[1] = T0; probe[12] = path; }
+        if (r < SM) {  // Moller (R10)
+            st.n_moller += 1;
+            double W = sample_moller(s, T0, P.e_cut) * T0, c1, c2;
+            moller_angles(T0, W, c1, c2);
+            Particle e = p; e.q = -1; e.blk0 = 0; e.E = W; e.trk_lo = id_lo; e.trk_hi = id_hi;
+            rotate_dir(e.d, c2, phi + PI);
+            rotate_dir(p.d, c1, phi);
+            p.E = T0 - W;
+            push(e);
+        } else {  // bremsstrahlung (R11)
+            st.n_brems += 1;
+            double kk = sample_brems(s, c.mats[c.mat[vi]], T0, P.g_cut);
+            Particle g = p; g.q = 0; g.blk0 = 0; g.E = kk; g.trk_lo = id_lo; g.trk_hi = id_hi;
+            rotate_dir(g.d, std::cos(MEC2 / (T0 + MEC2)), phi);
+            p.E = T0 - kk;
+            push(g);
         }
     }
 

@@ -62,6 +62,7 @@ FLAG_NO_HARD = 1        # no Moller / bremsstrahlung events
 FLAG_NO_MS = 2          # no multiple-scattering deflection
 FLAG_LOCAL_SECONDARIES = 4  # secondaries are deposited where they are born
 FLAG_MS_GS = 8          # Goudsmit-Saunderson multiple-scattering angle instead of the Gaussian model (R27)
+FLAG_MULTI_VOXEL = 16   # electron steps are not limited by the voxel: they cross faces (gDPM-style stepping; R28)
 
 
 # --- phantoms ------------------------------------------------------------------------------------
