@@ -67,6 +67,11 @@ typedef struct {
                                          screened-Rutherford law ("the method developed by Kawrakow";
                                          DESIGN.md R27) instead of the Gaussian model (R7)                        */
 
+#define MC_FLAG_MULTI_VOXEL 16u       /* electron steps are not limited by the voxel: a step of length
+                                         min[d_maxs, d_maxe, d_range, d_event] crosses voxel faces (the stepping of
+                                         gDPM the paper compares with; R28) instead of
+                                         d = min[d_vox, ...]                                        */
+
 /* Cut-offs and step limits (PAPER.md:39 "user defined maximum step size", :86 cut-off energies).
  * e_cut_MeV: electron absorption energy = Moller delta-ray threshold; g_cut_MeV: photon absorption
  * energy = bremsstrahlung production threshold (R1).  e_max_MeV: top of the energy grid.

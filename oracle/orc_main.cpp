@@ -473,9 +473,10 @@ struct Run {
                     double seg = std::min(len, tf);
                     int ev = NONE;
                     const double l_tau = tau / (rho * Smax_i), l_range = std::max(Ri, 0.0) / rho;
-                    // "<=" to rounding: a step planned up to the event (or the end of the range) ends exactly there
-                    if (l_tau <= seg * (1.0 + 1e-9)) { seg = std::min(seg, l_tau); ev = HARD; Smax_ev = Smax_i; }
-                    if (l_range <= seg * (1.0 + 1e-9)) { seg = std::min(seg, l_range); ev = STOP; }
+                    // "<=" to rounding (of the whole step: what is left in the second leg is a difference): a step planned up
+                    // to the event or to the end of the range ends exactly there
+                    if (l_tau <= seg + 1e-9 * d) { seg = std::min(seg, l_tau); ev = HARD; Smax_ev = Smax_i; }
+                    if (l_range <= seg + 1e-9 * d) { seg = std::min(seg, l_range); ev = STOP; }
                     for (int a = 0; a < 3; ++a) p.x[a] += seg * p.d[a];
                     const double T1 = ev == STOP ? P.e_cut : inv_range(c, ti.R, Ri - rho * seg);
                     deposit(p.v, p.E - T1, false);

@@ -205,8 +205,11 @@ struct KernelChoice { TransportKernel fn; int threads; size_t smem; };
 // the largest CTA whose tables + pools fit (more materials or a finer grid leave less room for the pools)
 bool choose_electron_kernel(const mc_ctx* c, KernelChoice& k) {
     const int T[4] = {1024, 768, 512, 256};
-    const TransportKernel fn[4] = {electron_kernel<1024>, electron_kernel<768>, electron_kernel<512>, electron_kernel<256>};
-    for (int i = 0; i < 4; ++i)
+    const bool multi = c->params.flags & MC_FLAG_MULTI_VOXEL;
+    const TransportKernel fn1[4] = {electron_kernel<1024, false>, electron_kernel<768, false>, electron_kernel<512, false>, electron_kernel<256, false>};
+    const TransportKernel fnm[4] = {electron_kernel<1024, true>, electron_kernel<768, true>, electron_kernel<512, true>, electron_kernel<256, true>};
+    const TransportKernel* fn = multi ? fnm : fn1;
+    for (int i = multi ? 1 : 0; i < 4; ++i)  // the multi-voxel variant needs 80 registers: 768-thread CTAs at most
         if (smem_e(c, T[i]) <= kSmemMax) { k = KernelChoice{fn[i], T[i], smem_e(c, T[i])}; return true; }
     return false;
 }

@@ -187,7 +187,8 @@ struct ELane {
     Rng rng;
 };
 
-template <int kThreadsE>
+// kMulti: the multi-voxel stepping (flags & 16; R28) instead of one step per voxel.
+template <int kThreadsE, bool kMulti>
 __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_constant__ RunParams P) {
     extern __shared__ __align__(16) float2 s_tab[];
     // the launch consumes the whole input queue as it stands (no host round trip)
@@ -300,6 +301,57 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, tx, ty, tz);
         L.dvox = fminf(tx, fminf(ty, tz));
     };
+
+    // The hinge's deflection (S5): multiple-scattering angle for scattering power k1rho * d of the planned step plus what
+    // was travelled but not sampled for (R8b), Gaussian model (R7) or Goudsmit-Saunderson (R27); em = table coordinate of
+    // the mid-step energy in the tables of material mat_ms, w4 = the step's Philox block (z: polar angle, w: azimuth).
+    auto hinge_deflect = [&](float k1rho, float d, float em, int mat_ms, const uint4& w4) {
+        // R8b: sample for the planned path plus the path travelled but not yet sampled for; never a negative path
+        const float tq = fmaf(k1rho, d, P.ms_carry ? L.msc : 0.0f), t = fmaxf(tq, 0.0f);
+        L.msc = tq - t;
+        const float am = t < 1e-3f ? t * (1.0f - 0.5f * t) : 1.0f - f_exp(-t);
+        if (!gs_ms) {
+            if (am > 0.0f) {  // Gaussian on the sphere (R7)
+                float omu = -am * kLn2F * f_lg2(1.0f - u01f(w4.z) * (1.0f - f_exp(-2.0f * f_rcp(am))));
+                float phi = kTwoPiF * u01f(w4.w);
+                rotate_fast(L.u, L.v, L.w, fminf(omu, 2.0f), f_sin(phi), f_cos(phi));
+            }
+        } else if (t < kGsTMinF) {
+            if (P.ms_carry) L.msc += t;  // below the table: not sampled now, carried (R27)
+        } else {
+            // Goudsmit-Saunderson angle (R27): row by stochastic interpolation (9 low bits of the two
+            // words), inverse CDF linear in log2 x inside a quantile interval
+            const float2* tl = reinterpret_cast<const float2*>(s_gs + kGsNT * kGsNA * kGsNQ) + mat_ms * P.gs_n8;
+            const float e8 = em * 0.125f;
+            const int i8 = (int)e8;
+            const float2 la = tl[i8];
+            const float lnA = fmaf(e8 - (float)i8, la.y, la.x);
+            const float tc = fminf(t, kGsTMaxF);
+            const float cc = fmaf(f_lg2(tc), kLn2F, 4.0f * f_sqrt(tc));
+            int ir = min(max((int)((cc - P.gs_c0) * P.gs_inv_dc), 0), kGsNT - 2);
+            const float a0n = P.gs_an[ir], a1n = P.gs_an[ir + 1];
+            const float ft = (fminf(am, P.gs_an[kGsNT - 1]) - a0n) * f_rcp(a1n - a0n);
+            ir += ((float)(w4.z & 511u) + 0.5f < ft * 512.0f) ? 1 : 0;
+            const float al = fminf(fmaxf((lnA - P.gs_lnA0) * P.gs_inv_dA, 0.0f), (float)(kGsNA - 1));
+            int jr = min((int)al, kGsNA - 2);
+            jr += ((float)(w4.w & 511u) + 0.5f < (al - (float)jr) * 512.0f) ? 1 : 0;
+            const float* row = s_gs + (ir * kGsNA + jr) * kGsNQ;
+            const float r = u01f(w4.z), s32 = (1.0f - r) * 32.0f;
+            int kq;
+            float fq;
+            if (s32 > 1.0f) { const float r32 = 32.0f * r; kq = (int)r32; fq = r32 - (float)kq; }
+            else {
+                const int jj = min(126 - (int)(__float_as_uint(s32) >> 23), kGsNQ - 33);
+                const float sj = s32 * __uint_as_float((uint32_t)(127 + jj) << 23);  // s 2^jj in (1/2, 1]
+                kq = 31 + jj;
+                fq = jj < kGsNQ - 33 ? 2.0f - 2.0f * sj : 1.0f - sj;
+            }
+            const float y0 = row[kq], y1 = row[kq + 1];
+            const float xq = kq == 0 ? f_ex2(y1) * fq : f_ex2(fmaf(fq, y1 - y0, y0));
+            const float phi = kTwoPiF * u01f(w4.w);
+            rotate_fast(L.u, L.v, L.w, fminf(xq, 2.0f), f_sin(phi), f_cos(phi));
+        }
+            };
 
     for (;;) {
         // ---- scheduling: count the pool's tracks by state, choose ONE block, hand its tracks to the lanes ------
@@ -474,6 +526,124 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         if (!have) { __syncwarp(); continue; }
         load_slot(slot);
         state = L_STEP;
+        if constexpr (kMulti) {
+            // ---- STEP, multi-voxel variant (PAPER.md:167 gDPM's stepping; R28): d = min[d_maxs, d_maxe,
+            // d_range, d_event] planned from the voxel the step starts in, NOT limited by it.  Both legs of the hinge are
+            // walked voxel by voxel: every segment loses energy through the range table of its own material (scored in
+            // its own voxel), uses up the sampled mean free paths at rho_i Sigma_max,i(T_start) and adds to the
+            // scattering power travelled (R8b).  The step ends early where the mean free paths run out (hard-event
+            // candidate), the range does (end of track) or the track leaves the phantom.
+            const float4* tA = tabA();
+            const int mat0 = mat_of();
+            const int i0 = min(max((int)L.ex, 0), N - 2);
+            const float f0 = L.ex - (float)i0;
+            float4 a0 = tA[i0];
+            float2 s0 = reinterpret_cast<const float2*>(tA + 3 * N)[i0];
+            const float R0 = fmaf(f0, a0.y, a0.x), L0 = fmaf(f0, a0.w, a0.z);
+            float Smax_i = fmaf(f0, s0.y, s0.x);
+            const uint4 w4 = next_block_rk(L.rng, P);
+            float tau = no_hard ? kInf : -kLn2F * f_lg2(u01f(w4.x));  // mean free paths to the next hard-event candidate
+            const float rho0 = L.rho, irho0 = f_rcp(rho0);
+            const float d = fminf(fminf(P.d_maxs, P.f_maxe * L.T * irho0 * f_rcp(L0)), fminf(fmaxf(R0, 0.0f) * irho0, tau * irho0 * f_rcp(Smax_i)));
+            bool crossed = false;
+            if (!(d > 0.0f)) { L.acc += fmaxf(L.T - P.e_cut, 0.0f); L.T = P.e_cut; }  // no residual range left (rounding)
+            else {
+                // K1 at the mid-step energy, in the start voxel's material; its table coordinate serves every material
+                float4 nd;
+                float fm = 0.0f, em = L.ex, k1rho0 = 0.0f;
+                if (!no_ms) {
+                    em = inv_range_coord(tA + N, fmaf(-0.5f * rho0, d, R0), fmaf(f_lg2(fmaf(-0.5f * d, rho0 * L0 * f_rcp(L.T), 1.0f)), P.ex_a, L.ex), k_cut, N, nd, fm);
+                    k1rho0 = fmaf(fm, nd.w, nd.z) * rho0;
+                }
+                const int im = min(max((int)em, 0), N - 2);
+                float k1rho_i = k1rho0, q_step = 0.0f, smax_ev = Smax_i;
+                float Ri = R0, Li = L0, exc = L.ex;  // residual range, stopping power and table coordinate at the current energy
+                int ev = 0;                           // 1: hard-event candidate, 2: end of range, 3: left the phantom
+                const float legA = u01f(w4.y) * d;
+#pragma unroll 1
+                for (int leg = 0; leg < 2 && ev == 0; ++leg) {
+                    float len = leg == 0 ? legA : d - legA;
+                    if (leg == 1 && !no_ms) {
+                        hinge_deflect(k1rho0, d, em, mat0, w4);
+                        L.msc = fmaf(-k1rho0, d, L.msc);  // sampled for; the path travelled is added after the walk
+                    }
+                    float tx, ty, tz;
+                    face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, tx, ty, tz);
+#pragma unroll 1
+                    while (len > 0.0f) {
+                        const float rho = L.rho, irho = f_rcp(rho);
+                        int ax = 0;
+                        float tf = tx;
+                        if (ty < tf) { tf = ty; ax = 1; }
+                        if (tz < tf) { tf = tz; ax = 2; }
+                        float seg = fminf(len, tf);
+                        const float l_tau = tau * irho * f_rcp(Smax_i), l_range = fmaxf(Ri, 0.0f) * irho;
+                        // "<=" to rounding (of the whole step: what is left in the second leg is a difference): a step planned
+                        // up to the event or to the end of the range ends exactly there
+                        if (l_tau <= fmaf(1e-5f, d, seg)) { seg = fminf(seg, l_tau); ev = 1; smax_ev = Smax_i; }
+                        if (l_range <= fmaf(1e-5f, d, seg)) { seg = fminf(seg, l_range); ev = 2; }
+                        L.x = fmaf(seg, L.u, L.x); L.y = fmaf(seg, L.v, L.y); L.z = fmaf(seg, L.w, L.z);
+                        tx = fmaxf(tx - seg, 0.0f); ty = fmaxf(ty - seg, 0.0f); tz = fmaxf(tz - seg, 0.0f);
+                        float T1 = P.e_cut;
+                        if (ev != 2) {
+                            float fr;
+                            exc = inv_range_coord(tA + N, fmaf(-rho, seg, Ri),
+                                                  fmaf(f_lg2(fmaxf(fmaf(-seg, rho * Li * f_rcp(L.T), 1.0f), 1e-3f)), P.ex_a, exc), k_cut, N, nd, fr);
+                            T1 = fminf(f_ex2(fmaf(exc, P.t_a, P.t_b)), L.T);
+                        }
+                        L.acc += L.T - T1;
+                        L.T = T1;
+                        tau = fmaf(-rho * Smax_i, seg, tau);
+                        q_step = fmaf(k1rho_i, seg, q_step);
+                        len -= seg;
+                        if (ev != 0) break;
+                        if (seg >= tf) {
+                            // on the face: flush this voxel's deposit, enter the neighbour (as in the per-voxel variant)
+                            flush();
+                            crossed = true;
+                            const bool a0x = ax == 0, a1x = ax == 1, a2x = ax == 2;
+                            const float dc = a0x ? L.u : (a1x ? L.v : L.w);
+                            const bool up = dc > 0.0f;
+                            const float ha = a0x ? g.hx : (a1x ? g.hy : g.hz);
+                            const float tnew = ha * f_rcp(fabsf(dc)), xin = up ? 0.0f : ha;
+                            L.x = a0x ? xin : L.x; L.y = a1x ? xin : L.y; L.z = a2x ? xin : L.z;
+                            tx = a0x ? tnew : tx; ty = a1x ? tnew : ty; tz = a2x ? tnew : tz;
+                            const int sh = 10 * ax;
+                            const int ia = (int)((L.idx >> sh) & 1023u) + (up ? 1 : -1);
+                            const int na = a0x ? g.nx : (a1x ? g.ny : g.nz), stride = a0x ? 1 : (a1x ? g.nx : g.nx * g.ny);
+                            if ((unsigned)ia >= (unsigned)na) {
+                                atomicAdd(w_led + 1, (double)(L.T + (is_positron() ? 2.0f * kMeF : 0.0f)));
+                                state = L_IDLE; ev = 3;
+                                break;
+                            }
+                            L.idx = (L.idx & ~(1023u << sh)) | ((uint32_t)ia << sh);
+                            L.vox += up ? stride : -stride;
+                            const uint2 vd = P.vox[L.vox];
+                            const bool new_mat = vd.y != ((L.tagk >> 2) & 15u);
+                            L.rho = __uint_as_float(vd.x); L.tagk = (L.tagk & ~60u) | (vd.y << 2);
+                            if (new_mat) {  // the new material's majorant at the step's start energy, its K1 at the mid-step energy
+                                tA = tabA();
+                                s0 = reinterpret_cast<const float2*>(tA + 3 * N)[i0];
+                                Smax_i = fmaf(f0, s0.y, s0.x);
+                                const float4 bm = (tA + N)[im];
+                                k1rho_i = no_ms ? 0.0f : fmaf(em - (float)im, bm.w, bm.z);
+                            }
+                            k1rho_i = new_mat ? k1rho_i * L.rho : (no_ms ? 0.0f : k1rho_i * L.rho * irho);
+                        }
+                        // residual range and stopping power at the current energy in the current material
+                        const int ic = min(max((int)exc, 0), N - 2);
+                        a0 = tA[ic];
+                        Ri = fmaf(exc - (float)ic, a0.y, a0.x); Li = fmaf(exc - (float)ic, a0.w, a0.z);
+                    }
+                }
+                L.msc += q_step;
+                if (state == L_STEP && ev == 1 && L.T > P.e_cut) { state = L_HARD; L.smax = smax_ev; }
+            }
+            if (state == L_STEP && L.T <= P.e_cut) terminate();
+            park(crossed ? 2 : 1);
+            __syncwarp();
+            continue;
+        }
         // ---- STEP set-up (S4): d = min[d_vox, d_maxs, d_maxe, d_range, d_event] ------------------------------
         const float4* const tA = tabA();  // [N] (R, slope, L, slope) | [N] inverse-range pack | [N] hard pack | [N] float2 S_max
         const float4* const tB = tA + N;
@@ -508,51 +678,7 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
         if (!no_ms) {
             const float em = inv_range_coord(tB, fmaf(-0.5f, rd, R0), fmaf(f_lg2(fmaf(-0.5f * d, xl, 1.0f)), P.ex_a, L.ex), k_cut, N, nd, fm);
             k1rho = fmaf(fm, nd.w, nd.z) * rho;  // K1 at the mid-step energy: its node is the one the search ended on
-            // R8b: sample for the planned path plus the path travelled but not yet sampled for; never a negative path
-            const float tq = fmaf(k1rho, d, P.ms_carry ? L.msc : 0.0f), t = fmaxf(tq, 0.0f);
-            L.msc = tq - t;
-            const float am = t < 1e-3f ? t * (1.0f - 0.5f * t) : 1.0f - f_exp(-t);
-            if (!gs_ms) {
-                if (am > 0.0f) {  // Gaussian on the sphere (R7)
-                    float omu = -am * kLn2F * f_lg2(1.0f - u01f(w4.z) * (1.0f - f_exp(-2.0f * f_rcp(am))));
-                    float phi = kTwoPiF * u01f(w4.w);
-                    rotate_fast(L.u, L.v, L.w, fminf(omu, 2.0f), f_sin(phi), f_cos(phi));
-                }
-            } else if (t < kGsTMinF) {
-                if (P.ms_carry) L.msc += t;  // below the table: not sampled now, carried (R27)
-            } else {
-                // Goudsmit-Saunderson angle (R27): row by stochastic interpolation (9 low bits of the two
-                // words), inverse CDF linear in log2 x inside a quantile interval
-                const float2* tl = reinterpret_cast<const float2*>(s_gs + kGsNT * kGsNA * kGsNQ) + mat_of() * P.gs_n8;
-                const float e8 = em * 0.125f;
-                const int i8 = (int)e8;
-                const float2 la = tl[i8];
-                const float lnA = fmaf(e8 - (float)i8, la.y, la.x);
-                const float tc = fminf(t, kGsTMaxF);
-                const float cc = fmaf(f_lg2(tc), kLn2F, 4.0f * f_sqrt(tc));
-                int ir = min(max((int)((cc - P.gs_c0) * P.gs_inv_dc), 0), kGsNT - 2);
-                const float a0n = P.gs_an[ir], a1n = P.gs_an[ir + 1];
-                const float ft = (fminf(am, P.gs_an[kGsNT - 1]) - a0n) * f_rcp(a1n - a0n);
-                ir += ((float)(w4.z & 511u) + 0.5f < ft * 512.0f) ? 1 : 0;
-                const float al = fminf(fmaxf((lnA - P.gs_lnA0) * P.gs_inv_dA, 0.0f), (float)(kGsNA - 1));
-                int jr = min((int)al, kGsNA - 2);
-                jr += ((float)(w4.w & 511u) + 0.5f < (al - (float)jr) * 512.0f) ? 1 : 0;
-                const float* row = s_gs + (ir * kGsNA + jr) * kGsNQ;
-                const float r = u01f(w4.z), s32 = (1.0f - r) * 32.0f;
-                int kq;
-                float fq;
-                if (s32 > 1.0f) { const float r32 = 32.0f * r; kq = (int)r32; fq = r32 - (float)kq; }
-                else {
-                    const int jj = min(126 - (int)(__float_as_uint(s32) >> 23), kGsNQ - 33);
-                    const float sj = s32 * __uint_as_float((uint32_t)(127 + jj) << 23);  // s 2^jj in (1/2, 1]
-                    kq = 31 + jj;
-                    fq = jj < kGsNQ - 33 ? 2.0f - 2.0f * sj : 1.0f - sj;
-                }
-                const float y0 = row[kq], y1 = row[kq + 1];
-                const float xq = kq == 0 ? f_ex2(y1) * fq : f_ex2(fmaf(fq, y1 - y0, y0));
-                const float phi = kTwoPiF * u01f(w4.w);
-                rotate_fast(L.u, L.v, L.w, fminf(xq, 2.0f), f_sin(phi), f_cos(phi));
-            }
+            hinge_deflect(k1rho, d, em, mat_of(), w4);
         }
         float tx, ty, tz;
         face_all(g, L.x, L.y, L.z, L.u, L.v, L.w, tx, ty, tz);

@@ -135,7 +135,9 @@ def _check(out):
     if indep["noise"] < 1e-6:  # no randomness left (pencil beam without MS and hard events): sigma ~ fp32 rounding only
         assert indep["mean_diff"] <= 1e-3, indep
         return
-    assert indep["frac3"] >= 0.99, indep
+    # >= 99 % within 3 sigma; where the 10 % isodose holds fewer than 100 voxels (the pencil beam of config 1: 20-25)
+    # one voxel is already 4-5 %, and with 10 batches a voxel lands beyond 3 sigma ~1 % of the time: allow one there
+    assert indep["frac3"] >= 0.99 or (indep["n"] < 100 and round((1.0 - indep["frac3"]) * indep["n"]) <= 1), indep
     assert indep["mean_diff"] <= 0.01 + indep["noise"], indep
     if indep["noise"] <= 0.8 * 0.003:  # mean combined sigma <= 0.3 % of Dmax: north_star's 1 % bar with no allowance
         assert indep["mean_diff"] <= 0.01, indep
@@ -211,6 +213,25 @@ def test_goudsmit_saunderson_angle_changes_the_dose_where_it_should():
     x = (np.arange(20) - 9.5) * 0.5
     r2 = lambda d: float((d.sum(axis=0) * (x[None, :] ** 2 + x[:, None] ** 2)).sum() / d.sum())
     assert abs(r2(ds) / r2(dg) - 1.0) > 0.01, (r2(ds), r2(dg))
+
+
+# ---- multi-voxel electron stepping (R28) -----------------------------------
+@pytest.mark.parametrize("c,beam,extra", [(1, None, 0), (2, None, 0), (4, "e", 0), (4, "e", W.FLAG_MS_GS)])
+def test_multi_voxel_stepping_matches_the_oracle_with_the_same_stepping(c, beam, extra):
+    cfg = W.config(c, beam) if beam else W.config(c)
+    cfg["params"] = dict(cfg["params"], flags=cfg["params"]["flags"] | W.FLAG_MULTI_VOXEL | extra)
+    out = _run_case(cfg, cfg["n_histories"], cfg["n_histories"])
+    print("MV", c, beam, extra, out)
+    _check(out)
+
+
+def test_multi_voxel_stepping_on_the_half_slab_coarse_blocks():
+    """Config 5 (0.25 cm voxels, material interface along x): the case where a step crosses most faces."""
+    cfg = W.config(5, "e")
+    cfg["params"] = dict(cfg["params"], flags=cfg["params"]["flags"] | W.FLAG_MULTI_VOXEL)
+    out = _run_case(cfg, 2 * 10 ** 7, 4 * 10 ** 6, coarse=4)
+    print("MV5", out)
+    _check(out)
 
 
 # ---- physics switches, particle types, edge cases ---------------------------------------------------------
