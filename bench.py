@@ -51,6 +51,7 @@ def parse():
     ap.add_argument("--beam", default=None, choices=[None, "e", "g"], help="configs 4, 5: electron or photon beam")
     ap.add_argument("--histories", type=int, default=0, help="override n_histories (the line then says so)")
     ap.add_argument("--ms-model", default="gaussian", choices=["gaussian", "gs"], help="multiple-scattering angle model (north_star: Gaussian or Goudsmit-Saunderson)")
+    ap.add_argument("--stepping", default="voxel", choices=["voxel", "multi"], help="electron stepping: one step per voxel (PAPER.md:39) or multi-voxel steps (PAPER.md:167)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--option", action="append", default=[], help="engine option name=value (mc_set_option)")
@@ -117,6 +118,8 @@ def workload(args):
     cfg = W.config(args.config, args.beam)
     if args.histories:
         cfg["n_histories"] = args.histories
+    if args.stepping == "multi":  # steps cross voxel faces (gDPM's scheme; R28); the line says so
+        cfg["params"] = dict(cfg["params"], flags=cfg["params"]["flags"] | W.FLAG_MULTI_VOXEL)
     if args.ms_model == "gs":  # Goudsmit-Saunderson angle instead of the Gaussian model (R27); the line says so
         cfg["params"] = dict(cfg["params"], flags=cfg["params"]["flags"] | W.FLAG_MS_GS)
     return cfg
@@ -127,7 +130,7 @@ def config_dict(cfg, args, extra=None):
          "n_batches": cfg["n_batches"], "dims": [int(x) for x in cfg["phantom"]["dims"]],
          "voxel_cm": float(cfg["phantom"]["voxel_cm"][0]), "e_cut_MeV": cfg["params"]["e_cut_MeV"],
          "g_cut_MeV": cfg["params"]["g_cut_MeV"], "seed": cfg["seed"],
-         "histories_overridden": bool(args.histories), "ms_model": args.ms_model}
+         "histories_overridden": bool(args.histories), "ms_model": args.ms_model, "stepping": args.stepping}
     d.update(extra or {})
     return d
 
@@ -238,19 +241,41 @@ def run_engine(args):
     if world > 1:
         exchange = os.environ.get("MC_BENCH_EXCHANGE", "peer")
         if exchange == "peer":
-            ok = 1
+            ok = True
             try:
                 own = mc.mc_edep_buffer(eng.ctx, B)
                 handles = [None] * world
                 dist.all_gather_object(handles, mc.mc_ipc_get_handle(own))
+                if os.environ.get("MC_BENCH_FAIL_PEER_RANK") == str(rank):  # fault injection for the fallback test
+                    raise RuntimeError("injected peer-mapping failure")
                 peers = [own if r == rank else mc.mc_ipc_open_handle(handles[r]) for r in range(world)]
             except Exception as exc:  # noqa: BLE001  (any failure -> every rank falls back together)
                 print(f"rank {rank}: peer mapping failed ({exc}); falling back to all-reduce", file=sys.stderr)
-                ok = 0
-            flag = torch.tensor([ok], device="cuda" if backend == "nccl" else "cpu")
-            dist.all_reduce(flag, op=dist.ReduceOp.MIN)
-            if int(flag.item()) == 0:
+                ok = False
+
+            def all_min(v):
+                flag = torch.tensor([v], device="cuda" if backend == "nccl" else "cpu")
+                dist.all_reduce(flag, op=dist.ReduceOp.MIN)
+                return int(flag.item())
+            if not sharding.agree_on_peer_exchange(ok, all_min):
+                for r in range(world if peers else 0):
+                    if r != rank and peers[r] is not None:
+                        mc.mc_ipc_close_handle(peers[r])
                 exchange, peers = "allreduce (peer mapping failed)", None
+            else:
+                exchange = "peer, one voxel slice per rank + all-gather of dose and sigma"
+    chunk = sharding.voxel_slice(rank, world, nvox)[0]
+    d_slice = torch.zeros(chunk, dtype=torch.float32, device="cuda")
+    s_slice = torch.zeros_like(d_slice)
+    gathered = torch.empty(world * chunk, dtype=torch.float32, device="cuda") if world > 1 else None
+
+    def all_gather(t, _chunk):
+        if backend == "nccl":
+            dist.all_gather_into_tensor(gathered, t)
+            return gathered.clone()  # the buffer is reused for sigma
+        parts = [torch.empty(_chunk, dtype=torch.float32) for _ in range(world)]  # gloo: through the host (functional check)
+        dist.all_gather(parts, t.cpu())
+        return torch.cat(parts).cuda()
 
     def step(dose_out=None, sigma_out=None, e=None):
         e = e or eng
@@ -258,11 +283,17 @@ def run_engine(args):
         if world == 1:
             mc.mc_run(e.ctx, cfg["beam"], n, seed, B, d_out, s_out)
         elif peers is not None and e is eng:
-            mc.mc_run_range(e.ctx, cfg["beam"], n_job, h_lo, h_hi, seed, B, peers[rank])  # shard stays in place
-            st = mc.mc_get_stats(e.ctx)
-            dist.barrier()                                   # every rank's grids are complete
-            mc.mc_finalize_multi(e.ctx, peers, n_job, B, d_out, s_out)
-            dist.barrier()                                   # nobody overwrites its grids while a peer still reads
+            def finalize_slice(nj, v0, v1):
+                mc.mc_finalize_multi_range(e.ctx, peers, nj, B, v0, v1, d_slice, s_slice)
+                return d_slice, s_slice
+            d, sg = sharding.run_sharded_peer(rank, world, n, nvox,
+                                              lambda nj, a, b: mc.mc_run_range(e.ctx, cfg["beam"], nj, a, b, seed, B, peers[rank]),
+                                              dist.barrier, finalize_slice, all_gather)
+            st = mc.mc_get_stats(e.ctx)  # the transport's counters (mc_finalize_multi_range adds one launch)
+            if torch.is_tensor(d_out):
+                d_out.copy_(d); s_out.copy_(sg)
+            else:
+                d_out[:] = d.cpu().numpy(); s_out[:] = sg.cpu().numpy()
             return st
         else:
             def run_range(nj, a, b):

@@ -201,6 +201,11 @@ mc_status mc_finalize(mc_ctx *ctx, const float *edep, uint64_t n_histories, int3
 mc_status mc_edep_buffer(mc_ctx *ctx, int32_t n_batches, float **out);
 mc_status mc_finalize_multi(mc_ctx *ctx, const float *const *edep_grids, int32_t n_grids, uint64_t n_histories,
                             int32_t n_batches, float *dose_out, float *sigma_out);
+/* mc_finalize_multi_range — the same for voxels [v_begin, v_end) only: dose_out / sigma_out receive v_end - v_begin
+ * floats.  With one slice per rank (sharding.voxel_slice) every grid value is read over NVLink exactly once — the
+ * reduce-scatter shape of the exchange — and the dose / sigma slices (2 x nvox x 4 bytes in total) are all-gathered. */
+mc_status mc_finalize_multi_range(mc_ctx *ctx, const float *const *edep_grids, int32_t n_grids, uint64_t n_histories,
+                                  int32_t n_batches, int64_t v_begin, int64_t v_end, float *dose_out, float *sigma_out);
 mc_status mc_ipc_get_handle(const void *dev_ptr, uint8_t handle[64]);
 mc_status mc_ipc_open_handle(const uint8_t handle[64], void **dev_ptr);
 mc_status mc_ipc_close_handle(void *dev_ptr);

@@ -30,7 +30,7 @@ TABLE_IDS = {"mu_tot": 0, "mu_C": 1, "mu_pp": 2, "R": 3, "L": 4, "S_hard": 5, "S
 # every symbol include/mc.h declares (tests check that the library exports each of them)
 SYMBOLS = ["mc_create", "mc_destroy", "mc_build_tables", "mc_export_table", "mc_export_grid", "mc_export_gs_table",
            "mc_set_photon_tables", "mc_run", "mc_run_particles", "mc_run_range", "mc_finalize", "mc_edep_buffer",
-           "mc_finalize_multi", "mc_ipc_get_handle", "mc_ipc_open_handle", "mc_ipc_close_handle", "mc_run_atten",
+           "mc_finalize_multi", "mc_finalize_multi_range", "mc_ipc_get_handle", "mc_ipc_open_handle", "mc_ipc_close_handle", "mc_run_atten",
            "mc_philox_selftest", "mc_bench_red", "mc_bench_issue", "mc_get_stats", "mc_set_stream", "mc_set_option",
            "mc_last_error", "mc_version"]
 
@@ -89,6 +89,7 @@ def lib():
         L.mc_finalize.argtypes = [vp, vp, u64, i32, vp, vp]
         L.mc_edep_buffer.argtypes = [vp, i32, C.POINTER(vp)]
         L.mc_finalize_multi.argtypes = [vp, vp, i32, u64, i32, vp, vp]
+        L.mc_finalize_multi_range.argtypes = [vp, vp, i32, u64, i32, C.c_int64, C.c_int64, vp, vp]
         L.mc_ipc_get_handle.argtypes = [vp, vp]
         L.mc_ipc_open_handle.argtypes = [vp, C.POINTER(vp)]
         L.mc_ipc_close_handle.argtypes = [vp]
@@ -259,6 +260,14 @@ def mc_finalize_multi(ctx, grids, n_histories, n_batches, dose_out, sigma_out):
     arr = (C.c_void_p * len(addr))(*addr)
     _check(ctx, lib().mc_finalize_multi(ctx, C.addressof(arr), len(addr), int(n_histories), int(n_batches), _ptr(dose_out),
                                         _ptr(sigma_out)))
+
+
+def mc_finalize_multi_range(ctx, grids, n_histories, n_batches, v_begin, v_end, dose_out, sigma_out):
+    """As mc_finalize_multi for voxels [v_begin, v_end): the outputs hold v_end - v_begin floats."""
+    addr = [g if isinstance(g, int) else _ptr(g) for g in grids]
+    arr = (C.c_void_p * len(addr))(*addr)
+    _check(ctx, lib().mc_finalize_multi_range(ctx, C.addressof(arr), len(addr), int(n_histories), int(n_batches), int(v_begin),
+                                              int(v_end), _ptr(dose_out), _ptr(sigma_out)))
 
 
 def mc_ipc_get_handle(dev_ptr):

@@ -742,28 +742,36 @@ mc_status mc_edep_buffer(mc_ctx* ctx, int32_t n_batches, float** out) {
     return MC_OK;
 }
 
-mc_status mc_finalize_multi(mc_ctx* ctx, const float* const* edep_grids, int32_t n_grids, uint64_t n_histories, int32_t n_batches,
-                            float* dose_out, float* sigma_out) {
+mc_status mc_finalize_multi_range(mc_ctx* ctx, const float* const* edep_grids, int32_t n_grids, uint64_t n_histories, int32_t n_batches,
+                                  int64_t v_begin, int64_t v_end, float* dose_out, float* sigma_out) {
     if (!ctx) return MC_ERR_INVALID_ARG;
     if (!edep_grids || n_grids < 1 || n_grids > kMaxGrids || !dose_out || !sigma_out || n_batches < 2 || n_histories < (uint64_t)n_batches)
         return fail(ctx, MC_ERR_INVALID_ARG, "mc_finalize_multi arguments (1 <= n_grids <= 16)");
+    if (v_begin < 0 || v_end < v_begin || v_end > (int64_t)ctx->g.nvox) return fail(ctx, MC_ERR_INVALID_ARG, "mc_finalize_multi_range: voxel range");
     mc_status st;
     if ((st = ensure_device(ctx)) != MC_OK) return st;
     GridList gl;
     gl.n = n_grids;
     for (int r = 0; r < kMaxGrids; ++r) gl.g[r] = r < n_grids ? edep_grids[r] : nullptr;
     for (int r = 0; r < n_grids; ++r) if (!gl.g[r]) return fail(ctx, MC_ERR_INVALID_ARG, "mc_finalize_multi: null grid");
-    const int nvox = ctx->g.nvox;
+    const int nvox = ctx->g.nvox, nv = (int)(v_end - v_begin);
+    if (nv == 0) return MC_OK;  // an empty slice (more ranks than voxels)
     const double vol = (double)ctx->g.hx * (double)ctx->g.hy * (double)ctx->g.hz;
-    const int grid = std::min(ctx->sm_count * 8, (nvox + kThreads - 1) / kThreads);
-    finalize_multi_kernel<<<grid, kThreads, n_batches * sizeof(double), ctx->stream>>>(gl, ctx->d_vox, nvox, n_batches, n_histories, vol,
-                                                                                       ctx->d_dose, ctx->d_sigma);
+    const int grid = std::max(1, std::min(ctx->sm_count * 8, (nv + kThreads - 1) / kThreads));
+    finalize_multi_kernel<<<grid, kThreads, n_batches * sizeof(double), ctx->stream>>>(gl, ctx->d_vox, nvox, (int)v_begin, (int)v_end, n_batches,
+                                                                                       n_histories, vol, ctx->d_dose, ctx->d_sigma);
     CU(cudaGetLastError());
     ++ctx->stats.n_kernel_launches;
-    CU(cudaMemcpyAsync(dose_out, ctx->d_dose, (size_t)nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
-    CU(cudaMemcpyAsync(sigma_out, ctx->d_sigma, (size_t)nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
+    CU(cudaMemcpyAsync(dose_out, ctx->d_dose + v_begin, (size_t)nv * sizeof(float), cudaMemcpyDefault, ctx->stream));
+    CU(cudaMemcpyAsync(sigma_out, ctx->d_sigma + v_begin, (size_t)nv * sizeof(float), cudaMemcpyDefault, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     return MC_OK;
+}
+
+mc_status mc_finalize_multi(mc_ctx* ctx, const float* const* edep_grids, int32_t n_grids, uint64_t n_histories, int32_t n_batches,
+                            float* dose_out, float* sigma_out) {
+    if (!ctx) return MC_ERR_INVALID_ARG;
+    return mc_finalize_multi_range(ctx, edep_grids, n_grids, n_histories, n_batches, 0, ctx->g.nvox, dose_out, sigma_out);
 }
 
 mc_status mc_ipc_get_handle(const void* dev_ptr, uint8_t handle[64]) {

@@ -1131,12 +1131,13 @@ __global__ void __launch_bounds__(kThreads) finalize_kernel(const float* __restr
 constexpr int kMaxGrids = 16;
 struct GridList { const float* g[kMaxGrids]; int n; };
 __global__ void __launch_bounds__(kThreads) finalize_multi_kernel(const __grid_constant__ GridList grids, const uint2* __restrict__ vox,
-                                                                  int nvox, int B, unsigned long long n_total, double voxel_volume,
-                                                                  float* __restrict__ dose, float* __restrict__ sigma) {
+                                                                  int nvox, int v_begin, int v_end, int B, unsigned long long n_total,
+                                                                  double voxel_volume, float* __restrict__ dose, float* __restrict__ sigma) {
     extern __shared__ double s_inv_nb[];
     for (int b = threadIdx.x; b < B; b += blockDim.x) s_inv_nb[b] = 1.0 / batch_size(n_total, B, b);
     __syncthreads();
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < nvox; i += gridDim.x * blockDim.x) {
+    // voxels [v_begin, v_end): with one slice per rank every grid value crosses NVLink once (reduce-scatter shape)
+    for (int i = v_begin + blockIdx.x * blockDim.x + threadIdx.x; i < v_end; i += gridDim.x * blockDim.x) {
         const double inv_mass = 1.0 / ((double)__uint_as_float(vox[i].x) * voxel_volume);
         double mean = 0.0, sq = 0.0;
         for (int b = 0; b < B; ++b) {

@@ -69,6 +69,17 @@ def _rank_main(rank, world, port, n_per_rank, B, out_dir):
     peers = [own if r == rank else mc.mc_ipc_open_handle(handles[r]) for r in range(world)]
     dose, sig = np.zeros(eng.nvox, np.float32), np.zeros(eng.nvox, np.float32)
     mc.mc_finalize_multi(eng.ctx, peers, n_job, B, dose, sig)
+    # the sliced form bench.py --gpus N uses: this rank's voxel slice of the sum, then an all-gather of the slices
+    chunk, v0, v1 = sharding.voxel_slice(rank, world, eng.nvox)
+    ds, ss = np.zeros(chunk, np.float32), np.zeros(chunk, np.float32)
+    mc.mc_finalize_multi_range(eng.ctx, peers, n_job, B, v0, v1, ds, ss)
+    parts = [torch.empty(chunk) for _ in range(world)]
+    dist.all_gather(parts, torch.from_numpy(ds))
+    assert np.array_equal(torch.cat(parts).numpy()[:eng.nvox], dose)
+    dist.all_gather(parts, torch.from_numpy(ss))
+    assert np.array_equal(torch.cat(parts).numpy()[:eng.nvox], sig)
+    with pytest.raises(mc.McError):
+        mc.mc_finalize_multi_range(eng.ctx, peers, n_job, B, 5, eng.nvox + 1, ds, ss)
     dist.barrier()                                                   # nobody frees before everybody has read
     for r in range(world):
         if r != rank:
@@ -94,3 +105,27 @@ def test_two_ranks_exchange_their_grids_through_cuda_ipc(tmp_path):
         assert np.allclose(d, d_ref, rtol=2e-5, atol=1e-7 * d_ref.max())
         assert np.allclose(s, s_ref, rtol=5e-3, atol=1e-6 * d_ref.max())
     assert d_ref.max() > 0
+
+
+@pytest.mark.parametrize("fail_rank", ["", "1"])
+def test_bench_two_ranks_on_one_gpu_peer_exchange_and_joint_fallback(fail_rank):
+    """bench.py --gpus 2 with both ranks on this box's one GPU (gloo for the plumbing: a functional check, not a measurement):
+    the fused, voxel-sliced exchange, and — with a peer-mapping failure injected on rank 1 — the joint fallback of ALL
+    ranks to the all-reduce; both give the same statistics as each other."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, MC_BENCH_BACKEND="gloo", MC_BENCH_FAIL_PEER_RANK=fail_rank)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(_free_port()), os.path.join(root, "bench.py"), "--gpus", "2", "--config", "1", "--steps", "2",
+           "--warmup", "3", "--no-cpu-baseline", "--no-e2e"]
+    out = subprocess.run(cmd, env=env, capture_output=True, text=True, timeout=600, cwd=root)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
+    assert line["n_gpus"] == 2 and line["ledger_rel"] < 1e-4
+    par = line["config"]["parallelism"]
+    assert ("peer mapping failed" in par) == (fail_rank != ""), par
+    assert ("one voxel slice per rank" in par) == (fail_rank == ""), par
+    # the statistics do not depend on the exchange: same job, same seed
+    assert line["mean_rel_sigma_10pct_isodose"] == pytest.approx(0.006, rel=0.25)
