@@ -178,6 +178,18 @@ typedef struct {
 mc_status mc_run_particles(mc_ctx *ctx, const mc_particle *particles, uint64_t n, uint64_t seed, int32_t n_batches,
                            float *dose_out, float *sigma_out);
 
+/* mc_run_source — as mc_run_particles, but the records come from a user function ("a user can either load source
+ * particles from a phase-space file or write a CPU/GPU function"): the library calls
+ *     fn(user, h_begin, n, out, cuda_stream)
+ * once per wave of histories [h_begin, h_begin + n) (n <= option "wave_size", waves in ascending order); the function
+ * writes records h_begin .. h_begin + n - 1 to out — DEVICE memory owned by the library, valid during the call — either
+ * with a kernel of its own launched on cuda_stream (a cudaStream_t; work enqueued there is ordered before the
+ * library's use of the records, no synchronisation needed) or with a copy from host memory, and returns 0 (anything
+ * else aborts the run with MC_ERR_INVALID_ARG).  Records are validated on the device as for a device-resident list. */
+typedef int (*mc_source_fn)(void *user, uint64_t h_begin, uint64_t n, mc_particle *out, void *cuda_stream);
+mc_status mc_run_source(mc_ctx *ctx, mc_source_fn fn, void *user, uint64_t n, uint64_t seed, int32_t n_batches,
+                        float *dose_out, float *sigma_out);
+
 /* mc_run_range — the shard of mc_run one GPU of several computes: histories [h_begin, h_end) of a
  * job of n_histories.  edep_out: n_batches*nvox floats (host or device), energy deposited per batch
  * grid in MeV (sum these over shards, then call mc_finalize). */

@@ -29,7 +29,7 @@ TABLE_IDS = {"mu_tot": 0, "mu_C": 1, "mu_pp": 2, "R": 3, "L": 4, "S_hard": 5, "S
 
 # every symbol include/mc.h declares (tests check that the library exports each of them)
 SYMBOLS = ["mc_create", "mc_destroy", "mc_build_tables", "mc_export_table", "mc_export_grid", "mc_export_gs_table",
-           "mc_set_photon_tables", "mc_run", "mc_run_particles", "mc_run_range", "mc_finalize", "mc_edep_buffer",
+           "mc_set_photon_tables", "mc_run", "mc_run_particles", "mc_run_source", "mc_run_range", "mc_finalize", "mc_edep_buffer",
            "mc_finalize_multi", "mc_finalize_multi_range", "mc_ipc_get_handle", "mc_ipc_open_handle", "mc_ipc_close_handle", "mc_run_atten",
            "mc_philox_selftest", "mc_bench_red", "mc_bench_issue", "mc_get_stats", "mc_set_stream", "mc_set_option",
            "mc_last_error", "mc_version"]
@@ -235,6 +235,22 @@ def mc_run_particles(ctx, particles, seed, n_batches, dose_out, sigma_out, n=Non
         n = len(particles)
     _check(ctx, lib().mc_run_particles(ctx, _ptr(particles), int(n), int(seed), int(n_batches), _ptr(dose_out),
                                        _ptr(sigma_out)))
+
+
+SOURCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p)
+
+
+def mc_run_source(ctx, fn, n, seed, n_batches, dose_out, sigma_out):
+    """fn(h_begin, n, out_device_address, cuda_stream) -> 0 on success: writes records h_begin .. h_begin + n - 1 (PARTICLE_DTYPE
+    layout) to device memory at out_device_address, with work enqueued on cuda_stream or a blocking copy (marshalling only)."""
+    def trampoline(_user, h_begin, cnt, out, stream):
+        try:
+            return int(fn(int(h_begin), int(cnt), int(out), int(stream or 0)) or 0)
+        except Exception:  # noqa: BLE001  (an exception must not cross the C boundary)
+            return 1
+    cb = SOURCE_FN(trampoline)
+    _check(ctx, lib().mc_run_source(ctx, cb, None, C.c_uint64(int(n)), C.c_uint64(int(seed)), int(n_batches), C.c_void_p(_ptr(dose_out)),
+                                    C.c_void_p(_ptr(sigma_out))))
 
 
 def mc_run_range(ctx, beam, n_histories, h_begin, h_end, seed, n_batches, edep_out):

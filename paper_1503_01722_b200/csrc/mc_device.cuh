@@ -49,7 +49,7 @@ struct Queue {
     uint32_t* count;  // device counter (tail)
     uint32_t cap;
 };
-enum Counter { C_HEAD = 0, C_E_A, C_E_B, C_P, C_OVERFLOW, C_DONE, C_COUNT };  // C_DONE: CTAs of the running launch that have finished
+enum Counter { C_HEAD = 0, C_E_A, C_E_B, C_P, C_OVERFLOW, C_DONE, C_FLAGS, C_COUNT };  // C_FLAGS: validation flags of a source function's records;  // C_DONE: CTAs of the running launch that have finished
 enum StatId {
     S_ESTEP = 0, S_FLIGHT, S_FICT, S_COMPTON, S_PAIR, S_PE, S_MOLLER, S_BREMS, S_SEC_E, S_SEC_G, S_ATOMICS,
     S_HIST, S_COUNT

@@ -32,6 +32,8 @@ struct mc_ctx {
     uint2* d_vox = nullptr;
     float2 *d_tabP = nullptr, *d_tabE = nullptr;
     size_t tabP_cap = 0, tabE_cap = 0;
+    ListParticle* d_wave = nullptr;  // one wave of records filled by a user source function (mc_run_source)
+    size_t wave_cap = 0;
     float* d_gs = nullptr;  // Goudsmit-Saunderson quantile table + per-material coarse ln A table (flags & MC_FLAG_MS_GS)
     size_t gs_cap = 0, gs_words = 0;
     int gs_n8 = 0;
@@ -309,8 +311,11 @@ namespace {
 // full wave goes first, otherwise the group with the most particles (source included).
 // Source: a beam (primaries sampled inside the transport kernels) or, with beam == nullptr, a device-resident
 // particle list whose entry h is history h (loaded into the queues a wave at a time).
+// A user source function (mc_run_source) stands in for the list: it fills one wave of records at a time.
+struct SourceFn { mc_source_fn fn = nullptr; void* user = nullptr; };
+
 mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list, uint64_t n_total, uint64_t h0, uint64_t h1,
-                    uint64_t seed, int n_batches, float* d_edep) {
+                    uint64_t seed, int n_batches, float* d_edep, SourceFn src = SourceFn()) {
     mc_status st;
     if ((st = ensure_device(ctx)) != MC_OK) return st;
     if ((st = upload_tables(ctx)) != MC_OK) return st;
@@ -421,6 +426,8 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
             ctx->beam_key = -1.0;  // the remembered ratios admitted too much: probe again next time
             return fail(ctx, MC_ERR_QUEUE_OVERFLOW, "particle queue overflow: lower option wave_size or raise queue_factor");
         }
+        if (ctx->h_counters[C_FLAGS] & 1u) return fail(ctx, MC_ERR_ENERGY_RANGE, "source function: particle energy not in (0, e_max_MeV]");
+        if (ctx->h_counters[C_FLAGS] & 6u) return fail(ctx, MC_ERR_INVALID_ARG, "source function: directions must be unit vectors and particle types -1, 0 or 1");
         cnt_e[0] = ctx->h_counters[C_E_A]; cnt_e[1] = ctx->h_counters[C_E_B]; cnt_p = ctx->h_counters[C_P];
         return MC_OK;
     };
@@ -441,9 +448,24 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
     // ---- launches decided one at a time from the counters (Table 1): particle lists, the probe launches of
     // a beam whose secondaries-per-primary ratios are not known yet, and everything when option plan_ahead is 0 --------
     while ((remaining > 0 || cnt_e[cur] > 0 || cnt_p > 0) && !(plan_ahead && have_ratio)) {
-        if (d_list && remaining > 0 && cnt_e[cur] < W && cnt_p < W) {
+        if ((d_list || src.fn) && remaining > 0 && cnt_e[cur] < W && cnt_p < W) {
             // particle-list source: the next wave of listed particles goes straight into the input queues
             const uint32_t n_load = (uint32_t)std::min<uint64_t>(remaining, W);
+            if (src.fn) {
+                // user source function ("write a CPU/GPU function"): it fills this wave's records — by a kernel of
+                // its own on the stream it is given, or by a copy — and the wave is validated like a device-resident list
+                if (ctx->wave_cap < n_load) {
+                    cudaFree(ctx->d_wave); ctx->d_wave = nullptr; ctx->wave_cap = 0;
+                    CU(cudaMalloc(&ctx->d_wave, (size_t)W * sizeof(ListParticle)));
+                    ctx->wave_cap = W;
+                }
+                if (src.fn(src.user, h_next, n_load, reinterpret_cast<mc_particle*>(ctx->d_wave), (void*)s) != 0)
+                    return fail(ctx, MC_ERR_INVALID_ARG, "the source function reported a failure");
+                check_particles_kernel<<<std::min<uint32_t>((n_load + kThreads - 1) / kThreads, (uint32_t)ctx->sm_count * 8), kThreads, 0, s>>>(
+                    ctx->d_wave, n_load, ctx->params.e_max_MeV, ctx->d_counters + C_FLAGS);
+                CU(cudaGetLastError());
+                d_list = ctx->d_wave - h_next;  // record h of the job = entry h - h_next of the wave
+            }
             P.h_first = h_next; P.n_new = 0;
             P.q_e_out = Queue{ctx->d_q[cur], ctx->d_counters + C_E_A + cur, ctx->q_cap};
             P.q_p_out = Queue{ctx->d_q[2], ctx->d_counters + C_P, ctx->q_cap};
@@ -613,7 +635,7 @@ mc_status mc_create(const uint8_t* material_idx, const float* density_gcc, const
 void mc_destroy(mc_ctx* ctx) {
     if (!ctx) return;
     if (ctx->dev_ready) {
-        cudaFree(ctx->d_vox); cudaFree(ctx->d_tabP); cudaFree(ctx->d_tabE); cudaFree(ctx->d_gs);
+        cudaFree(ctx->d_vox); cudaFree(ctx->d_tabP); cudaFree(ctx->d_tabE); cudaFree(ctx->d_gs); cudaFree(ctx->d_wave);
         for (auto q : ctx->d_q) if (q) cudaFreeAsync(q, nullptr);  // back to the pool (see transport())
         cudaFree(ctx->d_counters); cudaFreeHost(ctx->h_counters); cudaFree(ctx->d_stats); cudaFree(ctx->d_ledger);
         cudaFree(ctx->d_edep); cudaFree(ctx->d_dose); cudaFree(ctx->d_sigma); cudaFree(ctx->d_beam);
@@ -870,6 +892,27 @@ mc_status mc_run_particles(mc_ctx* ctx, const mc_particle* particles, uint64_t n
     } else cudaStreamSynchronize(ctx->stream);
     if (staged) cudaFree(staged);
     return st;
+}
+
+mc_status mc_run_source(mc_ctx* ctx, mc_source_fn fn, void* user, uint64_t n, uint64_t seed, int32_t n_batches, float* dose_out,
+                        float* sigma_out) {
+    if (!ctx) return MC_ERR_INVALID_ARG;
+    if (!ctx->have_tables) return fail(ctx, MC_ERR_STATE, "mc_build_tables has not been called");
+    if (!fn || !dose_out || !sigma_out) return fail(ctx, MC_ERR_INVALID_ARG, "null pointer");
+    if (n == 0 || n >= (1ull << 32)) return fail(ctx, MC_ERR_INVALID_ARG, "n must be in [1, 2^32)");
+    if (n_batches < 2 || (uint64_t)n_batches > n) return fail(ctx, MC_ERR_INVALID_ARG, "n_batches must be in [2, n]");
+    if ((uint64_t)n_batches * (uint64_t)ctx->g.nvox >= (1ull << 32)) return fail(ctx, MC_ERR_INVALID_ARG, "n_batches * nvox must be < 2^32");
+    mc_status st;
+    if ((st = ensure_device(ctx)) != MC_OK) return st;
+    const size_t nvox = ctx->g.nvox;
+    if ((st = ensure_edep(ctx, (size_t)n_batches * nvox)) != MC_OK) return st;
+    SourceFn src; src.fn = fn; src.user = user;
+    if ((st = transport(ctx, nullptr, nullptr, n, 0, n, seed, n_batches, ctx->d_edep, src)) != MC_OK) { cudaStreamSynchronize(ctx->stream); return st; }
+    if ((st = finalize_device(ctx, ctx->d_edep, n, n_batches)) != MC_OK) return st;
+    CU(cudaMemcpyAsync(dose_out, ctx->d_dose, nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
+    CU(cudaMemcpyAsync(sigma_out, ctx->d_sigma, nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return MC_OK;
 }
 
 mc_status mc_run_atten(mc_ctx* ctx, const mc_beam* beam, uint64_t n, uint64_t seed, int32_t* voxel_out, uint8_t* channel_out) {

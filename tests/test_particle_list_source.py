@@ -125,3 +125,58 @@ def test_mc_run_particles_matches_the_oracle():
     mc.mc_run_particles(eng.ctx, t, 2, B, d2, s2, n=n)  # the context still works after a rejected list
     assert np.allclose(d2.cpu().numpy(), d, rtol=1e-4, atol=1e-6 * d.max())
     eng.close()
+
+
+@pytest.mark.gpu
+def test_mc_run_source_user_gpu_and_cpu_functions_reproduce_the_list():
+    """PAPER.md:84: "a user can either load source particles from a phase-space file or write a CPU/GPU function".  The
+    function is called once per wave; a GPU function enqueues its work on the stream it is given (here: a torch kernel
+    plus a device-to-device copy), a CPU function copies from host memory.  Both must reproduce mc_run_particles on the
+    same records exactly (same histories, same streams), over several waves."""
+    import ctypes as C
+    import torch
+    import paper_1503_01722_b200 as mc
+    assert torch.cuda.is_available()
+    cudart = C.CDLL("libcudart.so.12")
+    cfg = W.config(4, "g")
+    n, B = 60000, 6
+    p = W.phase_space(n, seed=5)
+    eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])
+    mc.mc_set_option(eng.ctx, "wave_size", 16384)
+    d0, s0 = np.zeros(eng.nvox, np.float32), np.zeros(eng.nvox, np.float32)
+    mc.mc_run_particles(eng.ctx, p, 3, B, d0, s0)
+    st0 = eng.stats()
+    t_all = torch.from_numpy(p.view(np.uint8).reshape(-1).copy()).cuda()
+    calls = []
+
+    def gpu_fn(h0, cnt, out, stream):
+        calls.append((h0, cnt))
+        with torch.cuda.stream(torch.cuda.ExternalStream(stream) if stream else torch.cuda.default_stream()):
+            chunk = t_all[32 * h0:32 * (h0 + cnt)].clone()  # the user's own kernel, on the library's stream
+            rc = cudart.cudaMemcpyAsync(C.c_void_p(out), C.c_void_p(chunk.data_ptr()), C.c_size_t(32 * cnt), 3, C.c_void_p(stream))
+            chunk.record_stream(torch.cuda.current_stream())
+        return rc
+
+    def cpu_fn(h0, cnt, out, stream):
+        q = np.ascontiguousarray(p[h0:h0 + cnt])
+        return cudart.cudaMemcpy(C.c_void_p(out), C.c_void_p(q.ctypes.data), C.c_size_t(32 * cnt), 1)
+
+    for fn in (gpu_fn, cpu_fn):
+        d, s = np.zeros(eng.nvox, np.float32), np.zeros(eng.nvox, np.float32)
+        mc.mc_run_source(eng.ctx, fn, n, 3, B, d, s)
+        st = eng.stats()
+        assert (st["n_electron_steps"], st["n_photon_flights"], st["n_compton"]) == (st0["n_electron_steps"], st0["n_photon_flights"], st0["n_compton"])
+        assert np.allclose(d, d0, rtol=1e-4, atol=1e-6 * d0.max()) and np.allclose(s, s0, rtol=5e-3, atol=1e-6 * d0.max())
+    assert calls == [(0, 16384), (16384, 16384), (32768, 16384), (49152, n - 49152)]  # ascending waves of at most wave_size
+    # a function that fails, and records that break the contract
+    with pytest.raises(mc.McError) as e:
+        mc.mc_run_source(eng.ctx, lambda *a: 7, n, 3, B, d, s)
+    assert e.value.status == mc.MC_ERR_INVALID_ARG
+    bad = p.copy(); bad["E"][20000] = 99.0
+    with pytest.raises(mc.McError) as e:
+        mc.mc_run_source(eng.ctx, lambda h0, cnt, out, stream: cudart.cudaMemcpy(
+            C.c_void_p(out), C.c_void_p(np.ascontiguousarray(bad[h0:h0 + cnt]).ctypes.data), C.c_size_t(32 * cnt), 1), n, 3, B, d, s)
+    assert e.value.status == mc.MC_ERR_ENERGY_RANGE
+    mc.mc_run_source(eng.ctx, cpu_fn, n, 3, B, d, s)  # the context still works
+    assert np.allclose(d, d0, rtol=1e-4, atol=1e-6 * d0.max())
+    eng.close()
