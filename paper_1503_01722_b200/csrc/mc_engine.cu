@@ -198,8 +198,9 @@ size_t smem_e(const mc_ctx* c, int T) {
            2 * (size_t)T * sizeof(uint32_t) + (size_t)(T / 32) * (2 * sizeof(double) + 8 * sizeof(uint32_t)) + gs;
 }
 size_t smem_p(const mc_ctx* c, int T) {
-    return (size_t)(1 + c->tabs.n_mat * TP_COUNT) * c->tabs.N * sizeof(float2) + (size_t)SP_COUNT * T * sizeof(uint32_t) +
-           2 * (size_t)T * sizeof(double) + (size_t)(kTrackWordsP * kSlotsP + kSlotsP + 1) * T * sizeof(uint32_t);
+    const size_t ntab = (size_t)(1 + c->tabs.n_mat * TP_COUNT) * c->tabs.N;
+    return ((ntab + 1) & ~(size_t)1) * sizeof(float2) + (size_t)kGroupsP * kSlotsP * T * sizeof(uint4) + (size_t)kSlotsP * T * sizeof(uint32_t) +
+           2 * (size_t)T * sizeof(uint32_t) + (size_t)T * sizeof(double) + (size_t)(T / 32) * (sizeof(double) + 8 * sizeof(uint32_t));
 }
 constexpr size_t kSmemMax = 227 * 1024;  // opt-in dynamic shared memory per CTA on sm_100
 using TransportKernel = void (*)(const RunParams);
@@ -216,8 +217,8 @@ bool choose_electron_kernel(const mc_ctx* c, KernelChoice& k) {
     return false;
 }
 bool choose_photon_kernel(const mc_ctx* c, KernelChoice& k) {
-    const int T[3] = {896, 768, 512};
-    const TransportKernel fn[3] = {photon_kernel<896>, photon_kernel<768>, photon_kernel<512>};
+    const int T[3] = {1024, 768, 512};
+    const TransportKernel fn[3] = {photon_kernel<1024>, photon_kernel<768>, photon_kernel<512>};
     for (int i = 0; i < 3; ++i)
         if (smem_p(c, T[i]) <= kSmemMax) { k = KernelChoice{fn[i], T[i], smem_p(c, T[i])}; return true; }
     return false;

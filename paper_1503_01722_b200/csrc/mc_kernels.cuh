@@ -750,70 +750,82 @@ __global__ void __launch_bounds__(kThreadsE, 1) electron_kernel(const __grid_con
 // =================================================================================================
 // photon kernel: Woodcock tracking (R3), Compton (R4), pair (R12),
 // photoelectric absorption (R16).  One Philox block serves two flights.  Same warp scheduling as the electron
-// kernel: per iteration a warp runs ONE of  FLY (lanes in L_STEP) / COMPTON (lanes in L_HARD, pending) /
-// REFILL (lanes in L_IDLE), the rare blocks only when enough lanes want them.
+// kernel: per iteration a warp runs ONE of  FLY (tracks in L_STEP) / COMPTON (tracks in L_HARD, pending) /
+// REFILL (slots in L_IDLE), the rare blocks only when enough tracks want them.  A track is three 16-byte groups
+//   G0 x y z E | G1 u v w block | G2 tag hist trk_lo trk_hi   (+ one word: the voxel of a pending Compton event),
+// positions in world coordinates (Woodcock flights look the voxel up by position, no boundary computation).
 // =================================================================================================
-// kThreadsP = CTA size of the photon kernel: 896 (28 warps), 768 or 512 by what fits (one CTA per SM)
+// kThreadsP = CTA size of the photon kernel: 1024 (32 warps), 768 or 512 by what fits (one CTA per SM)
 constexpr int kSlotsP = 3;     // tracks per lane in the warp's pool (shared memory)
-constexpr int kTrackWordsP = 13;
+constexpr int kGroupsP = 3;    // 16-byte groups per track
 enum { SP_FLIGHT = 0, SP_FICT, SP_COMPTON, SP_PAIR, SP_PE, SP_SEC_E, SP_HIST, SP_RED, SP_COUNT };
 
 template <int kThreadsP>
 __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_constant__ RunParams P) {
-    extern __shared__ float2 s_tab[];
+    extern __shared__ __align__(16) float2 s_tab[];
     const uint32_t n_in = *static_cast<const volatile uint32_t*>(P.q_in.count);  // as in electron_kernel
     if (n_in + P.n_new == 0u) return;
     const int ntab = (1 + P.n_mat * TP_COUNT) * P.N;
-    uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_tab + ntab);              // [SP_COUNT][kThreadsP]
-    double* s_led = reinterpret_cast<double*>(s_cnt + SP_COUNT * kThreadsP);  // [2][kThreadsP]: e_src, e_esc
-    uint32_t* s_trk = reinterpret_cast<uint32_t*>(s_led + 2 * kThreadsP);      // [kTrackWordsP][kSlotsP][kThreadsP]
-    uint32_t* s_st = s_trk + kTrackWordsP * kSlotsP * kThreadsP;               // [kSlotsP][kThreadsP]: slot states
-    uint32_t* s_asg = s_st + kSlotsP * kThreadsP;                              // [kThreadsP]: per-warp assignment
+    constexpr int kWarps = kThreadsP / 32;
+    constexpr int GS = kSlotsP * kThreadsP;  // uint4 stride between the groups of a track
+    uint4* s_trk = reinterpret_cast<uint4*>(s_tab + ((ntab + 1) & ~1));        // [kGroupsP][kSlotsP][kThreadsP]
+    uint32_t* s_vox = reinterpret_cast<uint32_t*>(s_trk + kGroupsP * GS);      // [kSlotsP][kThreadsP]: voxel of a pending Compton event
+    uint32_t* s_st = s_vox + GS;                                               // [kThreadsP]: byte k = state of slot k
+    uint32_t* s_asg = s_st + kThreadsP;                                        // [kThreadsP]: per-warp assignment
+    double* s_esc = reinterpret_cast<double*>(s_asg + kThreadsP);              // [kThreadsP]: escaped energy per thread
+    double* s_src = s_esc + kThreadsP;                                         // [kWarps]: source energy of the warp
+    uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_src + kWarps);             // [kWarps][8]: event counters of the warp
     for (int i = threadIdx.x; i < ntab; i += kThreadsP) s_tab[i] = P.tabP[i];
     const int tid = threadIdx.x;
+    if (tid < 8 * kWarps) s_cnt[tid] = 0u;
+    if (tid < kWarps) s_src[tid] = 0.0;
+    s_esc[tid] = 0.0;
+    uint32_t st0 = 0u;  // slots beyond kSlotsP do not exist: L_DONE
 #pragma unroll
-    for (int k = 0; k < SP_COUNT; ++k) s_cnt[k * kThreadsP + tid] = 0u;
-    s_led[tid] = 0.0; s_led[kThreadsP + tid] = 0.0;
+    for (int k = kSlotsP; k < 4; ++k) st0 |= (uint32_t)L_DONE << (8 * k);
+    s_st[tid] = st0;
     __syncthreads();
     const int lane = tid & 31;
+    const unsigned lt_mask = (1u << lane) - 1u;
     const int N = P.N;
     const Geometry& g = P.g;
     const bool local_sec = P.flags & 4u;
     const int KC = P.hard_lanes, KR = P.refill_lanes;
     const float lg_a = kLn2F * P.inv_dlnP, lg_b = P.lnE0P * P.inv_dlnP;  // table coordinate = lg2(E) * lg_a - lg_b
+    uint32_t* const w_cnt = s_cnt + 8 * (tid >> 5);
 
     int state = L_IDLE;  // state of the track being worked on
-#pragma unroll
-    for (int k = 0; k < kSlotsP; ++k) s_st[k * kThreadsP + tid] = L_IDLE;
     const int wbase = tid & ~31;
-    int slot = 0;
+    int slot = 0;        // pool slot of the track being worked on: owner thread * 4 + k
     float x = 0, y = 0, z = 0, u = 0, v = 0, w = 1, E = 0, lf = 0, maj = 1;
     int li = 0, vox = 0;
     Rng rng = {0, 0, 0, 0};
     uint32_t tag = 0;
-    auto W = [&](int f, int sl) -> uint32_t& { return s_trk[f * (kSlotsP * kThreadsP) + sl]; };
-    auto store_slot = [&](int sl) {
-        W(0, sl) = __float_as_uint(x); W(1, sl) = __float_as_uint(y); W(2, sl) = __float_as_uint(z);
-        W(3, sl) = __float_as_uint(u); W(4, sl) = __float_as_uint(v); W(5, sl) = __float_as_uint(w);
-        W(6, sl) = __float_as_uint(E); W(7, sl) = (uint32_t)vox; W(8, sl) = tag;
-        W(9, sl) = rng.hist; W(10, sl) = rng.trk_lo; W(11, sl) = rng.trk_hi; W(12, sl) = rng.block;
+    auto trk = [&](int s) -> uint4* { return s_trk + (s & 3) * kThreadsP + (s >> 2); };
+    // what = 0: a new track, every group; 1: after flights or a Compton event (identity words unchanged)
+    auto store_slot = [&](int s, int what) {
+        uint4* t = trk(s);
+        t[0] = make_uint4(__float_as_uint(x), __float_as_uint(y), __float_as_uint(z), __float_as_uint(E));
+        t[GS] = make_uint4(__float_as_uint(u), __float_as_uint(v), __float_as_uint(w), rng.block);
+        if (what == 0) t[2 * GS] = make_uint4(tag, rng.hist, rng.trk_lo, rng.trk_hi);
+        if (state == L_HARD) s_vox[(s & 3) * kThreadsP + (s >> 2)] = (uint32_t)vox;
     };
-    auto load_slot = [&](int sl) {
-        x = __uint_as_float(W(0, sl)); y = __uint_as_float(W(1, sl)); z = __uint_as_float(W(2, sl));
-        u = __uint_as_float(W(3, sl)); v = __uint_as_float(W(4, sl)); w = __uint_as_float(W(5, sl));
-        E = __uint_as_float(W(6, sl)); vox = (int)W(7, sl); tag = W(8, sl);
-        rng.hist = W(9, sl); rng.trk_lo = W(10, sl); rng.trk_hi = W(11, sl); rng.block = W(12, sl);
+    auto load_slot = [&](int s) {
+        const uint4* t = trk(s);
+        const uint4 a = t[0], b = t[GS], c = t[2 * GS];
+        x = __uint_as_float(a.x); y = __uint_as_float(a.y); z = __uint_as_float(a.z); E = __uint_as_float(a.w);
+        u = __uint_as_float(b.x); v = __uint_as_float(b.y); w = __uint_as_float(b.z); rng.block = b.w;
+        tag = c.x; rng.hist = c.y; rng.trk_lo = c.z; rng.trk_hi = c.w;
     };
-    auto park = [&]() {
-        if (state == L_STEP || state == L_HARD) store_slot(slot);
-        s_st[slot] = (uint32_t)state;
+    auto park = [&](int what) {
+        if (state == L_STEP || state == L_HARD) store_slot(slot, what);
+        reinterpret_cast<volatile uint8_t*>(s_st)[slot] = (uint8_t)state;
     };
-
-    auto bump = [&](int k, uint32_t n) { s_cnt[k * kThreadsP + tid] += n; };
+    auto bump = [&](int k) { atomicAdd(w_cnt + k, 1u); };
     auto deposit = [&](int vx, float e) {
         const uint32_t cell = (tag >> 2) * (uint32_t)g.nvox + (uint32_t)vx;
-        if (P.aggregate) { if (red_add_aggregated(P.edep, cell, e)) bump(SP_RED, 1u); }
-        else { atomicAdd(P.edep + cell, e); bump(SP_RED, 1u); }
+        if (P.aggregate) { if (red_add_aggregated(P.edep, cell, e)) bump(SP_RED); }
+        else { atomicAdd(P.edep + cell, e); bump(SP_RED); }
     };
     auto set_energy = [&]() {  // table coordinate and majorant of the current energy
         float t = fmaf(f_lg2(E), lg_a, -lg_b);
@@ -822,29 +834,29 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
     };
     auto emit_e = [&](const QRec& r) {
         if (local_sec) { deposit(r.vox, r.E + (((r.tag & 3u) == CODE_POSITRON) ? 2.0f * kMeF : 0.0f)); return; }
-        bump(SP_SEC_E, 1u);
+        bump(SP_SEC_E);
         push_record(P.q_e_out, P.counters + C_OVERFLOW, r);
     };
 
     for (;;) {
-        unsigned ms[kSlotsP], mh[kSlotsP], mi[kSlotsP];
-        int nf = 0, nc = 0, ni = 0;
+        // scheduling as in electron_kernel: one-hot byte counters of the slot states summed over the warp
+        const uint32_t sw = s_st[tid];
+        uint32_t cnt1 = 0u;
 #pragma unroll
-        for (int k = 0; k < kSlotsP; ++k) {
-            const uint32_t sk = s_st[k * kThreadsP + tid];
-            ms[k] = __ballot_sync(kFull, sk == L_STEP); mh[k] = __ballot_sync(kFull, sk == L_HARD);
-            mi[k] = __ballot_sync(kFull, sk == L_IDLE);
-            nf += __popc(ms[k]); nc += __popc(mh[k]); ni += __popc(mi[k]);
-        }
-        if ((nf | nc | ni) == 0) break;
+        for (int k = 0; k < kSlotsP; ++k) cnt1 += 1u << (8u * ((sw >> (8 * k)) & 3u));
+        const uint32_t tot = __reduce_add_sync(kFull, cnt1);
+        const int ni = (int)(tot & 0xffu), nf = (int)((tot >> 8) & 0xffu), nc = (int)((tot >> 16) & 0xffu);
+        if ((tot & 0xffffffu) == 0u) break;
         const bool do_comp = nc >= KC || (nc > nf && nc >= ni);
         const bool do_refill = !do_comp && (ni >= KR || ni > nf);
+        const uint32_t cs = do_comp ? (uint32_t)L_HARD : (do_refill ? (uint32_t)L_IDLE : (uint32_t)L_STEP);
         int rank = 0;
 #pragma unroll
         for (int k = 0; k < kSlotsP; ++k) {
-            const unsigned m = do_comp ? mh[k] : (do_refill ? mi[k] : ms[k]);
-            const int r = rank + __popc(m & ((1u << lane) - 1u));
-            if (((m >> lane) & 1u) && r < 32) s_asg[wbase + r] = (uint32_t)(k * kThreadsP + tid);
+            const bool mine = ((sw >> (8 * k)) & 0xffu) == cs;
+            const unsigned m = __ballot_sync(kFull, mine);
+            const int r = rank + __popc(m & lt_mask);
+            if (mine && r < 32) s_asg[wbase + r] = (uint32_t)(tid * 4 + k);
             rank += __popc(m);
         }
         __syncwarp();
@@ -856,6 +868,7 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
         if (do_refill) {
             // ---- REFILL (S0, S1) --------------------------------------------------------------------------------
             uint32_t item = claim(P.counters + C_HEAD, n_work >= 32 ? kFull : ((1u << n_work) - 1u), lane);
+            float e_new = 0.0f;  // source energy of a new primary
             if (have) {
                 state = L_IDLE;
                 bool ok = false;
@@ -871,18 +884,24 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
                     uint4 w4 = next_block_rk(rng, P);
                     Primary p = sample_primary<false>(P, w4);
                     tag = (batch_of(h, P.n_batches, P.n_total, P.inv_n_total) << 2) | CODE_PHOTON;
-                    s_led[tid] += (double)p.E; bump(SP_HIST, 1u);
+                    e_new = p.E;
                     x = p.x; y = p.y; z = p.z; u = p.u; v = p.v; w = p.w; E = p.E;
                     vox = p.ix + g.nx * (p.iy + g.ny * p.iz);
-                    if (p.inside) ok = true; else s_led[kThreadsP + tid] += (double)p.E;
+                    if (p.inside) ok = true; else s_esc[tid] += (double)p.E;
                 } else state = L_DONE;
                 if (ok) {
                     if (E < P.g_cut) deposit(vox, E);  // absorbed where it was born
                     else state = L_STEP;
                 }
-                park();
+                park(0);
             }
             __syncwarp();
+            const unsigned m_new = __ballot_sync(kFull, e_new > 0.0f);
+            if (m_new) {  // ledger and history count of this refill: one warp-level sum
+                const float s_new = warp_sum_f(e_new);
+                if (lane == 0) { s_src[tid >> 5] += (double)s_new; w_cnt[SP_HIST] += (uint32_t)__popc(m_new); }
+                __syncwarp();
+            }
             continue;
         }
 
@@ -890,7 +909,8 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
             // ---- COMPTON: Klein-Nishina by the epsilon decomposition (R4) ----------------------------------------
             if (have) {
                 load_slot(slot);
-                bump(SP_COMPTON, 1u);
+                vox = (int)s_vox[(slot & 3) * kThreadsP + (slot >> 2)];
+                bump(SP_COMPTON);
                 const float k0 = E * (1.0f / kMeF), e0 = f_rcp(1.0f + 2.0f * k0), e02 = e0 * e0;
                 const float a1 = -f_lg2(e0) * kLn2F, a2 = 0.5f * (1.0f - e02), ik0 = f_rcp(k0);
                 float eps, tt;
@@ -926,7 +946,7 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
                 if (E < P.g_cut) { dep += E; state = L_IDLE; }
                 else state = L_STEP;
                 if (dep > 0.0f) deposit(vox, dep);
-                park();
+                park(1);
             }
             __syncwarp();
             continue;
@@ -949,7 +969,7 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
             ++n_fl;
             float gx = (x - g.ox) * g.ihx, gy = (y - g.oy) * g.ihy, gz = (z - g.oz) * g.ihz;
             if (!(gx >= 0.0f && gx < (float)g.nx && gy >= 0.0f && gy < (float)g.ny && gz >= 0.0f && gz < (float)g.nz)) {
-                s_led[kThreadsP + tid] += (double)E; state = L_IDLE; break;
+                s_esc[tid] += (double)E; state = L_IDLE; break;
             }
             vox = (int)gx + g.nx * ((int)gy + g.ny * (int)gz);
             uint2 vd = P.vox[vox];
@@ -962,15 +982,18 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
             chan = r < mc ? 0 : (r < mc + mp ? 1 : 2);
             break;
         }
-        bump(SP_FLIGHT, n_fl);
-        if (n_fi) bump(SP_FICT, n_fi);
+        {   // flights and fictitious interactions of the lanes that flew: one warp-level sum, one lane books it
+            const unsigned act = __activemask();
+            const uint32_t both = __reduce_add_sync(act, n_fl | (n_fi << 16));
+            if (lane == __ffs(act) - 1) { w_cnt[SP_FLIGHT] += both & 0xffffu; w_cnt[SP_FICT] += both >> 16; }
+        }
         if (chan == 0) state = L_HARD;  // Compton: pending
         else if (chan == 2) {           // photoelectric: absorbed locally
-            bump(SP_PE, 1u);
+            bump(SP_PE);
             deposit(vox, E);
             state = L_IDLE;
         } else if (chan == 1) {  // pair: both along the photon direction, uniform split
-            bump(SP_PAIR, 1u);
+            bump(SP_PAIR);
             QRec q; q.x = x; q.y = y; q.z = z; q.hist = rng.hist; q.vox = vox;
             uint4 a4 = next_block_rk(rng, P);
             float Tk = E - 2.0f * kMeF, us = u01f(a4.z);
@@ -982,19 +1005,16 @@ __global__ void __launch_bounds__(kThreadsP, 1) photon_kernel(const __grid_const
             emit_e(q);
             state = L_IDLE;
         }
-        park();
+        park(1);
         __syncwarp();
     }
+    __syncwarp();
     const int sid[SP_COUNT] = {S_FLIGHT, S_FICT, S_COMPTON, S_PAIR, S_PE, S_SEC_E, S_HIST, S_ATOMICS};
-#pragma unroll
-    for (int k = 0; k < SP_COUNT; ++k) {
-        unsigned long long s = warp_sum(s_cnt[k * kThreadsP + tid]);
-        if (lane == 0) stat_add(P.stats, sid[k], s);
-    }
-    double s_src = warp_sum(s_led[tid]), s_esc = warp_sum(s_led[kThreadsP + tid]);
+    if (lane < SP_COUNT) stat_add(P.stats, sid[lane], (unsigned long long)w_cnt[lane]);
+    const double s_e = warp_sum(s_esc[tid]);
     if (lane == 0) {
-        if (s_src != 0.0) atomicAdd(P.ledger + LG_SRC, s_src);
-        if (s_esc != 0.0) atomicAdd(P.ledger + LG_ESC, s_esc);
+        if (s_src[tid >> 5] != 0.0) atomicAdd(P.ledger + LG_SRC, s_src[tid >> 5]);
+        if (s_e != 0.0) atomicAdd(P.ledger + LG_ESC, s_e);
     }
     launch_epilogue(P);
 }
