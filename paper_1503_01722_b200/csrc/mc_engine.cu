@@ -52,6 +52,7 @@ struct mc_ctx {
     std::vector<char> lev_p;       // launch i was a photon kernel
     // options (M "manually adjusted")
     int64_t wave_size = 1 << 24, queue_factor = 4, blocks_per_sm = 0, refill_lanes = 32, aggregate = -1, hard_lanes = 32, adaptive = 1;
+    int64_t electron_threads = 0;  // cap on the electron kernel's CTA size (0 = the largest that fits)
     int64_t plan_ahead = 1;  // enqueue launches ahead of the counters once the secondaries-per-primary ratios are known
     int64_t hinge_overrun_pct = 25, ms_carry = 1;  // readings R8 / R8b; the oracle has the same switches
     mc_stats stats{};
@@ -207,13 +208,18 @@ using TransportKernel = void (*)(const RunParams);
 struct KernelChoice { TransportKernel fn; int threads; size_t smem; };
 // the largest CTA whose tables + pools fit (more materials or a finer grid leave less room for the pools)
 bool choose_electron_kernel(const mc_ctx* c, KernelChoice& k) {
-    const int T[4] = {1024, 768, 512, 256};
+    constexpr int n = 4;
+    const int T[n] = {1024, 768, 512, 256};
     const bool multi = c->params.flags & MC_FLAG_MULTI_VOXEL;
-    const TransportKernel fn1[4] = {electron_kernel<1024, false>, electron_kernel<768, false>, electron_kernel<512, false>, electron_kernel<256, false>};
-    const TransportKernel fnm[4] = {electron_kernel<1024, true>, electron_kernel<768, true>, electron_kernel<512, true>, electron_kernel<256, true>};
+    const TransportKernel fn1[n] = {electron_kernel<1024, false>, electron_kernel<768, false>, electron_kernel<512, false>,
+                                    electron_kernel<256, false>};
+    const TransportKernel fnm[n] = {electron_kernel<1024, true>, electron_kernel<768, true>, electron_kernel<512, true>,
+                                    electron_kernel<256, true>};
     const TransportKernel* fn = multi ? fnm : fn1;
-    for (int i = multi ? 1 : 0; i < 4; ++i)  // the multi-voxel variant needs 80 registers: 768-thread CTAs at most
-        if (smem_e(c, T[i]) <= kSmemMax) { k = KernelChoice{fn[i], T[i], smem_e(c, T[i])}; return true; }
+    // the multi-voxel variant needs 80 registers: 768-thread CTAs at most; option "electron_threads" caps the CTA size
+    const int cap = c->electron_threads > 0 ? (int)c->electron_threads : (multi ? 768 : 1024);
+    for (int i = 0; i < n; ++i)
+        if (T[i] <= cap && smem_e(c, T[i]) <= kSmemMax) { k = KernelChoice{fn[i], T[i], smem_e(c, T[i])}; return true; }
     return false;
 }
 bool choose_photon_kernel(const mc_ctx* c, KernelChoice& k) {
@@ -1024,6 +1030,7 @@ mc_status mc_set_option(mc_ctx* ctx, const char* name, int64_t value) {
     else if (n == "adaptive") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "adaptive in {0, 1}"); ctx->adaptive = value; }
     else if (n == "aggregate") { if (value < -1 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "aggregate in {-1, 0, 1}"); ctx->aggregate = value; }
     else if (n == "hinge_overrun_pct") { if (value < 0 || value > 100) return fail(ctx, MC_ERR_INVALID_ARG, "hinge_overrun_pct in [0, 100]"); ctx->hinge_overrun_pct = value; }
+    else if (n == "electron_threads") { if (value < 0 || value > 1024) return fail(ctx, MC_ERR_INVALID_ARG, "electron_threads in [0, 1024]"); ctx->electron_threads = value; }
     else if (n == "plan_ahead") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "plan_ahead in {0, 1}"); ctx->plan_ahead = value; }
     else if (n == "ms_carry") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "ms_carry in {0, 1}"); ctx->ms_carry = value; }
     else return fail(ctx, MC_ERR_INVALID_ARG, "unknown option: " + n);
