@@ -264,7 +264,7 @@ mc_status mc_set_stream(mc_ctx *ctx, void *cuda_stream);
  *                   previous run with the same kind of beam) the launches of a run are enqueued ahead — every kernel
  *                   reads the size of its input queue on the device and leaves it empty — and the host reads the
  *                   counters back only once per round of the final cascade; 0: one read-back per launch
- *   "electron_threads" cap on the electron kernel's CTA size (0 = default: the largest of 1024 / 768 / 512 / 256
+ *   "electron_threads" cap on the electron kernel's CTA size: 256, 512, 768 or 1024 (0 = default: the largest of 1024 / 768 / 512 / 256
  *                   threads whose tables and track pools fit in shared memory)
  *   "blocks_per_sm" cap on the CTAs per SM (0 = as many as fit; the transport kernels use one)
  *   "aggregate"     1: lanes of a warp that score into the same cell at the same moment combine into one

@@ -393,6 +393,7 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
     double m_new_e = have_ratio ? ctx->last_m_e : 16.0, m_new_p = have_ratio ? ctx->last_m_p : 16.0;
     // Every transport launch: the kernel reads the size of its input queue on the device, and its last CTA empties that
     // queue and the work counter, so a launch needs nothing from the host but the number of new primaries.
+    unsigned long long list_h0 = 0;  // history of d_list[0]
     size_t n_timed = 0;  // event pairs ctx->lev[2i], [2i+1] bracket the launches of this run; lev_p[i] = photon kernel
     auto issue = [&](bool run_p, uint32_t n_new, uint64_t items_hint) -> mc_status {
         P.n_new = n_new; P.h_first = h_next;
@@ -471,12 +472,12 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
                 check_particles_kernel<<<std::min<uint32_t>((n_load + kThreads - 1) / kThreads, (uint32_t)ctx->sm_count * 8), kThreads, 0, s>>>(
                     ctx->d_wave, n_load, ctx->params.e_max_MeV, ctx->d_counters + C_FLAGS);
                 CU(cudaGetLastError());
-                d_list = ctx->d_wave - h_next;  // record h of the job = entry h - h_next of the wave
+                d_list = ctx->d_wave; list_h0 = h_next;  // record h of the job = entry h - h_next of the wave
             }
             P.h_first = h_next; P.n_new = 0;
             P.q_e_out = Queue{ctx->d_q[cur], ctx->d_counters + C_E_A + cur, ctx->q_cap};
             P.q_p_out = Queue{ctx->d_q[2], ctx->d_counters + C_P, ctx->q_cap};
-            load_particles_kernel<<<std::min<uint32_t>((n_load + kThreads - 1) / kThreads, (uint32_t)ctx->sm_count * 8), kThreads, 0, s>>>(P, d_list, n_load);
+            load_particles_kernel<<<std::min<uint32_t>((n_load + kThreads - 1) / kThreads, (uint32_t)ctx->sm_count * 8), kThreads, 0, s>>>(P, d_list, list_h0, n_load);
             CU(cudaGetLastError());
             ++S.n_kernel_launches;
             if ((st = read_counters()) != MC_OK) return st;
@@ -1030,7 +1031,7 @@ mc_status mc_set_option(mc_ctx* ctx, const char* name, int64_t value) {
     else if (n == "adaptive") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "adaptive in {0, 1}"); ctx->adaptive = value; }
     else if (n == "aggregate") { if (value < -1 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "aggregate in {-1, 0, 1}"); ctx->aggregate = value; }
     else if (n == "hinge_overrun_pct") { if (value < 0 || value > 100) return fail(ctx, MC_ERR_INVALID_ARG, "hinge_overrun_pct in [0, 100]"); ctx->hinge_overrun_pct = value; }
-    else if (n == "electron_threads") { if (value < 0 || value > 1024) return fail(ctx, MC_ERR_INVALID_ARG, "electron_threads in [0, 1024]"); ctx->electron_threads = value; }
+    else if (n == "electron_threads") { if (value != 0 && value != 256 && value != 512 && value != 768 && value != 1024) return fail(ctx, MC_ERR_INVALID_ARG, "electron_threads in {0, 256, 512, 768, 1024}"); ctx->electron_threads = value; }
     else if (n == "plan_ahead") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "plan_ahead in {0, 1}"); ctx->plan_ahead = value; }
     else if (n == "ms_carry") { if (value < 0 || value > 1) return fail(ctx, MC_ERR_INVALID_ARG, "ms_carry in {0, 1}"); ctx->ms_carry = value; }
     else return fail(ctx, MC_ERR_INVALID_ARG, "unknown option: " + n);

@@ -1091,14 +1091,15 @@ __global__ void __launch_bounds__(kThreads) check_particles_kernel(const ListPar
     if ((threadIdx.x & 31) == 0 && bad) atomicOr(flags, bad);
 }
 
+// list[0] is the record of history list_h0 (0 for a whole list, the first history of the wave for a source function's buffer).
 __global__ void __launch_bounds__(kThreads) load_particles_kernel(const __grid_constant__ RunParams P, const ListParticle* __restrict__ list,
-                                                                  uint32_t n) {
+                                                                  unsigned long long list_h0, uint32_t n) {
     const Geometry& g = P.g;
     double e_src = 0.0, e_esc = 0.0;
     uint32_t n_hist = 0;
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const unsigned long long h = P.h_first + i;
-        const ListParticle p = list[h];
+        const ListParticle p = list[h - list_h0];
         const uint32_t code = p.particle == 0 ? CODE_PHOTON : (p.particle > 0 ? CODE_POSITRON : CODE_ELECTRON);
         const float e0 = p.E + (code == CODE_POSITRON ? 2.0f * kMeF : 0.0f);
         e_src += (double)e0; ++n_hist;

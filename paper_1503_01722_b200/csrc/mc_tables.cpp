@@ -191,7 +191,7 @@ double k1_transport(const Mat& m, double T) {
 // fn(i) for i in [0, n) on a few host threads (the nodes of a table are independent; the build is part of the
 // end-to-end time of a fresh context)
 template <class F> void parallel_for(int n, F fn) {
-    int nt = (int)std::min<unsigned>(std::max(1u, std::thread::hardware_concurrency()), 8u);
+    int nt = (int)std::min<unsigned>(std::max(1u, std::thread::hardware_concurrency()), 16u);
     nt = std::min(nt, std::max(1, n / 8));
     if (nt <= 1) { for (int i = 0; i < n; ++i) fn(i); return; }
     std::vector<std::thread> th;

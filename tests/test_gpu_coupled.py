@@ -364,7 +364,8 @@ def test_scheduling_options_do_not_change_the_result():
     n, B = 100000, 10
     ref = None
     for opts in ({}, {"wave_size": 8192, "queue_factor": 16}, {"refill_lanes": 1}, {"refill_lanes": 32, "blocks_per_sm": 1},
-                 {"aggregate": 1}, {"aggregate": 0}, {"hard_lanes": 8, "refill_lanes": 48}):
+                 {"aggregate": 1}, {"aggregate": 0}, {"hard_lanes": 8, "refill_lanes": 48}, {"electron_threads": 512}, {"plan_ahead": 0},
+                 {"plan_ahead": 0, "wave_size": 16384}):
         eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])
         for k, v in opts.items():
             mc.mc_set_option(eng.ctx, k, v)
