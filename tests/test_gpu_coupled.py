@@ -410,12 +410,12 @@ def test_more_materials_pick_a_smaller_cta_and_give_the_same_histories():
     eng.close()
 
 
-HIGH_STAT = [  # (config, beam, engine histories, oracle histories, block size for the oracle's statistics)
-    pytest.param(2, None, 10 ** 8, 10 ** 7, id="config2_15MeV_e_water"),
-    pytest.param(3, None, 4 * 10 ** 8, 4 * 10 ** 7, id="config3_6MV_photons_water"),
-    pytest.param(4, "e", 10 ** 8, 10 ** 7, id="config4_slab_electrons"),
-    pytest.param(4, "g", 4 * 10 ** 8, 4 * 10 ** 7, id="config4_slab_photons"),
-    pytest.param(5, "e", 10 ** 8, 4 * 10 ** 6, id="config5_halfslab_electrons"),
+HIGH_STAT = [  # (config, beam, engine histories, oracle histories): the oracle's share is ~30 s of the host cores per case
+    pytest.param(2, None, 10 ** 8, 3 * 10 ** 7, id="config2_15MeV_e_water"),
+    pytest.param(3, None, 4 * 10 ** 8, 10 ** 8, id="config3_6MV_photons_water"),
+    pytest.param(4, "e", 10 ** 8, 3 * 10 ** 7, id="config4_slab_electrons"),
+    pytest.param(4, "g", 4 * 10 ** 8, 10 ** 8, id="config4_slab_photons"),
+    pytest.param(5, "e", 10 ** 8, 10 ** 7, id="config5_halfslab_electrons"),
 ]
 
 
@@ -450,7 +450,7 @@ def test_depth_dose_profiles_and_total_energy_agree_at_high_statistics(c, beam, 
     range, energy loss, scattering or interface handling would show.
     Bars: depth curve within 0.3 % of its maximum, no noise allowance; profiles within 0.3 % of their maximum plus 4
     standard errors of the difference at that point (from the 20 batches of each side; the oracle's statistics are
-    what 30 s of the host cores buy); deposited energy fraction within 5e-4."""
+    what ~30 s of the host cores buy) and within 0.6 % with no allowance; deposited energy fraction within 5e-4."""
     cfg = W.config(c, beam) if beam else W.config(c)
     ph = cfg["phantom"]
     B = 20
@@ -477,7 +477,7 @@ def test_depth_dose_profiles_and_total_energy_agree_at_high_statistics(c, beam, 
     assert res["depth"]["max_diff"] < 3e-3, res
     for k in ("profile_1_4cm", "profile_4_7cm"):
         assert res[k]["worst_excess"] < 3e-3, (k, res)
-        assert res[k]["max_diff"] < 1e-2, (k, res)  # north_star's bar, point by point, no allowance
+        assert res[k]["max_diff"] < 6e-3, (k, res)  # point by point with no allowance (north_star's bar is 1 %)
     assert res["energy"] == pytest.approx(1.0, abs=5e-4), res
     assert res["e_frac"][0] == pytest.approx(res["e_frac"][1], abs=5e-4), res
     if c == 2:
