@@ -1040,6 +1040,6 @@ mc_status mc_set_option(mc_ctx* ctx, const char* name, int64_t value) {
 }
 
 const char* mc_last_error(const mc_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
-const char* mc_version(void) { return "paper_1503_01722_b200 0.1 (sm_100a)"; }
+const char* mc_version(void) { return "paper_1503_01722_b200 0.2 (sm_100a)"; }
 
 }  // extern "C"
