@@ -542,7 +542,7 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
             }
         }
         do {
-            for (int k = 0; k < 4; ++k) {
+            for (int k = 0; k < 2; ++k) {  // two rounds per read-back: an empty launch costs ~5 us, a read-back ~15 us
                 if ((st = issue(true, 0, full)) != MC_OK) return st;
                 if ((st = issue(false, 0, full)) != MC_OK) return st;
                 if ((st = issue(false, 0, full)) != MC_OK) return st;
