@@ -195,6 +195,16 @@ def test_goudsmit_saunderson_angle_matches_the_oracle_with_the_same_model(c, bea
     _check(out)
 
 
+def test_both_variants_together_on_the_photon_beam_through_the_slab():
+    """6 MV photons on the slab phantom with the Goudsmit-Saunderson angle AND multi-voxel steps for the secondary
+    electrons (engine at the full 1e8 histories, oracle 4e7): the two options compose."""
+    cfg = W.config(4, "g")
+    cfg["params"] = dict(cfg["params"], flags=cfg["params"]["flags"] | W.FLAG_MS_GS | W.FLAG_MULTI_VOXEL)
+    out = _run_case(cfg, cfg["n_histories"], 4 * 10 ** 7)
+    print("GS+MV 4g", out)
+    _check(out)
+
+
 def test_goudsmit_saunderson_angle_changes_the_dose_where_it_should():
     """The model is not a no-op: against the Gaussian model the lateral spread of a 6 MeV pencil beam changes (single-
     scattering tail), while the deposited energy and the energy ledger do not."""
