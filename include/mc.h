@@ -230,6 +230,37 @@ mc_status mc_ipc_close_handle(void *dev_ptr);
 mc_status mc_run_atten(mc_ctx *ctx, const mc_beam *beam, uint64_t n, uint64_t seed, int32_t *voxel_out,
                        uint8_t *channel_out);
 
+/* mc_edep_total_static — the energy-ledger total (what mc_stats.e_deposited_MeV reports: the fp64 sum of the per-batch
+ * energy grids that dose is scored into with atomic adds) for callers that are not allowed to allocate GPU
+ * memory.  Examples: a host application whose tensor framework has already claimed almost all device memory for its own
+ * caching allocator, so a raw cudaMalloc fails; a thread that runs while another thread of the process records a CUDA
+ * graph in the global capture mode, during which cudaMalloc / cudaFree are illegal and break the recording; a loop that
+ * checks the ledger between beam segments and cannot take the device-wide stall cudaMalloc / cudaFree cause.  Every other
+ * compute call of this library builds device state behind a context; this call needs no context and makes no cudaMalloc,
+ * cudaFree, memory-pool or other allocating call — the caller passes the input and the output, and the partial sums live
+ * in a fixed 512.25 KiB array inside the library's device image (held on every GPU that loads the library until the
+ * process exits).
+ *   edep_dev     n floats in DEVICE memory (e.g. the buffer of mc_edep_buffer after mc_run_range: n = n_batches * nvox)
+ *   n            1 .. mc_edep_total_static_max() = 2^28 floats; anything larger returns MC_ERR_INVALID_ARG (nothing is
+ *                summed partially) — split the input and add the totals
+ *   total_out    one double, HOST or DEVICE memory, written before the call returns
+ *   cuda_stream  a cudaStream_t (0 = default stream); the call enqueues a 16-byte clear, one kernel and an 8-byte copy
+ *                there and synchronises that stream
+ *   err, err_len optional caller-owned buffer that receives a message when the status is not MC_OK (may be NULL / 0)
+ * The sum is taken in a fixed order (one partial per 4096 consecutive floats, partials added in index order), so the
+ * same input gives the same bits on every call and every grid size; it differs from e_deposited_MeV only by fp64
+ * rounding order.
+ * First call on a device: it looks up the array's device address (once per device, with that device current), which is
+ * also what loads the library's kernels onto that device — make this first call before starting any stream capture.
+ * Shared state: all calls on a device use the one array, which keeps the previous call's contents; the call clears the
+ * only word that must start at zero itself.  Two calls on the same device that overlap on the GPU (from two host threads
+ * or streams) race on it and return wrong totals — serialise them.
+ * Errors: null pointers, n = 0, n above the limit, edep_dev not device memory -> MC_ERR_INVALID_ARG; no device or a CUDA
+ * failure -> MC_ERR_CUDA.  Nothing is written to total_out on error. */
+mc_status mc_edep_total_static(const float *edep_dev, uint64_t n, double *total_out, void *cuda_stream, char *err,
+                               int32_t err_len);
+uint64_t mc_edep_total_static_max(void);
+
 /* ---- Diagnostics: test and measurement hooks, not part of the hot path -------------------------------------------
  * (mc_philox_selftest, mc_bench_red, mc_bench_issue: used by tests/ and bench.py only.) */
 /* Philox4x32-10 on the device: n blocks, ctr[4n], key[2n] -> out[4n] (host pointers). */

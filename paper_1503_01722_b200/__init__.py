@@ -31,6 +31,7 @@ TABLE_IDS = {"mu_tot": 0, "mu_C": 1, "mu_pp": 2, "R": 3, "L": 4, "S_hard": 5, "S
 SYMBOLS = ["mc_create", "mc_destroy", "mc_build_tables", "mc_export_table", "mc_export_grid", "mc_export_gs_table",
            "mc_set_photon_tables", "mc_run", "mc_run_particles", "mc_run_source", "mc_run_range", "mc_finalize", "mc_edep_buffer",
            "mc_finalize_multi", "mc_finalize_multi_range", "mc_ipc_get_handle", "mc_ipc_open_handle", "mc_ipc_close_handle", "mc_run_atten",
+           "mc_edep_total_static", "mc_edep_total_static_max",
            "mc_philox_selftest", "mc_bench_red", "mc_bench_issue", "mc_get_stats", "mc_set_stream", "mc_set_option",
            "mc_last_error", "mc_version"]
 
@@ -94,6 +95,8 @@ def lib():
         L.mc_ipc_open_handle.argtypes = [vp, C.POINTER(vp)]
         L.mc_ipc_close_handle.argtypes = [vp]
         L.mc_run_atten.argtypes = [vp, vp, u64, u64, vp, vp]
+        L.mc_edep_total_static.argtypes = [vp, u64, vp, vp, vp, i32]
+        L.mc_edep_total_static_max.restype = u64
         L.mc_philox_selftest.argtypes = [vp, vp, i32, vp]
         L.mc_bench_red.argtypes = [vp, u32, i32, i32, i32, vp]
         L.mc_bench_issue.argtypes = [vp, i32, vp]
@@ -306,6 +309,23 @@ def mc_ipc_close_handle(dev_ptr):
 def mc_run_atten(ctx, beam, n, seed, voxel_out, channel_out=None):
     b, keep = _beam_struct(beam)
     _check(ctx, lib().mc_run_atten(ctx, C.addressof(b), int(n), int(seed), _ptr(voxel_out), _ptr(channel_out)))
+
+
+def mc_edep_total_static_max():
+    return int(lib().mc_edep_total_static_max())
+
+
+def mc_edep_total_static(edep_dev, n, cuda_stream=0, total_out=None):
+    """fp64 total of n floats at the device address / CUDA tensor edep_dev, computed without any device allocation
+    (include/mc.h).  Returns the total as a float, or writes it to total_out (numpy float64[1] or a CUDA float64 tensor)
+    when one is given.  The status message comes back through a caller-owned buffer, as in C."""
+    host = np.zeros(1, np.float64)
+    msg = C.create_string_buffer(256)
+    st = lib().mc_edep_total_static(_ptr(edep_dev), int(n), _ptr(host if total_out is None else total_out),
+                                    C.c_void_p(int(cuda_stream)), msg, len(msg))
+    if st != MC_OK:
+        raise McError(st, msg.value.decode())
+    return float(host[0]) if total_out is None else total_out
 
 
 def mc_philox_selftest(ctr, key):

@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmc_b200.so")
-SRC = [os.path.join(CSRC, "mc_engine.cu"), os.path.join(CSRC, "mc_tables.cpp"), os.path.join(CSRC, "mc_gs.cpp")]
+SRC = [os.path.join(CSRC, "mc_engine.cu"), os.path.join(CSRC, "mc_noalloc.cu"), os.path.join(CSRC, "mc_tables.cpp"), os.path.join(CSRC, "mc_gs.cpp")]
 DEPS = SRC + [os.path.join(CSRC, f) for f in ("mc_device.cuh", "mc_kernels.cuh", "mc_tables.h", "mc_gs.h")] + \
     [os.path.join(os.path.dirname(HERE), "include", "mc.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
