@@ -12,7 +12,7 @@
  * electrons and positrons by a Class II condensed-history scheme with
  * d = min[d_vox, d_maxs, d_maxe, d_event], secondaries on per-type stacks
  * (PAPER.md:60, :72), dose by atomic adds.  Readings of everything the paper leaves
- * open are listed in DESIGN.md (R1..R26).
+ * open are listed in DESIGN.md (R1..R28, with R8b and R13b).
  *
  * Conventions
  *   - Every call returns an mc_status and never throws or aborts; mc_last_error() gives a message.
@@ -182,10 +182,16 @@ mc_status mc_run_particles(mc_ctx *ctx, const mc_particle *particles, uint64_t n
  * particles from a phase-space file or write a CPU/GPU function"): the library calls
  *     fn(user, h_begin, n, out, cuda_stream)
  * once per wave of histories [h_begin, h_begin + n) (n <= option "wave_size", waves in ascending order); the function
- * writes records h_begin .. h_begin + n - 1 to out — DEVICE memory owned by the library, valid during the call — either
- * with a kernel of its own launched on cuda_stream (a cudaStream_t; work enqueued there is ordered before the
- * library's use of the records, no synchronisation needed) or with a copy from host memory, and returns 0 (anything
- * else aborts the run with MC_ERR_INVALID_ARG).  Records are validated on the device as for a device-resident list. */
+ * writes records h_begin .. h_begin + n - 1 to out — DEVICE memory owned by the library, valid during the call — and
+ * returns 0 (anything else aborts the run with MC_ERR_INVALID_ARG).  The writes must be ordered before the library's
+ * use of the records, which happens on cuda_stream (a cudaStream_t: the context's stream, see mc_set_stream).  Three
+ * ways satisfy that: (1) work enqueued on cuda_stream itself — a kernel of the function's own or cudaMemcpyAsync(...,
+ * cuda_stream) — needs no synchronisation; (2) a plain cudaMemcpy / work on the LEGACY default stream: the library makes
+ * cuda_stream wait for everything the function left on the legacy stream (this matters when mc_set_stream installed a
+ * non-blocking stream: a copy from pageable host memory may return before its DMA has landed); (3) anything else (another
+ * stream, a per-thread default stream) must be complete on the device before the function returns.  A host buffer
+ * handed to an asynchronous copy must stay valid until that copy is done.  Records are validated on the device as for a
+ * device-resident list. */
 typedef int (*mc_source_fn)(void *user, uint64_t h_begin, uint64_t n, mc_particle *out, void *cuda_stream);
 mc_status mc_run_source(mc_ctx *ctx, mc_source_fn fn, void *user, uint64_t n, uint64_t seed, int32_t n_batches,
                         float *dose_out, float *sigma_out);

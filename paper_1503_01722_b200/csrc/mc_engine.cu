@@ -48,6 +48,7 @@ struct mc_ctx {
     float *d_dose = nullptr, *d_sigma = nullptr;
     float* d_beam = nullptr;  // E nodes, pdf nodes, cdf: 3 x kMaxNodes
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t ev_src = nullptr;  // orders the context's stream after a source function's legacy-stream copies
     std::vector<cudaEvent_t> lev;  // event pairs around the transport launches of a run (read after the run's last sync)
     std::vector<char> lev_p;       // launch i was a photon kernel
     // options (M "manually adjusted")
@@ -232,8 +233,21 @@ bool choose_photon_kernel(const mc_ctx* c, KernelChoice& k) {
 
 // what the remembered secondaries-per-primary ratios belong to (mc_build_tables, mc_set_photon_tables and mc_set_option
 // forget them: cut-offs, tables and scheduling options change the ratios)
+// The key covers everything of the beam the ratios depend on: particle, shape, geometry of the field and the whole
+// spectrum (FNV-1a over the bytes; 52 bits of it, held exactly in a double; negative values mean "no beam remembered").
 double beam_key_of(const mc_ctx*, const mc_beam* b) {
-    return (double)b->particle * 1e3 + (double)b->E_nodes_MeV[b->n_nodes - 1] + 1e-3 * b->n_nodes;
+    uint64_t h = 1469598103934665603ull;
+    auto eat = [&](const void* p, size_t n) {
+        const unsigned char* c = static_cast<const unsigned char*>(p);
+        for (size_t i = 0; i < n; ++i) { h ^= c[i]; h *= 1099511628211ull; }
+    };
+    eat(&b->particle, sizeof b->particle); eat(&b->shape, sizeof b->shape);
+    eat(b->entry_cm, sizeof b->entry_cm); eat(b->axis, sizeof b->axis);
+    eat(&b->ssd_cm, sizeof b->ssd_cm); eat(b->field_cm, sizeof b->field_cm);
+    eat(&b->n_nodes, sizeof b->n_nodes);
+    eat(b->E_nodes_MeV, sizeof(float) * (size_t)b->n_nodes);
+    if (b->n_nodes > 1) eat(b->pdf_nodes, sizeof(float) * (size_t)b->n_nodes);
+    return (double)(h >> 12);
 }
 
 mc_status check_beam(mc_ctx* ctx, const mc_beam* b) {
@@ -469,6 +483,14 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
                 }
                 if (src.fn(src.user, h_next, n_load, reinterpret_cast<mc_particle*>(ctx->d_wave), (void*)s) != 0)
                     return fail(ctx, MC_ERR_INVALID_ARG, "the source function reported a failure");
+                if (s != nullptr && s != cudaStreamLegacy) {
+                    // A function that filled the wave with a plain cudaMemcpy used the legacy default stream; a copy from
+                    // pageable memory may return before its DMA has landed, and a non-blocking context stream is not
+                    // ordered after the legacy stream by itself: make it wait for whatever the function left there.
+                    if (!ctx->ev_src) CU(cudaEventCreateWithFlags(&ctx->ev_src, cudaEventDisableTiming));
+                    CU(cudaEventRecord(ctx->ev_src, cudaStreamLegacy));
+                    CU(cudaStreamWaitEvent(s, ctx->ev_src, 0));
+                }
                 check_particles_kernel<<<std::min<uint32_t>((n_load + kThreads - 1) / kThreads, (uint32_t)ctx->sm_count * 8), kThreads, 0, s>>>(
                     ctx->d_wave, n_load, ctx->params.e_max_MeV, ctx->d_counters + C_FLAGS);
                 CU(cudaGetLastError());
@@ -576,6 +598,21 @@ mc_status transport(mc_ctx* ctx, const mc_beam* beam, const ListParticle* d_list
     return MC_OK;
 }
 
+// A beam run whose launches were enqueued ahead from REMEMBERED ratios (an earlier run with the same beam) can find
+// that they admitted too much; the overflow is detected, nothing is returned, and the run is repeated once with the
+// ratios forgotten, i.e. starting with counter-driven probe launches.  An overflow of that second attempt, or of a run
+// that was counter-driven to begin with, is the caller's (queue_factor / wave_size too small) and is reported.
+mc_status transport_beam(mc_ctx* ctx, const mc_beam* beam, uint64_t n_total, uint64_t h0, uint64_t h1, uint64_t seed, int n_batches,
+                         float* d_edep) {
+    const bool from_memory = ctx->plan_ahead && ctx->adaptive && ctx->beam_key == beam_key_of(ctx, beam);
+    mc_status st = transport(ctx, beam, nullptr, n_total, h0, h1, seed, n_batches, d_edep);
+    if (st == MC_ERR_QUEUE_OVERFLOW && from_memory) {
+        cudaStreamSynchronize(ctx->stream);
+        st = transport(ctx, beam, nullptr, n_total, h0, h1, seed, n_batches, d_edep);  // beam_key was reset: probes first
+    }
+    return st;
+}
+
 mc_status check_run_args(mc_ctx* ctx, const mc_beam* beam, uint64_t n_histories, uint64_t h0, uint64_t h1, int32_t n_batches) {
     if (!ctx) return MC_ERR_INVALID_ARG;
     if (!ctx->have_tables) return fail(ctx, MC_ERR_STATE, "mc_build_tables has not been called");
@@ -648,6 +685,7 @@ void mc_destroy(mc_ctx* ctx) {
         cudaFree(ctx->d_counters); cudaFreeHost(ctx->h_counters); cudaFree(ctx->d_stats); cudaFree(ctx->d_ledger);
         cudaFree(ctx->d_edep); cudaFree(ctx->d_dose); cudaFree(ctx->d_sigma); cudaFree(ctx->d_beam);
         for (auto e : ctx->ev) if (e) cudaEventDestroy(e);
+        if (ctx->ev_src) cudaEventDestroy(ctx->ev_src);
         for (auto e : ctx->lev) cudaEventDestroy(e);
     }
     delete ctx;
@@ -742,7 +780,7 @@ mc_status mc_run_range(mc_ctx* ctx, const mc_beam* beam, uint64_t n_histories, u
     if ((st = ensure_device(ctx)) != MC_OK) return st;
     const size_t n = (size_t)n_batches * ctx->g.nvox;
     if ((st = ensure_edep(ctx, n)) != MC_OK) return st;
-    if ((st = transport(ctx, beam, nullptr, n_histories, h_begin, h_end, seed, n_batches, ctx->d_edep)) != MC_OK) return st;
+    if ((st = transport_beam(ctx, beam, n_histories, h_begin, h_end, seed, n_batches, ctx->d_edep)) != MC_OK) return st;
     if (edep_out != ctx->d_edep) CU(cudaMemcpyAsync(edep_out, ctx->d_edep, n * sizeof(float), cudaMemcpyDefault, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     return MC_OK;
@@ -833,7 +871,7 @@ mc_status mc_run(mc_ctx* ctx, const mc_beam* beam, uint64_t n_histories, uint64_
     if ((st = ensure_device(ctx)) != MC_OK) return st;
     const size_t nvox = ctx->g.nvox;
     if ((st = ensure_edep(ctx, (size_t)n_batches * nvox)) != MC_OK) return st;
-    if ((st = transport(ctx, beam, nullptr, n_histories, 0, n_histories, seed, n_batches, ctx->d_edep)) != MC_OK) return st;
+    if ((st = transport_beam(ctx, beam, n_histories, 0, n_histories, seed, n_batches, ctx->d_edep)) != MC_OK) return st;
     if ((st = finalize_device(ctx, ctx->d_edep, n_histories, n_batches)) != MC_OK) return st;
     CU(cudaMemcpyAsync(dose_out, ctx->d_dose, nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
     CU(cudaMemcpyAsync(sigma_out, ctx->d_sigma, nvox * sizeof(float), cudaMemcpyDefault, ctx->stream));
@@ -861,10 +899,11 @@ mc_status mc_run_particles(mc_ctx* ctx, const mc_particle* particles, uint64_t n
     if (!on_device) {
         for (uint64_t i = 0; i < n; ++i) {
             const mc_particle& q = particles[i];
-            if (!(q.E > 0.0f) || !std::isfinite(q.E)) return fail(ctx, MC_ERR_INVALID_ARG, "particle energies must be positive");
-            if (q.E > ctx->params.e_max_MeV) return fail(ctx, MC_ERR_ENERGY_RANGE, "particle energy above e_max_MeV");
+            // the same three checks, with the same status codes, as check_particles_kernel applies to a device list
+            if (!(q.E > 0.0f) || !(q.E <= ctx->params.e_max_MeV)) return fail(ctx, MC_ERR_ENERGY_RANGE, "particle energy not in (0, e_max_MeV]");
             const float nn = q.u * q.u + q.v * q.v + q.w * q.w;
             if (!(std::fabs(nn - 1.0f) < 1e-3f)) return fail(ctx, MC_ERR_INVALID_ARG, "particle directions must be unit vectors");
+            if (q.particle < -1 || q.particle > 1) return fail(ctx, MC_ERR_INVALID_ARG, "particle types must be -1, 0 or 1");
         }
         CU(cudaMalloc(&staged, n * sizeof(ListParticle)));
         cudaError_t e = cudaMemcpyAsync(staged, particles, n * sizeof(ListParticle), cudaMemcpyHostToDevice, ctx->stream);
@@ -876,14 +915,14 @@ mc_status mc_run_particles(mc_ctx* ctx, const mc_particle* particles, uint64_t n
     if (on_device) {
         // a device-resident list is checked where it is: one pass, one flag word back (bit 0: energy not in (0, e_max],
         // bit 1: direction not a unit vector, bit 2: unknown particle type)
-        cudaError_t e = cudaMemsetAsync(ctx->d_counters + C_DONE, 0, sizeof(uint32_t), ctx->stream);
+        cudaError_t e = cudaMemsetAsync(ctx->d_counters + C_FLAGS, 0, sizeof(uint32_t), ctx->stream);
         if (e == cudaSuccess) {
             check_particles_kernel<<<std::min<uint64_t>((n + kThreads - 1) / kThreads, (uint64_t)ctx->sm_count * 8), kThreads, 0, ctx->stream>>>(
-                d_list, (uint32_t)n, ctx->params.e_max_MeV, ctx->d_counters + C_DONE);
+                d_list, (uint32_t)n, ctx->params.e_max_MeV, ctx->d_counters + C_FLAGS);
             e = cudaGetLastError();
         }
         uint32_t bad = 0;
-        if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, ctx->d_counters + C_DONE, sizeof bad, cudaMemcpyDeviceToHost, ctx->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, ctx->d_counters + C_FLAGS, sizeof bad, cudaMemcpyDeviceToHost, ctx->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
         if (e != cudaSuccess) st = fail(ctx, MC_ERR_CUDA, cudaGetErrorString(e));
         else if (bad & 1u) st = fail(ctx, MC_ERR_ENERGY_RANGE, "particle energy not in (0, e_max_MeV]");

@@ -111,6 +111,15 @@ def test_mc_run_particles_matches_the_oracle():
     bad = p[:10].copy(); bad["u"][2] = 0.9
     with pytest.raises(mc.McError):
         mc.mc_run_particles(eng.ctx, bad, 1, 2, d, s)
+    bad = p[:10].copy(); bad["particle"][4] = 5  # an unknown type is refused, not transported as a positron
+    with pytest.raises(mc.McError) as e:
+        mc.mc_run_particles(eng.ctx, bad, 1, 2, d, s)
+    assert e.value.status == mc.MC_ERR_INVALID_ARG
+    for wrong in (0.0, -1.0, float("nan")):  # the header's code for an energy outside (0, e_max]: as for a device list
+        bad = p[:10].copy(); bad["E"][1] = wrong
+        with pytest.raises(mc.McError) as e:
+            mc.mc_run_particles(eng.ctx, bad, 1, 2, d, s)
+        assert e.value.status == mc.MC_ERR_ENERGY_RANGE
     # ... and of a device-resident list (checked by one kernel pass, same error codes)
     bad = p[:1000].copy(); bad["E"][777] = 25.0
     tb = torch.from_numpy(bad.view(np.uint8).reshape(-1)).cuda()
@@ -118,6 +127,11 @@ def test_mc_run_particles_matches_the_oracle():
         mc.mc_run_particles(eng.ctx, tb, 1, 2, d2, s2, n=len(bad))
     assert e.value.status == mc.MC_ERR_ENERGY_RANGE
     bad = p[:1000].copy(); bad["u"][5] = 0.9
+    tb = torch.from_numpy(bad.view(np.uint8).reshape(-1)).cuda()
+    with pytest.raises(mc.McError) as e:
+        mc.mc_run_particles(eng.ctx, tb, 1, 2, d2, s2, n=len(bad))
+    assert e.value.status == mc.MC_ERR_INVALID_ARG
+    bad = p[:1000].copy(); bad["particle"][999] = 5
     tb = torch.from_numpy(bad.view(np.uint8).reshape(-1)).cuda()
     with pytest.raises(mc.McError) as e:
         mc.mc_run_particles(eng.ctx, tb, 1, 2, d2, s2, n=len(bad))
@@ -168,6 +182,18 @@ def test_mc_run_source_user_gpu_and_cpu_functions_reproduce_the_list():
         assert (st["n_electron_steps"], st["n_photon_flights"], st["n_compton"]) == (st0["n_electron_steps"], st0["n_photon_flights"], st0["n_compton"])
         assert np.allclose(d, d0, rtol=1e-4, atol=1e-6 * d0.max()) and np.allclose(s, s0, rtol=5e-3, atol=1e-6 * d0.max())
     assert calls == [(0, 16384), (16384, 16384), (32768, 16384), (49152, n - 49152)]  # ascending waves of at most wave_size
+    # the same on a non-blocking context stream (torch streams are created non-blocking): a plain cudaMemcpy from pageable
+    # memory goes through the legacy stream, which such a stream does not wait for by itself — the library orders the two
+    side = torch.cuda.Stream()
+    mc.mc_set_stream(eng.ctx, side.cuda_stream)
+    for fn in (cpu_fn, gpu_fn):
+        d, s = np.zeros(eng.nvox, np.float32), np.zeros(eng.nvox, np.float32)
+        mc.mc_run_source(eng.ctx, fn, n, 3, B, d, s)
+        st = eng.stats()
+        assert (st["n_electron_steps"], st["n_photon_flights"], st["n_compton"]) == (st0["n_electron_steps"], st0["n_photon_flights"], st0["n_compton"])
+        assert np.allclose(d, d0, rtol=1e-4, atol=1e-6 * d0.max())
+    mc.mc_set_stream(eng.ctx, 0)
+    calls.clear()
     # a function that fails, and records that break the contract
     with pytest.raises(mc.McError) as e:
         mc.mc_run_source(eng.ctx, lambda *a: 7, n, 3, B, d, s)
