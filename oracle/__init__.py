@@ -222,7 +222,7 @@ class Oracle:
         out = {"first_hard": o[:, 0].astype(int), "T_first": o[:, 1], "pos": o[:, 2:5], "dir": o[:, 5:8], "path": o[:, 8],
                "steps": o[:, 9], "T_end": o[:, 10], "escaped": o[:, 11].astype(int), "path_first": o[:, 12],
                "fict_before_first": o[:, 13], "q_sampled": o[:, 14], "q_travelled": o[:, 15],
-               "annih_sum": o[:, 16:19], "annih_mu": o[:, 19]}
+               "annih_sum": o[:, 16:19], "annih_mu": o[:, 19], "brems_cos": o[:, 20], "T_brems": o[:, 21]}
         return out, dict(zip(STAT_NAMES, st))
 
     def run_particles_edep(self, particles, n_total, seed, n_batches, h0=0, h1=None):

@@ -268,7 +268,7 @@ struct Stats {  // doubles so that the Python side can read one flat array
     double max_ledger_rel;
 };
 constexpr int N_STATS = sizeof(Stats) / sizeof(double);
-constexpr int N_PROBE = 20;
+constexpr int N_PROBE = 22;
 
 struct Run {
     const Ctx& c;
@@ -650,6 +650,9 @@ struct Run {
             double kk = sample_brems(s, c.mats[c.mat[vi]], T0, P.g_cut);
             Particle g = p; g.q = 0; g.blk0 = 0; g.E = kk; g.trk_lo = id_lo; g.trk_hi = id_hi;
             rotate_dir(g.d, std::cos(MEC2 / (T0 + MEC2)), phi);
+            if (primary && probe[21] == 0) {  // instrumentation only: emission angle of the primary's first bremsstrahlung photon
+                probe[20] = p.d[0] * g.d[0] + p.d[1] * g.d[1] + p.d[2] * g.d[2]; probe[21] = T0;
+            }
             p.E = T0 - kk;
             push(g);
         }
@@ -1000,7 +1003,8 @@ int orc_n_probe() { return N_PROBE; }
 // [11] end (0 absorbed at the cut-off, 1 left the phantom), [12] path length at the first hard event,
 // [13] fictitious candidates before it, [14] sum of the scattering powers the MS angles were sampled for,
 // [15] sum of K1 rho x path actually travelled, [16..18] sum of the two annihilation-photon directions (positron),
-// [19] z direction cosine of the first annihilation photon.
+// [19] z direction cosine of the first annihilation photon, [20] cosine between the primary's direction and its first
+// bremsstrahlung photon's, [21] the primary's kinetic energy at that emission (0 = no bremsstrahlung event).
 int orc_run_probe(Ctx* c, const orc_beam* b, uint64_t h0, uint64_t h1, uint64_t n_total, uint64_t seed, double* out, double* stats_out) {
     if (!c || !c->have_tables) return 2;
     if (!b || !out || n_total >= (1ull << 32) || h1 > n_total || h0 > h1 || b->n_nodes < 1) return 1;

@@ -242,3 +242,25 @@ def test_annihilation_photons_are_isotropic_and_back_to_back():
     assert abs(pb["annih_mu"].mean()) < 4 / math.sqrt(3 * 2000)
     # the rest energy comes back: deposited = kinetic + 2 mc^2 per history with local secondaries
     assert st["e_dep"] == pytest.approx(st["e_src"], rel=1e-12)
+
+
+@pytest.mark.parametrize("T0", [1.0, 6.0, 15.0])
+def test_bremsstrahlung_photon_is_emitted_at_the_most_probable_angle(T0):
+    """PAPER.md:39: the bremsstrahlung photon's direction is "the angle with the maximum differential cross section";
+    reading R11 takes the textbook position of that maximum, theta = mc^2 / (T + mc^2) (= 1 / gamma) with T the kinetic
+    energy AT the emission, about the electron's direction of flight, and leaves the electron's direction unchanged.
+    Checked on the primary's first bremsstrahlung event of every history that has one: the angle between the two
+    directions is exactly that number (not 1 / gamma of the beam energy, not mc^2 / T, not its cosine taken twice), for
+    energies spread between the cut-off and T0; the azimuth is uniform (mean direction along the axis)."""
+    mec2 = 0.51099895
+    orc = oracle.Oracle(_one_voxel(), W.materials(1), W.params(flags=W.FLAG_LOCAL_SECONDARIES | W.FLAG_NO_MS))
+    pb, _ = orc.run_probe(W.beam(W.ELECTRON, W.PENCIL, energy=T0, entry=(0.0, 0.0, 200.0)), 20000, 3)
+    has = pb["T_brems"] > 0
+    assert has.sum() > 500
+    T, c = pb["T_brems"][has], pb["brems_cos"][has]
+    assert T.max() <= T0 and T.min() < 0.8 * T0  # emissions along the track, not only at the beam energy
+    theta = np.arccos(np.clip(c, -1.0, 1.0))
+    assert np.allclose(theta, mec2 / (T + mec2), rtol=0, atol=2e-8)  # arccos near 1 loses half the digits: 1e-16 -> 1e-8
+    # plausible mistakes are far outside that: 1/gamma of the beam energy, mc^2 / T, the angle's cosine used as the angle
+    for wrong in (mec2 / (T0 + mec2) * np.ones_like(T), mec2 / T, np.cos(mec2 / (T + mec2))):
+        assert np.max(np.abs(theta - wrong)) > 1e-3
