@@ -54,22 +54,33 @@ def parse():
     ap.add_argument("--stepping", default="voxel", choices=["voxel", "multi"], help="electron stepping: one step per voxel (PAPER.md:39) or multi-voxel steps (PAPER.md:167)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extra-configs", action="store_true", help="default run only: leave configs 3 and 5 off the line")
     ap.add_argument("--option", action="append", default=[], help="engine option name=value (mc_set_option)")
     return ap.parse_args()
 
 
-def profile_traffic(kernel):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full summary of the
-    current round (profiles/r2_<kernel>_ncu_full.txt, line 'dram_bytes_per_launch: <bytes> ...'), else null: the
-    bench does not run under ncu, so the figure can only come from the capture."""
-    p = os.path.join(ROOT, "profiles", f"r2_{kernel}_ncu_full.txt")
-    try:
-        for ln in open(p):
-            if ln.startswith("dram_bytes_per_launch:"):
-                return float(ln.split()[1]), f"profiles/r2_{kernel}_ncu_full.txt (ncu --set full, first wave of primaries of its config)"
-    except OSError:
-        pass
-    return None, "no ncu capture of this kernel committed for this round"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the one `ncu --set full` capture of each kernel (the bench does
+# not run under ncu, so the figure can only be quoted): valid for the capture's own configuration and nothing else.
+# key: (config, beam, ms_model, stepping, histories overridden, kernel) -> (bytes per launch, where it was captured)
+NCU_TRAFFIC = {
+    ("2", None, "gaussian", "voxel", False, "electron_kernel"):
+        (1847331000.0, "profiles/r2_electron_kernel_ncu_full.txt: ncu --set full of this configuration, first wave of primaries"),
+}
+
+
+def ncu_traffic(args, kernel):
+    key = (str(args.config), args.beam, args.ms_model, args.stepping, bool(args.histories), kernel)
+    if key in NCU_TRAFFIC and not args.option:
+        return NCU_TRAFFIC[key]
+    return None, "no ncu --set full capture of this kernel on this configuration"
+
+
+def queue_and_scoring_bytes(acc, steps):
+    """Algorithmic DRAM / L2 traffic of one step from the run's own counters: every queued secondary is one 48-byte record
+    written and read once, every scoring atomic one 32-byte sector update."""
+    rec = (acc["n_secondary_electrons"] + acc["n_secondary_photons"]) / steps
+    return {"queue_bytes_per_step": rec * 48 * 2, "scoring_bytes_per_step": acc["n_dose_atomics"] / steps * 32,
+            "what": "queued records x 48 B x (write + read); dose atomics x 32 B sector"}
 
 
 def peaks():
@@ -112,6 +123,12 @@ class ClockSampler:
         reasons = [n for i, n in enumerate(names) if any(len(r) >= 6 and r[2 + i] == "Active" for r in self.rows)]
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "reasons": reasons, "samples": len(sm)}
+
+
+def extras_wanted(args):
+    """The default line (BASELINE config 2, nothing overridden) also carries configs 3 and 5; --no-extra-configs drops them."""
+    return str(args.config) == "2" and not args.histories and args.ms_model == "gaussian" and args.stepping == "voxel" \
+        and not args.option and not args.no_extra_configs
 
 
 def workload(args):
@@ -197,6 +214,94 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+# ---- rooflines from the run's own counters and CUDA-event kernel times -----------------------------------
+def algorithmic_instr(acc, kernel, per):
+    if kernel == "electron_kernel":
+        return acc["n_electron_steps"] * per["e_step"] + (acc["n_moller"] + acc["n_brems"]) * per["hard_event"]
+    return acc["n_photon_flights"] * per["photon_flight"] + \
+        (acc["n_compton"] + acc["n_pair"] + acc["n_photoelectric"]) * per["photon_interaction"]
+
+
+def kernel_roofline(acc, kernel, K, total_ms, issue_peak, issue_measured, pk_kind, single_gpu=True):
+    """Issue-slot roofline of one transport kernel: algorithmic thread-instructions of the timed steps (counters x
+    SURVEY 8(d) figures) / the CUDA-event time of that kernel's launches, against the SM issue peak."""
+    kms = acc["electron_kernel_ms"] if kernel == "electron_kernel" else acc["photon_kernel_ms"]
+    achieved = algorithmic_instr(acc, kernel, INSTR_PER) / (kms * 1e-3) if kms > 0 else 0.0
+    achieved_top = algorithmic_instr(acc, kernel, INSTR_PER_TOP) / (kms * 1e-3) if kms > 0 else 0.0
+    return {"bound": "alu", "kernel": kernel, "achieved": achieved / 1e12, "peak": issue_peak / 1e12,
+            "unit": "Tinstr/s (thread-instructions)", "frac": achieved / issue_peak,
+            "instr_per_unit": INSTR_PER, "frac_top_of_range": achieved_top / issue_peak, "instr_per_unit_top_of_range": INSTR_PER_TOP,
+            "headline": "frac (SURVEY 8(d) ceiling figures: 225 thread-instructions per e- step, 75 per photon flight)",
+            "peak_source": f"148 SM x 4 schedulers x 32 lanes x sm_max_mhz ({pk_kind} MEASURED_PEAKS.json clock)",
+            "peak_measured": issue_measured / 1e12, "frac_of_measured": achieved / issue_measured,
+            "peak_measured_source": "mc_bench_issue: 2 x 1024-thread CTAs per SM, 8 independent FFMA chains per thread, best of 3",
+            "kernel_ms_per_step": kms / K, "kernel_share_of_step": kms / total_ms if single_gpu else None}
+
+
+def measure_extra_config(mc, torch, stream, flush, name, beam, steps, warmup, issue_peak, issue_measured, pk_kind, red_peak):
+    """One more BASELINE config on the same line (north_star quotes the metric for a photon AND an electron beam): the same
+    timed region as the headline (L2 flush between steps, CUDA events on the engine's stream), the same rooflines, and e2e
+    through mc_run with host buffers.  Single GPU only."""
+    a = argparse.Namespace(config=name, beam=beam, histories=0, ms_model="gaussian", stepping="voxel", option=[])
+    cfg = workload(a)
+    n, B, seed = cfg["n_histories"], cfg["n_batches"], cfg["seed"]
+    eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])
+    mc.mc_set_stream(eng.ctx, stream.cuda_stream)
+    dose = torch.empty(eng.nvox, dtype=torch.float32, device="cuda")
+    sigma = torch.empty_like(dose)
+    acc = {}
+    with torch.cuda.stream(stream):
+        for _ in range(warmup):
+            flush.fill_(1)
+            mc.mc_run(eng.ctx, cfg["beam"], n, seed, B, dose, sigma)
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for i in range(steps):
+            flush.fill_(1)
+            ev[i][0].record(stream)
+            mc.mc_run(eng.ctx, cfg["beam"], n, seed, B, dose, sigma)
+            ev[i][1].record(stream)
+            for k, v in mc.mc_get_stats(eng.ctx).items():
+                acc[k] = acc.get(k, 0) + v
+        torch.cuda.synchronize()
+        total_ms = sum(x.elapsed_time(y) for x, y in ev)
+        # e2e: host buffers in and out, wall clock around the calls
+        h_dose, h_sigma = np.zeros(eng.nvox, np.float32), np.zeros(eng.nvox, np.float32)
+        mc.mc_run(eng.ctx, cfg["beam"], n, seed, B, h_dose, h_sigma)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            mc.mc_run(eng.ctx, cfg["beam"], n, seed, B, h_dose, h_sigma)
+        torch.cuda.synchronize()
+        t_e2e = time.perf_counter() - t0
+    e_ms, p_ms = acc["electron_kernel_ms"], acc["photon_kernel_ms"]
+    dom, other = ("electron_kernel", "photon_kernel") if e_ms >= p_ms else ("photon_kernel", "electron_kernel")
+    d, sg = dose.cpu().numpy().astype(np.float64), sigma.cpu().numpy().astype(np.float64)
+    m = d >= 0.1 * d.max()
+    rel = float(np.mean(sg[m] / d[m]))
+    red_rate = acc["n_dose_atomics"] / ((e_ms + p_ms) * 1e-3)
+    out = {"config": config_dict(cfg, a), "steps": steps, "warmup": warmup, "ms_per_step": total_ms / steps,
+           "value": n * steps / (total_ms * 1e-3), "unit": "histories/s",
+           "e_steps_per_s": acc["n_electron_steps"] / (total_ms * 1e-3),
+           "photon_flights_per_s": acc["n_photon_flights"] / (total_ms * 1e-3),
+           "gpu_launches": int(acc["n_kernel_launches"]),
+           "ledger_rel": abs(acc["e_deposited_MeV"] + acc["e_escaped_MeV"] - acc["e_source_MeV"]) / acc["e_source_MeV"],
+           "roofline": dict(kernel_roofline(acc, dom, steps, total_ms, issue_peak, issue_measured, pk_kind),
+                            traffic=None, traffic_source="no ncu --set full capture of this kernel on this configuration",
+                            traffic_algorithmic=queue_and_scoring_bytes(acc, steps)),
+           "roofline_scoring": {"bound": "l2_atomic", "achieved": red_rate / 1e9, "peak": red_peak / 1e9, "unit": "Gred/s",
+                                "frac": red_rate / red_peak},
+           "mean_rel_sigma_10pct_isodose": rel, "time_to_1pct_s": (total_ms / steps * 1e-3) * (rel / 0.01) ** 2,
+           "e2e": {"value": n * steps / t_e2e, "unit": "histories/s", "h2d_bytes_per_step": int(3 * 4096 * 4),
+                   "d2h_bytes_per_step": int(2 * eng.nvox * 4 + 5 * 4 + 12 * 8 + 3 * 8),
+                   "what": "mc_run(beam from host, dose + sigma to host memory) per step on a resident context"}}
+    other_ms = p_ms if other == "photon_kernel" else e_ms
+    if other_ms > 0.25 * total_ms:
+        out["roofline_" + other.split("_")[0]] = kernel_roofline(acc, other, steps, total_ms, issue_peak, issue_measured, pk_kind)
+    eng.close()
+    return out
+
+
 # ---- the CUDA engine ---------------------------------------------------------------------------------
 def run_engine(args):
     import torch
@@ -205,6 +310,8 @@ def run_engine(args):
 
     rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:  # the line's n_gpus is the number of ranks that ran: refuse to print anything else
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but the launcher started WORLD_SIZE={world} ranks")
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the engine has no CPU path)")
     # one rank per GPU; MC_BENCH_BACKEND=gloo lets the N > 1 code path be exercised on a box with fewer GPUs than
@@ -248,7 +355,9 @@ def run_engine(args):
                 dist.all_gather_object(handles, mc.mc_ipc_get_handle(own))
                 if os.environ.get("MC_BENCH_FAIL_PEER_RANK") == str(rank):  # fault injection for the fallback test
                     raise RuntimeError("injected peer-mapping failure")
-                peers = [own if r == rank else mc.mc_ipc_open_handle(handles[r]) for r in range(world)]
+                peers = [None] * world  # filled one by one: what was opened before a failure is closed on fallback
+                for r in range(world):
+                    peers[r] = own if r == rank else mc.mc_ipc_open_handle(handles[r])
             except Exception as exc:  # noqa: BLE001  (any failure -> every rank falls back together)
                 print(f"rank {rank}: peer mapping failed ({exc}); falling back to all-reduce", file=sys.stderr)
                 ok = False
@@ -385,26 +494,15 @@ def run_engine(args):
     issue_measured = max(mc.mc_bench_issue(eng.ctx, 4096) for _ in range(3))  # FFMA micro-benchmark on this GPU
     e_ms, p_ms = acc["electron_kernel_ms"], acc["photon_kernel_ms"]
     dom = "electron_kernel" if e_ms >= p_ms else "photon_kernel"
-    kms = e_ms if dom == "electron_kernel" else p_ms
 
-    def algorithmic(per):
-        if dom == "electron_kernel":
-            return acc["n_electron_steps"] * per["e_step"] + (acc["n_moller"] + acc["n_brems"]) * per["hard_event"]
-        return acc["n_photon_flights"] * per["photon_flight"] + \
-            (acc["n_compton"] + acc["n_pair"] + acc["n_photoelectric"]) * per["photon_interaction"]
-
-    achieved = algorithmic(INSTR_PER) / (kms * 1e-3) if kms > 0 else 0.0
-    achieved_top = algorithmic(INSTR_PER_TOP) / (kms * 1e-3) if kms > 0 else 0.0
-    traffic, traffic_src = profile_traffic(dom)
-    roofline = {"bound": "alu", "kernel": dom, "achieved": achieved / 1e12, "peak": issue_peak / 1e12,
-                "unit": "Tinstr/s (thread-instructions)", "frac": achieved / issue_peak,
-                "instr_per_unit": INSTR_PER, "frac_top_of_range": achieved_top / issue_peak, "instr_per_unit_top_of_range": INSTR_PER_TOP,
-                "headline": "frac (SURVEY 8(d) ceiling figures: 225 thread-instructions per e- step)",
-                "traffic": traffic, "traffic_unit": "bytes per launch", "traffic_source": traffic_src,
-                "peak_source": f"148 SM x 4 schedulers x 32 lanes x sm_max_mhz ({pk_kind} MEASURED_PEAKS.json clock)",
-                "peak_measured": issue_measured / 1e12, "frac_of_measured": achieved / issue_measured,
-                "peak_measured_source": "mc_bench_issue: 2 x 1024-thread CTAs per SM, 8 independent FFMA chains per thread, best of 3",
-                "kernel_ms_per_step": kms / K, "kernel_share_of_step": kms / total_ms if world == 1 else None}
+    traffic, traffic_src = ncu_traffic(args, dom)
+    roofline = dict(kernel_roofline(acc, dom, K, total_ms, issue_peak, issue_measured, pk_kind, world == 1),
+                    traffic=traffic, traffic_unit="bytes per launch", traffic_source=traffic_src,
+                    traffic_algorithmic=queue_and_scoring_bytes(acc, K))
+    other = "photon_kernel" if dom == "electron_kernel" else "electron_kernel"
+    other_ms = p_ms if dom == "electron_kernel" else e_ms
+    roofline_other = kernel_roofline(acc, other, K, total_ms, issue_peak, issue_measured, pk_kind, world == 1) \
+        if other_ms > 0.25 * total_ms else None
     # scoring roofline: red.global.add.f32 peak, best over occupancy (1, 2, 4, 8 CTAs of 256 threads per SM) on windows
     # the size of one batch grid of configs 2-4 (0.9 MB) and of config 5 (7.1 MB), random cells (no intra-warp
     # collisions on average), >= 2 ms per launch; mode 1 (one cell per warp) beside it
@@ -445,12 +543,20 @@ def run_engine(args):
                "ledger_rel": abs(acc["e_deposited_MeV"] + acc["e_escaped_MeV"] - acc["e_source_MeV"]) / acc["e_source_MeV"],
                "clocks": clocks, "e2e": e2e, "gpu_launches": int(acc["n_kernel_launches"]),
                "roofline": roofline, "roofline_scoring": roofline_scoring}
+        if roofline_other is not None:  # the second kernel where it is more than a quarter of the step
+            out["roofline_" + other.split("_")[0]] = roofline_other
         # statistics of the result: mean sigma/D inside the 10 % isodose and time to 1 %
         d, s = dose.cpu().numpy().astype(np.float64), sigma.cpu().numpy().astype(np.float64)
         m = d >= 0.1 * d.max()
         rel = float(np.mean(s[m] / d[m]))
         out["mean_rel_sigma_10pct_isodose"] = rel
         out["time_to_1pct_s"] = (total_ms / K * 1e-3) * (rel / 0.01) ** 2
+        if world == 1 and extras_wanted(args):
+            # north_star names a 6 MV photon and a 15 MeV electron beam on water, and the heterogeneous phantom: configs 3
+            # and 5 (electron beam) ride on the same line, measured like the headline (3 timed steps each)
+            eng.close()  # its queues go back to the library's pool and are reused by the next contexts
+            out["configs"] = [measure_extra_config(mc, torch, stream, flush, c, b, 3, 3, issue_peak, issue_measured, pk_kind, red_peak)
+                              for c, b in (("3", None), ("5", "e"))]
         if world == 1 and not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(cfg)
         print(json.dumps(out))
@@ -464,9 +570,25 @@ def run_engine(args):
         dist.destroy_process_group()
 
 
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` without a launcher: start the N ranks here (one process per GPU, the same command line the
+    driver uses for N > 1) and become that launcher.  NCCL's own environment (NCCL_DEBUG, ...) is passed through untouched."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    os.execv(sys.executable, cmd)
+
+
 if __name__ == "__main__":
     a = parse()
+    if a.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
     if a.impl == "reference":
         run_reference(a)
     else:
+        if a.gpus > 1 and "WORLD_SIZE" not in os.environ:
+            respawn_under_torchrun(a)
         run_engine(a)

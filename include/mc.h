@@ -268,9 +268,13 @@ mc_status mc_edep_total_static(const float *edep_dev, uint64_t n, double *total_
 uint64_t mc_edep_total_static_max(void);
 
 /* ---- Diagnostics: test and measurement hooks, not part of the hot path -------------------------------------------
- * (mc_philox_selftest, mc_bench_red, mc_bench_issue: used by tests/ and bench.py only.) */
+ * (mc_philox_selftest, mc_u01_selftest, mc_bench_red, mc_bench_issue: used by tests/ and bench.py only.) */
 /* Philox4x32-10 on the device: n blocks, ctr[4n], key[2n] -> out[4n] (host pointers). */
 mc_status mc_philox_selftest(const uint32_t *ctr, const uint32_t *key, int32_t n, uint32_t *out);
+
+/* mc_u01_selftest — the device's uniform-from-word function (two instructions, no integer-to-float conversion) against
+ * its definition ((w >> 9) + 0.5) * 2^-23 (R15) for all 2^23 values: *n_mismatch (host) = words that differ. */
+mc_status mc_u01_selftest(uint64_t *n_mismatch);
 
 /* mc_bench_red — measures the scoring roofline: `blocks` x 256 threads each
  * issue per_thread red.global.add.f32 into a window of n_cells floats.  mode 0: pseudo-random cell per
@@ -284,6 +288,13 @@ mc_status mc_bench_red(mc_ctx *ctx, uint32_t n_cells, int32_t per_thread, int32_
 mc_status mc_bench_issue(mc_ctx *ctx, int32_t iters, double *thread_instr_per_s);
 
 /* ---- end of diagnostics ------------------------------------------------------------------------------------------- */
+
+/* mc_trim — the particle queues (gigabytes) come from a memory pool the library keeps per device so that the next
+ * context of the process reuses them; mc_destroy returns them to that pool, not to the driver, and memory in a private
+ * pool is invisible to every other allocator of the process.  mc_trim hands the unused part of the current device's pool
+ * back to the driver, keeping at most keep_bytes (0 = everything unused).  It synchronises the device.  Queues of live
+ * contexts are not touched. */
+mc_status mc_trim(uint64_t keep_bytes);
 
 mc_status mc_get_stats(const mc_ctx *ctx, mc_stats *out);
 /* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); 0 = default stream. */

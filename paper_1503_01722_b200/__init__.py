@@ -32,7 +32,7 @@ SYMBOLS = ["mc_create", "mc_destroy", "mc_build_tables", "mc_export_table", "mc_
            "mc_set_photon_tables", "mc_run", "mc_run_particles", "mc_run_source", "mc_run_range", "mc_finalize", "mc_edep_buffer",
            "mc_finalize_multi", "mc_finalize_multi_range", "mc_ipc_get_handle", "mc_ipc_open_handle", "mc_ipc_close_handle", "mc_run_atten",
            "mc_edep_total_static", "mc_edep_total_static_max",
-           "mc_philox_selftest", "mc_bench_red", "mc_bench_issue", "mc_get_stats", "mc_set_stream", "mc_set_option",
+           "mc_philox_selftest", "mc_u01_selftest", "mc_bench_red", "mc_bench_issue", "mc_trim", "mc_get_stats", "mc_set_stream", "mc_set_option",
            "mc_last_error", "mc_version"]
 
 
@@ -100,6 +100,7 @@ def lib():
         L.mc_philox_selftest.argtypes = [vp, vp, i32, vp]
         L.mc_bench_red.argtypes = [vp, u32, i32, i32, i32, vp]
         L.mc_bench_issue.argtypes = [vp, i32, vp]
+        L.mc_trim.argtypes = [u64]
         L.mc_get_stats.argtypes = [vp, vp]
         L.mc_set_stream.argtypes = [vp, vp]
         L.mc_set_option.argtypes = [vp, C.c_char_p, C.c_int64]
@@ -336,6 +337,12 @@ def mc_philox_selftest(ctr, key):
     return out
 
 
+def mc_u01_selftest():
+    n = C.c_uint64()
+    _check(None, lib().mc_u01_selftest(C.byref(n)))
+    return int(n.value)
+
+
 def mc_bench_red(ctx, n_cells, per_thread, mode, blocks):
     ms = C.c_double()
     _check(ctx, lib().mc_bench_red(ctx, int(n_cells), int(per_thread), int(mode), int(blocks), C.addressof(ms)))
@@ -346,6 +353,10 @@ def mc_bench_issue(ctx, iters=4096):
     r = C.c_double()
     _check(ctx, lib().mc_bench_issue(ctx, int(iters), C.addressof(r)))
     return r.value
+
+
+def mc_trim(keep_bytes=0):
+    _check(None, lib().mc_trim(int(keep_bytes)))
 
 
 def mc_get_stats(ctx):

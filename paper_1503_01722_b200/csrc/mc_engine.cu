@@ -680,6 +680,9 @@ mc_status mc_create(const uint8_t* material_idx, const float* density_gcc, const
 void mc_destroy(mc_ctx* ctx) {
     if (!ctx) return;
     if (ctx->dev_ready) {
+        // every call synchronises the context's stream before it returns, except on some error paths: wait here so that
+        // nothing the context enqueued still uses the buffers (the stream may be gone already: then there is nothing to wait for)
+        if (cudaStreamSynchronize(ctx->stream) != cudaSuccess) cudaGetLastError();
         cudaFree(ctx->d_vox); cudaFree(ctx->d_tabP); cudaFree(ctx->d_tabE); cudaFree(ctx->d_gs); cudaFree(ctx->d_wave);
         for (auto q : ctx->d_q) if (q) cudaFreeAsync(q, nullptr);  // back to the pool (see transport())
         cudaFree(ctx->d_counters); cudaFreeHost(ctx->h_counters); cudaFree(ctx->d_stats); cudaFree(ctx->d_ledger);
@@ -1010,6 +1013,23 @@ mc_status mc_philox_selftest(const uint32_t* ctr, const uint32_t* key, int32_t n
     return MC_OK;
 }
 
+mc_status mc_u01_selftest(uint64_t* n_mismatch) {
+    if (!n_mismatch) return MC_ERR_INVALID_ARG;
+    unsigned long long* d = nullptr;
+    cudaError_t e = cudaMalloc(&d, sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(d, 0, sizeof(unsigned long long));
+    if (e == cudaSuccess) {
+        u01_test_kernel<<<148 * 8, 256>>>(d);
+        e = cudaGetLastError();
+    }
+    unsigned long long h = ~0ull;
+    if (e == cudaSuccess) e = cudaMemcpy(&h, d, sizeof h, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) { cudaGetLastError(); return MC_ERR_CUDA; }
+    *n_mismatch = h;
+    return MC_OK;
+}
+
 mc_status mc_bench_red(mc_ctx* ctx, uint32_t n_cells, int32_t per_thread, int32_t mode, int32_t blocks, double* ms_out) {
     if (!ctx || !ms_out || n_cells == 0 || per_thread <= 0 || blocks <= 0 || mode < 0 || mode > 1) return MC_ERR_INVALID_ARG;
     mc_status st;
@@ -1044,6 +1064,16 @@ mc_status mc_bench_issue(mc_ctx* ctx, int32_t iters, double* thread_instr_per_s)
     if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, ctx->ev[2], ctx->ev[3]);
     if (e != cudaSuccess || !(ms > 0)) return fail(ctx, MC_ERR_CUDA, std::string("mc_bench_issue: ") + cudaGetErrorString(e));
     *thread_instr_per_s = (double)blocks * 1024.0 * (double)iters * 64.0 / (ms * 1e-3);
+    return MC_OK;
+}
+
+mc_status mc_trim(uint64_t keep_bytes) {
+    int n = 0;
+    if (cudaGetDeviceCount(&n) != cudaSuccess || n <= 0) { cudaGetLastError(); return MC_ERR_CUDA; }
+    cudaMemPool_t pool = queue_pool();
+    if (!pool) return MC_ERR_CUDA;
+    // queues go back to the pool with cudaFreeAsync: they count as unused once that has executed
+    if (cudaDeviceSynchronize() != cudaSuccess || cudaMemPoolTrimTo(pool, (size_t)keep_bytes) != cudaSuccess) { cudaGetLastError(); return MC_ERR_CUDA; }
     return MC_OK;
 }
 

@@ -1196,6 +1196,19 @@ __global__ void philox_test_kernel(const uint32_t* ctr, const uint32_t* key, int
     out[4 * i] = r.x; out[4 * i + 1] = r.y; out[4 * i + 2] = r.z; out[4 * i + 3] = r.w;
 }
 
+// u01f against its defining expression ((w >> 9) + 0.5) * 2^-23 for every 23-bit value, with the 9 discarded bits all
+// zero and all one: counts the words whose results differ in any bit.
+__global__ void u01_test_kernel(unsigned long long* mismatches) {
+    unsigned int bad = 0;
+    for (uint32_t m = blockIdx.x * blockDim.x + threadIdx.x; m < (1u << 23); m += gridDim.x * blockDim.x)
+        for (uint32_t low = 0; low < 2; ++low) {
+            const uint32_t w = (m << 9) | (low ? 0x1ffu : 0u);
+            const float ref = __fmaf_rn(__uint2float_rn(w >> 9), 1.1920928955078125e-07f, 5.9604644775390625e-08f);
+            if (__float_as_uint(u01f(w)) != __float_as_uint(ref) || __float_as_uint(u01(w)) != __float_as_uint(ref)) ++bad;
+        }
+    if (bad) atomicAdd(mismatches, (unsigned long long)bad);
+}
+
 // L2 reduction micro-benchmark (scoring roofline): every thread issues `per_thread`
 // red.global.add.f32 to pseudo-random cells of a window of `n_cells` floats (mode 0), or all lanes of a
 // warp to one cell (mode 1).

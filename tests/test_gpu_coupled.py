@@ -9,6 +9,9 @@ The oracle runs once per case (seed 1, 40 batches: R19).  The engine runs twice:
            applied strictly (a physics difference shows as a bias);
   seed 2 — independent streams: the 3-sigma criterion proper; the mean |difference| bar is then
            1 % + E|noise| = 1 % + 0.8 * mean(sigma_comb)/Dmax (half-normal mean), stated here once.
+           Where the oracle is thin (photon configs 3, 4g, 5g: mean combined sigma 2-3 % of Dmax per voxel) that
+           allowance makes the seed-2 bar about 3 %: those configs are carried by the seed-1 run (strict 1 %, measured
+           2e-5 .. 1e-3) and by the integrated curves of the high-statistics test below (0.3 %), not by seed 2.
 Event counters per history (flights, fictitious, Compton, pair, photoelectric, Moller, brems) must agree within 1 %
 and the energy ledger of every engine run must close.
 """
@@ -95,12 +98,19 @@ def _engine_run(eng, cfg, n, seed, coarse):
     return dg, sg, st
 
 
-def _run_case(cfg, n_gpu, n_orc, coarse=1):
+ORACLE_SWITCH = {"hinge_overrun_pct": ("hinge_overrun", 0.01), "ms_carry": ("ms_carry", 1.0)}  # engine option -> oracle's
+
+
+def _run_case(cfg, n_gpu, n_orc, coarse=1, options=None):
     """Oracle: n_orc histories, seed 1.  Engine: seed 1 with n_orc histories (same streams, same batches up to
-    the batch count) and seed 2 with n_gpu histories (independent, the size bench.py times)."""
+    the batch count) and seed 2 with n_gpu histories (independent, the size bench.py times).
+    options: switches of the readings R8 / R8b set on BOTH sides (engine option name -> value)."""
     ph = cfg["phantom"]
     eng = mc.Engine(ph, cfg["materials"], cfg["params"])
     orc = oracle.Oracle(ph, cfg["materials"], cfg["params"])
+    for k, v in (options or {}).items():
+        mc.mc_set_option(eng.ctx, k, v)
+        orc.set_option(ORACLE_SWITCH[k][0], v * ORACLE_SWITCH[k][1])
     eo, sto = orc.run_edep_parallel(cfg["beam"], n_orc, 1, B_ORC, WORKERS)
     assert sto["max_ledger_rel"] < 1e-5
     if coarse == 1:
@@ -173,16 +183,35 @@ def test_config4_slab_photons_full_size_engine():
     _check(_run_case(cfg, cfg["n_histories"], 4 * 10 ** 7))
 
 
-def test_config5_halfslab_electrons_full_size_engine_coarse_blocks():
-    """122x122x120 at 0.25 cm, 1e8 electron histories on the engine; the oracle affords 4e6, so the dose is
-    compared on 4x4x4 voxel blocks (1 cm^3), where its noise is below the 1 % bar."""
+def test_config5_halfslab_electrons_full_size_engine_per_voxel():
+    """122x122x120 at 0.25 cm (the half-slab of Fig. 3), 1e8 electron histories on the engine; the oracle
+    runs 3e7 (about a minute of the host cores), which brings its per-voxel sigma inside the 10 % isodose to ~1 % of Dmax:
+    north_star's criterion voxel by voxel, no block sums."""
     cfg = W.config(5, "e")
-    _check(_run_case(cfg, cfg["n_histories"], 4 * 10 ** 6, coarse=4))
+    out = _run_case(cfg, cfg["n_histories"], 3 * 10 ** 7)
+    print("config 5 e-", out)
+    _check(out)
 
 
-def test_config5_halfslab_photons_full_size_engine_coarse_blocks():
+def test_config5_halfslab_photons_full_size_engine_per_voxel():
     cfg = W.config(5, "g")
-    _check(_run_case(cfg, cfg["n_histories"], 4 * 10 ** 7, coarse=4))
+    out = _run_case(cfg, cfg["n_histories"], 3 * 10 ** 8)
+    print("config 5 photons", out)
+    _check(out)
+
+
+# ---- the literal readings of the step rule (PAPER.md:39 d = min[d_vox, ...], :167; DESIGN.md R8, R8b) -------------------
+@pytest.mark.parametrize("c,beam", [(2, None), (4, "e")])
+@pytest.mark.parametrize("options", [{"hinge_overrun_pct": 0}, {"ms_carry": 0}], ids=["no_hinge_overrun", "no_ms_carry"])
+def test_literal_step_rule_and_uncarried_ms_match_the_oracle_with_the_same_switch(c, beam, options):
+    """The defaults of R8 (a voxel-limited step may run on to the face by 25 % of its second leg) and R8b (scattering power
+    travelled but not sampled for is carried) are readings; the plain rule d = min[d_vox, d_maxs, d_maxe, d_event] with no
+    overrun, and the planned-path-only MS angle, are run here on both sides with the same switch and must agree to the
+    same bars as the defaults."""
+    cfg = W.config(c, beam) if beam else W.config(c)
+    out = _run_case(cfg, cfg["n_histories"], cfg["n_histories"], options=options)
+    print("literal readings", c, beam, options, {k: out[k] for k in (1, 2)})
+    _check(out)
 
 
 # ---- Goudsmit-Saunderson multiple-scattering angle (SURVEY 8(f)1; PAPER.md:39; DESIGN.md R27) -------------------
@@ -426,6 +455,7 @@ HIGH_STAT = [  # (config, beam, engine histories, oracle histories): the oracle'
     pytest.param(4, "e", 10 ** 8, 3 * 10 ** 7, id="config4_slab_electrons"),
     pytest.param(4, "g", 4 * 10 ** 8, 10 ** 8, id="config4_slab_photons"),
     pytest.param(5, "e", 10 ** 8, 10 ** 7, id="config5_halfslab_electrons"),
+    pytest.param(5, "g", 4 * 10 ** 8, 10 ** 8, id="config5_halfslab_photons"),
 ]
 
 
@@ -495,3 +525,21 @@ def test_depth_dose_profiles_and_total_energy_agree_at_high_statistics(c, beam, 
         # zero") is bremsstrahlung tail only
         zg = cg["depth"][0]
         assert zg[int(10.0 / 0.5):].max() < 0.02 * zg.max()
+
+
+def test_mc_trim_hands_the_queue_pool_back_to_the_driver():
+    """Queues of a destroyed context stay in the library's pool (reused by the next context); mc_trim releases them."""
+    import torch
+    cfg = W.config(1)
+    eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])
+    eng.run(cfg["beam"], 400000, 1, 4)  # three queues of 4 x 400000 records x 48 B = 230 MB
+    eng.close()
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    mc.mc_trim(0)
+    free1 = torch.cuda.mem_get_info()[0]
+    assert free1 - free0 >= 200e6, (free0, free1)
+    eng = mc.Engine(cfg["phantom"], cfg["materials"], cfg["params"])  # and a new context simply allocates again
+    d, _ = eng.run(cfg["beam"], 20000, 1, 4)
+    assert d.max() > 0 and _ledger(eng.stats()) < 1e-4
+    eng.close()

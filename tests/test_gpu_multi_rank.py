@@ -129,3 +129,23 @@ def test_bench_two_ranks_on_one_gpu_peer_exchange_and_joint_fallback(fail_rank):
     assert ("one voxel slice per rank" in par) == (fail_rank == ""), par
     # the statistics do not depend on the exchange: same job, same seed
     assert line["mean_rel_sigma_10pct_isodose"] == pytest.approx(0.006, rel=0.25)
+
+
+def test_bench_gpus_2_without_a_launcher_starts_two_ranks():
+    """A plain `python bench.py --gpus 2` (no torchrun around it) must start the two ranks itself and print n_gpus = 2; a
+    launcher that started another number of ranks than --gpus says is refused."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    env["MC_BENCH_BACKEND"] = "gloo"
+    cmd = [sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--config", "1", "--steps", "2", "--warmup", "3",
+           "--no-cpu-baseline", "--no-e2e"]
+    out = subprocess.run(cmd, env=env, capture_output=True, text=True, timeout=600, cwd=root)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
+    assert line["n_gpus"] == 2 and line["ledger_rel"] < 1e-4 and "x2" in line["config"]["parallelism"]
+    out = subprocess.run(cmd[:2] + ["--gpus", "3"] + cmd[4:], env=dict(env, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0"),
+                         capture_output=True, text=True, timeout=600, cwd=root)
+    assert out.returncode != 0 and "WORLD_SIZE=1" in (out.stderr + out.stdout)

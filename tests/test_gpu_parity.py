@@ -144,3 +144,9 @@ def test_roofline_micro_benchmarks_report_plausible_peaks():
     ms_hot = mc.mc_bench_red(eng.ctx, 223260, 64, 1, 148 * 8)
     assert ms_hot > 0
     eng.close()
+
+
+def test_uniform_from_word_is_bit_identical_to_its_definition_for_all_values():
+    """u = ((w >> 9) + 0.5) 2^-23 (R15) is computed on the device as bits-under-the-exponent minus (1 - 2^-24): exhaustive over
+    the 2^23 values (x two settings of the discarded bits), so the oracle's plain expression and the kernel's agree bit for bit."""
+    assert mc.mc_u01_selftest() == 0
