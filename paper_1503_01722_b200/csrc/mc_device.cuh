@@ -139,8 +139,11 @@ __device__ __forceinline__ uint4 next_block_rk(Rng& r, const RunParams& P) {
 // u = ((w >> 9) + 0.5) * 2^-23 in (0, 1): exact in fp32
 __device__ __forceinline__ float u01(uint32_t w) { return __fmul_rn(__fadd_rn((float)(w >> 9), 0.5f), 1.1920928955078125e-07f); }
 
-// same value as u01 (both exact in fp32), one FFMA
-__device__ __forceinline__ float u01f(uint32_t w) { return fmaf((float)(w >> 9), 1.1920928955078125e-07f, 5.9604644775390625e-08f); }
+// Same value as u01, without the integer-to-float conversion (a quarter-rate XU instruction): one funnel shift puts the 23
+// bits under the exponent of 1.0, f = 1 + m 2^-23 in [1, 2), and f - (1 - 2^-24) = (2m + 1) 2^-24 is exact in fp32 (both
+// operands and the result are representable, so the subtraction rounds nothing).  Checked for all 2^23 values on the
+// device by mc_u01_selftest.
+__device__ __forceinline__ float u01f(uint32_t w) { return __fsub_rn(__uint_as_float(__funnelshift_r(w, 0x7fu, 9)), 0.99999994f); }
 
 // ---- fp32 arithmetic contract (R20) -----------------------------------------------------------
 __device__ __forceinline__ float c_ln(float x) {
