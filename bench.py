@@ -64,7 +64,7 @@ def parse():
 # key: (config, beam, ms_model, stepping, histories overridden, kernel) -> (bytes per launch, where it was captured)
 NCU_TRAFFIC = {
     ("2", None, "gaussian", "voxel", False, "electron_kernel"):
-        (1847331000.0, "profiles/r2_electron_kernel_ncu_full.txt: ncu --set full of this configuration, first wave of primaries"),
+        (1848283000.0, "profiles/r3_electron_kernel_ncu_full.txt: ncu --set full of this configuration, the 1e7-primary wave"),
 }
 
 
